@@ -1,0 +1,176 @@
+/* dlm.h -- C ABI of the B200-native denoising-step library (libdlm.so).
+ *
+ * One confidence-thresholded denoising step of a masked diffusion language model under approximate
+ * (block-wise, prefix + suffix) KV caching: the GPU work a TeDiServe model instance performs for each
+ * scheduler command.  Citations are to /root/reference/PAPER.md as P:<line>.
+ *
+ *   - the executor command carries "the request prompt and output length (if not already present), the set
+ *     of tokens unmasked in the previous denoising step, and the selected confidence threshold" and
+ *     the reply carries "the newly unmasked tokens and confidence statistics";
+ *   - "cache steps compute only the tokens inside the current cache block, while recompute steps process
+ *     all tokens in the sequence"; here recompute step = dlm_refresh_step, cache step = dlm_cached_step;
+ *   - every step ends by unmasking "tokens whose confidence exceeds a predefined threshold. If no predicted
+ *     tokens have confidence exceeding the threshold, the token with the highest confidence is unmasked";
+ *   - "one-time latency profiling step to measure the per-denoising-step latency for each batch size"
+ *     = dlm_profile_step_costs.
+ *
+ * Conventions.  All functions return 0 (DLM_OK) or a negative DLM_E_* code; dlm_last_error() gives the text.
+ * Nothing is partially applied on error.  Calls are synchronous (results are in the caller's HOST buffers at
+ * return) and a ctx must be used from one thread at a time.  The library owns every device allocation; the
+ * caller owns every host buffer it passes.  Unless stated otherwise pointers are HOST pointers.
+ * There is no CPU fallback: without a CUDA device every compute entry point returns DLM_E_CUDA.
+ */
+#ifndef DLM_H_
+#define DLM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifndef DLM_API
+#define DLM_API __attribute__((visibility("default")))
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DLM_OK          0
+#define DLM_E_ARG      (-1)   /* bad argument (null pointer, length, G % B != 0, unknown request ...) */
+#define DLM_E_CAPACITY (-2)   /* request table, page pool, token budget or caller's result buffer too small */
+#define DLM_E_STATE    (-3)   /* cached step without a valid cache, step on a removed request ...       */
+#define DLM_E_CUDA     (-4)   /* CUDA error or no device                                                */
+
+#define DLM_DTYPE_F32   0
+#define DLM_DTYPE_BF16  1
+
+typedef struct dlm_ctx dlm_ctx;          /* opaque; owns all device memory */
+
+/* Model shape ("arch") and capacities.  Weights are [out, in] row-major; no biases; RMSNorm gains are 1. */
+typedef struct {
+  int32_t n_layers, d_model, n_heads, n_kv_heads, head_dim, d_ffn, vocab, mask_id;
+  int32_t weight_dtype;          /* DLM_DTYPE_F32: fp32 weights, all-fp32 arithmetic (config 1);
+                                    DLM_DTYPE_BF16: bf16 weights, tcgen05 GEMMs, fp32 accumulate/residual */
+  float   logit_scale, rms_eps, rope_theta, init_std;
+  int32_t max_requests;          /* request slots (cf. maxNumSeqPerBatch)                       */
+  int32_t max_seq;               /* longest prompt + generation per request                             */
+  int32_t max_block;             /* largest denoising block length B (<= 64)                            */
+  int32_t kv_page_tokens;        /* tokens per K/V page (64)                                            */
+  int32_t max_batch_tokens;      /* most tokens one step may compute (sum of S_r in a refresh batch)    */
+  int64_t kv_pool_tokens;        /* total tokens the paged K/V store can hold (0 => max_requests*max_seq) */
+} dlm_arch;
+
+/* Optional memory / stream provider: lets the Python harness hand out torch-owned device memory and a torch
+ * stream ("PyTorch only for device memory and streams").  NULL callbacks => cudaMalloc / cudaFree; NULL stream
+ * => a stream the library creates. alloc returns a DEVICE pointer (256-byte aligned) or NULL. */
+typedef struct {
+  void* (*alloc)(size_t bytes, void* user);
+  void  (*free)(void* dev_ptr, void* user);
+  void*  user;
+  void*  cuda_stream;            /* cudaStream_t */
+} dlm_mem;
+
+#define DLM_DRY_RUN 1u           /* compute and report, mutate nothing but the K/V store */
+
+/* One batch of requests for one step. */
+typedef struct {
+  int32_t        n;              /* number of requests                                                  */
+  const int32_t* req;            /* [n] request handles from dlm_request_add, distinct                  */
+  const float*   threshold;      /* [n] or NULL => each request's stored threshold                      */
+  uint32_t       flags;          /* DLM_DRY_RUN                                                         */
+} dlm_batch;
+
+/* Step result, caller-owned host buffers.  Commits are packed request by request in batch order, positions
+ * ascending inside a request; pos is the absolute index in prompt||generation. */
+typedef struct {
+  int32_t* n_committed;          /* [n] out: commits of request i                                       */
+  int32_t* pos;                  /* [capacity] out                                                      */
+  int32_t* tok;                  /* [capacity] out                                                      */
+  float*   conf;                 /* [capacity] out: softmax probability of the committed token          */
+  int32_t  capacity;             /* in: entries available in pos/tok/conf (n*max_block always suffices) */
+  int32_t  total;                /* out: sum of n_committed                                             */
+  int32_t* n_masked_left;        /* [n] out, may be NULL: MASK positions left in the request            */
+  float*   lse;                  /* [n*max_block] out, may be NULL: log-sum-exp of each block row       */
+  float*   row_conf;             /* [n*max_block] out, may be NULL: confidence of each block row        */
+  int32_t* row_tok;              /* [n*max_block] out, may be NULL: predicted token of each block row   */
+} dlm_result;
+
+#define DLM_KIND_REFRESH 0
+#define DLM_KIND_CACHED  1
+/* One row of the per-step cost table (the paper's latencyProfile[tp][batch], tp = 1,
+ * split by step kind as Algorithms 4/5 use it, with the K/V length added). */
+typedef struct { int32_t kind, n_requests, n_tokens, kv_tokens; float usec; } dlm_cost_row;
+
+/* dlm_init: build a model instance; weights are generated ON THE DEVICE from `seed` by the counter-based
+ * definition W in DESIGN.md (the paper gives no weights; BASELINE.json: "random-init ~N(0,0.02) from seed"). */
+DLM_API int  dlm_init(const dlm_arch* arch, uint64_t seed, dlm_ctx** out);
+DLM_API int  dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* mem, dlm_ctx** out);
+DLM_API void dlm_destroy(dlm_ctx* ctx);
+
+/* Register a request: prompt ids [prompt_len] (host), generation of gen_len positions initialised to [MASK]
+ * ("starting from a fully corrupted sequence containing only [MASK] tokens") in blocks of block_len
+ * (P:109).  gen_len % block_len must be 0 (P:380 outputs are rounded up to the block size).  *out_req is the
+ * handle.  dlm_request_set_tokens overwrites prompt||generation ([S] ids, host): it constructs mid-flight state
+ * (the constructed phases of configs 3/5) and applies tokens decided elsewhere (a command carries "the set
+ * of tokens unmasked in the previous denoising step").  keep_cache = 0 invalidates the request's K/V cache;
+ * keep_cache = 1 leaves the K/V store and its validity untouched (the approximate cache tolerates stale K/V by
+ * design) unless the current block changes, which always invalidates. */
+DLM_API int  dlm_request_add(dlm_ctx*, const int32_t* prompt, int32_t prompt_len, int32_t gen_len,
+                     int32_t block_len, float threshold, int32_t* out_req);
+DLM_API int  dlm_request_set_tokens(dlm_ctx*, int32_t req, const int32_t* tokens, int32_t n, int32_t keep_cache);
+DLM_API int  dlm_request_remove(dlm_ctx*, int32_t req);
+DLM_API int  dlm_request_tokens(dlm_ctx*, int32_t req, int32_t* out, int32_t cap);     /* returns S or error    */
+DLM_API int  dlm_request_info(dlm_ctx*, int32_t req, int32_t* cur_block, int32_t* cache_valid, int32_t* n_masked);
+
+/* Recompute step: all S_r positions of every request in the batch pass through the model,
+ * every layer's K (post-RoPE) and V are written to the request's pages, then the current block (the
+ * lowest-index block holding a MASK) is unmasked with the batch's / stored threshold.  Legal at any time;
+ * required at a block's first step.  A finished request commits 0. */
+DLM_API int  dlm_refresh_step(dlm_ctx*, const dlm_batch*, dlm_result*);
+
+/* Cache step: only the current block's B_r positions are computed; they attend, without any
+ * mask, to their own fresh K/V plus the cached K/V of every other position.  per_request_threshold
+ * ([n], may be NULL) overrides batch->threshold, which overrides the stored value (the threshold may
+ * change at every step).  DLM_E_STATE if a request's cache is not valid (new request, block just completed). */
+DLM_API int  dlm_cached_step(dlm_ctx*, const dlm_batch*, const float* per_request_threshold, dlm_result*);
+
+/* One-time latency profiling: times synthetic refresh and cached steps over a grid of (requests,
+ * tokens, K/V length) with CUDA events and fills rows[0..*n_rows).  Uses scratch requests; needs free slots. */
+DLM_API int  dlm_profile_step_costs(dlm_ctx*, dlm_cost_row* rows, int32_t cap, int32_t* n_rows);
+
+/* Options. */
+#define DLM_OPT_SIMPLE_KERNELS 1   /* 1: run the bf16 model through the plain SIMT kernels (on-device debugging
+                                      reference; same rounding points as the tcgen05 path; not a CPU fallback) */
+#define DLM_OPT_DEBUG_DUMP     2   /* 1: keep every stage tensor of the next steps for dlm_debug_tensor      */
+#define DLM_OPT_CUDA_GRAPH     3   /* 1: replay steps of an unchanged batch shape from a captured CUDA graph */
+#define DLM_OPT_FLASH_ATTENTION 4  /* 0: use the plain attention kernel in the bf16 path (debugging)          */
+DLM_API int  dlm_set_option(dlm_ctx*, int32_t key, int32_t value);
+
+/* Stage tensors of the LAST step (needs DLM_OPT_DEBUG_DUMP), as float32 on the host, for the rows the step
+ * computed for `req` (refresh: S rows, cached: B rows), row-major [rows, width].  Returns the number of
+ * floats written or an error.  Stages follow the rounding points of the bf16 path. */
+#define DLM_T_X_IN    0   /* residual stream entering the layer        [rows, d]      fp32 */
+#define DLM_T_NORM1   1   /* RMSNorm(x) fed to the QKV GEMM            [rows, d]           */
+#define DLM_T_Q       2   /* Q after RoPE                              [rows, H*d_h]       */
+#define DLM_T_K       3   /* K after RoPE, as written to the store     [rows, H_kv*d_h]    */
+#define DLM_T_V       4   /* V as written to the store                 [rows, H_kv*d_h]    */
+#define DLM_T_ATTN    5   /* attention output                          [rows, H*d_h]       */
+#define DLM_T_X_MID   6   /* residual after O-proj                     [rows, d]      fp32 */
+#define DLM_T_NORM2   7   /* RMSNorm(x_mid) fed to gate/up             [rows, d]           */
+#define DLM_T_ACT     8   /* silu(gate)*up                             [rows, F]           */
+#define DLM_T_X_OUT   9   /* residual leaving the layer                [rows, d]      fp32 */
+#define DLM_T_FINAL_NORM 10 /* layer ignored: RMSNorm of the block rows fed to the LM head [B, d] */
+#define DLM_T_KCACHE  11  /* the request's stored K for ALL S positions [S, H_kv*d_h]      */
+#define DLM_T_VCACHE  12  /* the request's stored V for ALL S positions [S, H_kv*d_h]      */
+DLM_API int64_t dlm_debug_tensor(dlm_ctx*, int32_t req, int32_t layer, int32_t which, float* out, int64_t cap_floats);
+
+/* Counters: kernels launched by this library since dlm_init (bench.py's gpu_launches). */
+DLM_API int64_t dlm_launch_count(dlm_ctx*);
+/* Device time of the last step in microseconds (CUDA events on the library's stream). */
+DLM_API float dlm_last_step_usec(dlm_ctx*);
+
+DLM_API const char* dlm_last_error(dlm_ctx*);     /* ctx may be NULL: error of the last failed dlm_init        */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DLM_H_ */

@@ -1,0 +1,57 @@
+/* dlm_ops.h -- kernel-level entry points of libdlm.so, for kernel parity tests and micro-benchmarks.
+ * All pointers are DEVICE pointers unless stated; `stream` is a cudaStream_t (NULL = default stream);
+ * calls are asynchronous on that stream.  Return 0 or a negative DLM_E_* code (see dlm.h);
+ * dlm_last_error(NULL) gives the text.
+ */
+#ifndef DLM_OPS_H_
+#define DLM_OPS_H_
+
+#include <stdint.h>
+
+#ifndef DLM_API
+#define DLM_API __attribute__((visibility("default")))
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DLM_EPI_F32    0   /* out fp32  [M, N]                      = A . W^T                              */
+#define DLM_EPI_BF16   1   /* out bf16  [M, N]                      = bf16(A . W^T)                         */
+#define DLM_EPI_RESID  2   /* out fp32  [M, N]                     += A . W^T   (residual stream, a6 / a9)  */
+#define DLM_EPI_SWIGLU 3   /* out bf16  [M, N]: W is [2N, K] (gate rows then up rows); silu(A.Wg^T)*(A.Wu^T) (a8) */
+
+/* tcgen05/TMEM GEMM fed by TMA (rows a3/a6/a8/a9 of DESIGN.md): A bf16 [M, K] row-major, W bf16 [N(or 2N), K]
+ * row-major ([out, in]), fp32 accumulation.  bn = MMA N of the CTA tile (0 = pick automatically; otherwise a
+ * multiple of 32 in [32, 256], multiple of 64 for SwiGLU).  K % 8 == 0 (16-byte rows for TMA). */
+DLM_API int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epilogue,
+                     int32_t bn, void* stream);
+
+/* Same contraction on the plain SIMT kernel (debugging reference of the engine; fp32 out only). */
+DLM_API int dlm_op_gemm_plain_bf16(const void* A, const void* W, float* out, int32_t M, int32_t N, int32_t K, void* stream);
+
+/* Fused LM head (a11 + a12): hidden bf16 [R, K] x W_lm bf16 [V, K] -> per row token = argmax_v z (lowest id on
+ * ties), conf = softmax(z)[token], lse = log sum exp z, z = scale * logits, z[mask_id] = -inf.
+ * Full logits are never written.  scratch: device buffer of dlm_op_lmhead_scratch_bytes(R, V) bytes. */
+DLM_API int64_t dlm_op_lmhead_scratch_bytes(int32_t R, int32_t V);
+DLM_API int dlm_op_lmhead_bf16(const void* hidden, const void* W_lm, int32_t R, int32_t V, int32_t K, float scale,
+                       int32_t mask_id, int32_t* tok, float* conf, float* lse, void* scratch, void* stream);
+
+/* Fused LM head + threshold unmask (a11..a13, config 5 micro-benchmark): n requests x B rows each (R = n*B);
+ * tokens_io int32 [n, B] holds each block's current ids (mask_id = still masked) and is updated in place;
+ * n_committed int32 [n]; commits (pos in block, tok, conf) packed per request with stride B. */
+DLM_API int dlm_op_lmhead_unmask_bf16(const void* hidden, const void* W_lm, int32_t n, int32_t B, int32_t V, int32_t K,
+                              float scale, int32_t mask_id, const float* tau, int32_t* tokens_io,
+                              int32_t* n_committed, int32_t* pos, int32_t* tok, float* conf, void* scratch,
+                              void* stream);
+
+/* Non-causal block attention over a contiguous (unpaged) K/V, bf16 (a5): q [Tq, H, d_h], k/v [S, H_kv, d_h]
+ * -> out [Tq, H, d_h]; softmax_j(q.k_j/sqrt(d_h)) v_j over all j.  flash = 1: tensor-core
+ * online-softmax kernel; 0: plain kernel. */
+DLM_API int dlm_op_attention_bf16(const void* q, const void* k, const void* v, void* out, int32_t Tq, int32_t S,
+                          int32_t H, int32_t H_kv, int32_t d_h, int32_t flash, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DLM_OPS_H_ */

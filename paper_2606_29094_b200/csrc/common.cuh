@@ -1,0 +1,67 @@
+// Shared declarations of the denoising-step engine (device helpers, launch bookkeeping).
+// Part of the CUDA product path; shares nothing with oracle/.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+namespace dlm {
+
+typedef __nv_bfloat16 bf16;
+
+__device__ __forceinline__ float to_f32(float v) { return v; }
+__device__ __forceinline__ float to_f32(bf16 v) { return __bfloat162float(v); }
+template <typename T> __device__ __forceinline__ T from_f32(float v);
+template <> __device__ __forceinline__ float from_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ bf16 from_f32<bf16>(float v) { return __float2bfloat16_rn(v); }
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// Per-step ragged batch descriptor, built on the host, copied once per step (a0 in DESIGN.md).
+// Request i of the batch computes q_len[i] consecutive positions starting at absolute position q_pos0[i];
+// its rows live at [q_off[i], q_off[i]+q_len[i]) of every [T, *] activation buffer.
+struct BatchDesc {
+  int n;             // requests
+  int T;             // computed tokens (sum q_len)
+  int R;             // rows that need logits (sum blk_len)
+  int max_q_len;     // max over requests (attention grid sizing)
+  int max_kv_len;
+  const int* slot;   // [n] request slot (row of tokens / page table)
+  const int* q_off;  // [n]
+  const int* q_len;  // [n]
+  const int* q_pos0; // [n]
+  const int* kv_len; // [n] S_r
+  const int* blk_lo; // [n] absolute position of the current block's first token
+  const int* blk_len;// [n] B_r (0 for a finished request)
+  const int* row_off;// [n] offset of the request's block rows in the [R, *] buffers
+  const float* tau;  // [n]
+  const int* tok_bi; // [T] batch index of each computed token
+};
+
+// Paged K/V store geometry: [layer][page][K|V][H_kv][page_tokens][d_h]
+struct KvGeom {
+  int n_kv_heads, head_dim, page_tokens, max_pages_per_req;
+  long long n_pages;
+  __host__ __device__ long long page_elems() const { return 2LL * n_kv_heads * page_tokens * head_dim; }
+  __host__ __device__ long long offset(int layer, int page, int kv, int head, int tok_in_page) const {
+    return ((((long long)layer * n_pages + page) * 2 + kv) * n_kv_heads + head) * (long long)page_tokens * head_dim +
+           (long long)tok_in_page * head_dim;
+  }
+};
+
+extern long long g_launches;   // kernels launched by this library (dlm_launch_count)
+
+#define DLM_LAUNCH_CHECK() do { ::dlm::g_launches++; } while (0)
+
+}  // namespace dlm

@@ -1,0 +1,1019 @@
+// Host side of libdlm.so: context, request table, paged K/V bookkeeping, the ragged step planner and the
+// extern "C" boundary declared in include/dlm.h and include/dlm_ops.h.  Every step of the path runs in the
+// CUDA kernels of this directory; there is no CPU fallback.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "../../include/dlm.h"
+#include "../../include/dlm_ops.h"
+#include "attn_flash.cuh"
+#include "common.cuh"
+#include "gemm_tc.cuh"
+#include "kernels_basic.cuh"
+
+namespace dlm {
+long long g_launches = 0;
+static std::string g_init_error;
+
+static void set_err(std::string* dst, const char* fmt, ...) {
+  char buf[1024];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  *dst = buf;
+}
+
+#define CU_TRY(ctx_err, expr)                                                                         \
+  do {                                                                                                \
+    cudaError_t e__ = (expr);                                                                         \
+    if (e__ != cudaSuccess) {                                                                         \
+      set_err(ctx_err, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__);   \
+      return DLM_E_CUDA;                                                                              \
+    }                                                                                                 \
+  } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// TMA tensor maps (driver entry point fetched through the runtime, so libcuda is not a link dependency)
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess) fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+// bf16 row-major [rows, cols] matrix, box = box_rows x 64 columns, 128-byte swizzle, OOB reads give zeros.
+static bool make_tmap_bf16(CUtensorMap* m, const void* ptr, long long rows, long long cols, int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)cols * 2};
+  cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+struct TmapCache {
+  std::map<std::tuple<const void*, long long, long long, int>, CUtensorMap> m;
+  const CUtensorMap* get(const void* ptr, long long rows, long long cols, int box_rows) {
+    auto key = std::make_tuple(ptr, rows, cols, box_rows);
+    auto it = m.find(key);
+    if (it != m.end()) return &it->second;
+    CUtensorMap t;
+    if (!make_tmap_bf16(&t, ptr, rows, cols, box_rows)) return nullptr;
+    return &m.emplace(key, t).first->second;
+  }
+};
+
+// ------------------------------------------------------------------------------------------------
+// tcgen05 GEMM launcher
+// ------------------------------------------------------------------------------------------------
+static int g_num_sms = 148;
+
+static int pick_bn(int M, int N, int epi) {
+  // N = output features (SwiGLU: F, each tile covers bn/2).  Aim for one resident wave of equal tiles:
+  // the largest tile that still yields >= ~0.8 * SMs CTAs; when even the smallest cannot, take the smallest.
+  const int m_tiles = (M + 127) / 128;
+  if (epi == EPI_LMHEAD) return 128;
+  static const int cand_std[] = {256, 192, 128, 96, 64, 32};
+  static const int cand_glu[] = {256, 192, 128, 64};
+  const int* cand = epi == EPI_SWIGLU ? cand_glu : cand_std;
+  const int nc = epi == EPI_SWIGLU ? 4 : 6;
+  for (int i = 0; i < nc; ++i) {
+    int per = epi == EPI_SWIGLU ? cand[i] / 2 : cand[i];
+    long long tiles = (long long)m_tiles * ((N + per - 1) / per);
+    if (tiles >= (long long)(g_num_sms * 4) / 5) return cand[i];
+  }
+  return cand[nc - 1];
+}
+
+template <int EPI>
+static cudaError_t launch_gemm_tc_t(const CUtensorMap* ma, const CUtensorMap* mb, const GemmTcParams& p, int n_tiles_x,
+                                    cudaStream_t st) {
+  static int configured = 0;
+  const int smem = gemm_tc_smem_bytes(p.bn, p.stages);
+  if (configured < smem) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    configured = 227 * 1024;
+  }
+  dim3 grid(n_tiles_x, (p.M + 127) / 128);
+  gemm_tc_kernel<EPI><<<grid, kGemmThreads, smem, st>>>(*ma, *mb, p);
+  DLM_LAUNCH_CHECK();
+  return cudaGetLastError();
+}
+
+// A: bf16 [a_rows_cap, K] buffer (M valid rows); W: bf16 [w_rows, K].
+static int gemm_tc(TmapCache& tc, std::string* err, const void* A, long long a_rows_cap, const void* W, long long w_rows,
+                   int M, int N, int K, int epi, int bn, GemmTcParams p, cudaStream_t st) {
+  if (M <= 0) return DLM_OK;
+  if (K % 8) { set_err(err, "gemm_tc: K=%d must be a multiple of 8", K); return DLM_E_ARG; }
+  if (epi != EPI_LMHEAD && p.ldc % 8) { set_err(err, "gemm_tc: output row pitch %lld must be a multiple of 8 elements", p.ldc); return DLM_E_ARG; }
+  if (bn <= 0) bn = pick_bn(M, N, epi);
+  if (bn % 32 || bn < 32 || bn > 256 || (epi == EPI_SWIGLU && bn % 64)) { set_err(err, "gemm_tc: bad bn=%d", bn); return DLM_E_ARG; }
+  p.M = M; p.N = N; p.K = K; p.bn = bn;
+  p.a_box_rows = M <= 32 ? 32 : (M <= 64 ? 64 : 128);
+  const int num_kb = (K + kBK - 1) / kBK;
+  p.stages = std::max(2, std::min(std::min(num_kb, 12), (200 * 1024) / gemm_tc_stage_bytes(bn)));
+  p.w_policy = DLM_L2_EVICT_FIRST;
+  const int per = epi == EPI_SWIGLU ? bn / 2 : bn;
+  const int n_tiles_x = (N + per - 1) / per;
+  if (epi == EPI_LMHEAD && n_tiles_x != p.n_tiles) { set_err(err, "gemm_tc: lm-head tile count mismatch"); return DLM_E_ARG; }
+  const CUtensorMap* ma = tc.get(A, a_rows_cap, K, p.a_box_rows);
+  const CUtensorMap* mb = tc.get(W, w_rows, K, per);
+  if (!ma || !mb) { set_err(err, "cuTensorMapEncodeTiled failed (A=%p rows=%lld K=%d, W=%p rows=%lld box=%d)", A, a_rows_cap, K, W, w_rows, per); return DLM_E_CUDA; }
+  cudaError_t e;
+  switch (epi) {
+    case EPI_F32: e = launch_gemm_tc_t<EPI_F32>(ma, mb, p, n_tiles_x, st); break;
+    case EPI_BF16: e = launch_gemm_tc_t<EPI_BF16>(ma, mb, p, n_tiles_x, st); break;
+    case EPI_RESID: e = launch_gemm_tc_t<EPI_RESID>(ma, mb, p, n_tiles_x, st); break;
+    case EPI_SWIGLU: e = launch_gemm_tc_t<EPI_SWIGLU>(ma, mb, p, n_tiles_x, st); break;
+    case EPI_LMHEAD: e = launch_gemm_tc_t<EPI_LMHEAD>(ma, mb, p, n_tiles_x, st); break;
+    default: set_err(err, "gemm_tc: bad epilogue %d", epi); return DLM_E_ARG;
+  }
+  if (e != cudaSuccess) { set_err(err, "gemm_tc launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+  return DLM_OK;
+}
+
+template <typename TA, typename TW>
+static void gemm_plain(float* C, const TA* A, const TW* W, int M, int N, int K, cudaStream_t st) {
+  if (M <= 0) return;
+  dim3 grid((N + 63) / 64, (M + 63) / 64);
+  gemm_plain_kernel<TA, TW><<<grid, 256, 0, st>>>(C, A, W, M, N, K, K, K, N);
+  DLM_LAUNCH_CHECK();
+}
+
+// Test op: contiguous q/k/v -> repack into a private paged store (64-token pages, identity page table) -> attention.
+__global__ void repack_kv_kernel(bf16* __restrict__ store, const bf16* __restrict__ k, const bf16* __restrict__ v, int S, KvGeom g) {
+  int j = blockIdx.x;
+  int page = j / g.page_tokens, off = j % g.page_tokens;
+  int n = g.n_kv_heads * g.head_dim;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    int h = i / g.head_dim, e = i % g.head_dim;
+    store[g.offset(0, page, 0, h, off) + e] = k[(long long)j * n + i];
+    store[g.offset(0, page, 1, h, off) + e] = v[(long long)j * n + i];
+  }
+}
+
+static int attn_op_contiguous(const void* q, const void* k, const void* v, void* out, int Tq, int S, int H, int Hkv, int dh, int flash,
+                              cudaStream_t st, std::string* err) {
+  if (!q || !k || !v || !out || Tq <= 0 || S <= 0 || H <= 0 || Hkv <= 0 || H % Hkv || dh <= 0 || dh > 256) { set_err(err, "dlm_op_attention_bf16: bad arguments"); return DLM_E_ARG; }
+  KvGeom g;
+  g.n_kv_heads = Hkv; g.head_dim = dh; g.page_tokens = 64; g.max_pages_per_req = (S + 63) / 64; g.n_pages = g.max_pages_per_req;
+  bf16* store = nullptr;
+  int* meta = nullptr;
+  const size_t store_bytes = (size_t)g.n_pages * g.page_elems() * 2;
+  if (cudaMalloc(&store, store_bytes) != cudaSuccess || cudaMalloc(&meta, (size_t)(g.n_pages + 16 + Tq) * 4) != cudaSuccess) { set_err(err, "dlm_op_attention_bf16: allocation failed"); return DLM_E_CAPACITY; }
+  cudaMemsetAsync(store, 0xFF, store_bytes, st);      // NaN pattern in the unused page tail: must not leak into results
+  std::vector<int> h(g.n_pages + 16 + Tq, 0);
+  for (int i = 0; i < g.n_pages; ++i) h[i] = i;
+  int* hd = h.data() + g.n_pages;   // slot, q_off, q_len, q_pos0, kv_len
+  hd[0] = 0; hd[1] = 0; hd[2] = Tq; hd[3] = 0; hd[4] = S;
+  cudaMemcpyAsync(meta, h.data(), h.size() * 4, cudaMemcpyHostToDevice, st);
+  repack_kv_kernel<<<S, 128, 0, st>>>(store, (const bf16*)k, (const bf16*)v, S, g);
+  DLM_LAUNCH_CHECK();
+  BatchDesc bd = {};
+  bd.n = 1; bd.T = Tq; bd.max_q_len = Tq; bd.max_kv_len = S;
+  int* md = meta + g.n_pages;
+  bd.slot = md; bd.q_off = md + 1; bd.q_len = md + 2; bd.q_pos0 = md + 3; bd.kv_len = md + 4; bd.tok_bi = md + 16;
+  const float scale = 1.f / sqrtf((float)dh);
+  int rc = DLM_OK;
+  bool done = false;
+  float* ws = nullptr; size_t wsb = 0;
+  if (flash) {
+    rc = attn_flash_launch((bf16*)out, (const bf16*)q, store, meta, bd, g, 0, H, scale, &ws, &wsb, g_num_sms, st, err, &done);
+    if (!rc && !done) { set_err(err, "dlm_op_attention_bf16: flash kernel does not support d_h=%d", dh); rc = DLM_E_ARG; }
+  } else {
+    attention_plain_kernel<bf16><<<dim3(Tq, H), 128, (size_t)S * 4, st>>>((bf16*)out, (const bf16*)q, store, meta, bd, g, 0, H, scale);
+    DLM_LAUNCH_CHECK();
+  }
+  cudaError_t e = cudaStreamSynchronize(st);
+  cudaFree(store); cudaFree(meta); if (ws) cudaFree(ws);
+  if (!rc && e != cudaSuccess) { set_err(err, "dlm_op_attention_bf16: %s", cudaGetErrorString(e)); rc = DLM_E_CUDA; }
+  return rc;
+}
+
+}  // namespace dlm
+
+using namespace dlm;
+
+// ------------------------------------------------------------------------------------------------
+// Context
+// ------------------------------------------------------------------------------------------------
+struct Req {
+  bool used = false;
+  int P = 0, G = 0, B = 0, S = 0;
+  float tau = 0.9f;
+  int cur_block = 0;          // lowest-index block holding a MASK; == G/B when finished
+  bool cache_valid = false;
+  int n_masked = 0;           // whole request
+  int n_masked_block = 0;     // current block
+  std::vector<int> pages;
+};
+
+struct LayerW { void *wqkv, *wo, *wgu, *wd; };
+
+struct HostBatch {
+  int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0;
+  std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, tok_bi;
+  std::vector<float> tau;
+};
+
+struct dlm_ctx {
+  dlm_arch a;
+  uint64_t seed;
+  dlm_mem mem;
+  bool own_stream = false;
+  cudaStream_t st = nullptr;
+  std::string err;
+  std::vector<void*> allocs;
+  size_t esize = 4;            // bytes per weight / activation element
+  bool bf16_model = false;
+
+  // weights
+  void *E = nullptr, *Wlm = nullptr;
+  std::vector<LayerW> L;
+  float *rope_cos = nullptr, *rope_sin = nullptr;
+  // request state
+  int* tokens = nullptr;       // [max_requests, max_seq]
+  int* page_table = nullptr;   // [max_requests, max_pages_per_req]
+  void* kv_store = nullptr;
+  KvGeom kg;
+  std::vector<Req> reqs;
+  std::vector<int> free_pages;
+  // activations
+  int Tmax = 0, Rmax = 0, n_tiles = 0;
+  float *x = nullptr, *qkv = nullptr, *tmp = nullptr, *logits = nullptr;
+  void *u = nullptr, *q = nullptr, *attn = nullptr, *act = nullptr, *hf = nullptr;
+  RowPartial* part = nullptr;
+  int* row_src = nullptr;
+  // descriptors / results
+  int* desc_dev = nullptr; int* desc_host = nullptr; size_t desc_cap_ints = 0;
+  char* out_dev = nullptr; char* out_host = nullptr; size_t out_bytes = 0;
+  // attention split-KV scratch
+  float* attn_ws = nullptr; size_t attn_ws_bytes = 0;
+  // options
+  int opt_simple = 0, opt_dump = 0, opt_graph = 0, opt_flash = 1;
+  // debug dump
+  std::map<std::pair<int, int>, void*> dump;   // (layer, which) -> device copy [T, width]
+  HostBatch last_batch;
+  bool last_refresh = false;
+  int dump_T = 0;
+  // timing
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  float last_usec = 0.f;
+  TmapCache tmaps;
+
+  void* dalloc(size_t bytes) {
+    void* p = nullptr;
+    bytes = (bytes + 255) & ~(size_t)255;
+    if (mem.alloc) p = mem.alloc(bytes, mem.user);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+    if (p) allocs.push_back(p);
+    return p;
+  }
+  void dfree_all() {
+    for (void* p : allocs) { if (mem.free) mem.free(p, mem.user); else if (!mem.alloc) cudaFree(p); }
+    allocs.clear();
+  }
+};
+
+static int nqkv(const dlm_arch& a) { return (a.n_heads + 2 * a.n_kv_heads) * a.head_dim; }
+
+// ------------------------------------------------------------------------------------------------
+// Init
+// ------------------------------------------------------------------------------------------------
+template <typename TW>
+static void gen_weight(dlm_ctx* c, void* dst, long long n, int tid) {
+  unsigned long long key = mix64(c->seed + DLM_GOLD * (unsigned long long)(tid + 1));
+  float cst = (float)((double)c->a.init_std / sqrt(4294967295.0 / 3.0));
+  int blocks = (int)std::min<long long>((n + 255) / 256, 148 * 16);
+  init_weight_kernel<TW><<<blocks, 256, 0, c->st>>>((TW*)dst, n, key, cst);
+  DLM_LAUNCH_CHECK();
+}
+static void gen_weight_any(dlm_ctx* c, void* dst, long long n, int tid) {
+  if (c->bf16_model) gen_weight<bf16>(c, dst, n, tid); else gen_weight<float>(c, dst, n, tid);
+}
+
+static int validate_arch(const dlm_arch* a, std::string* err) {
+  if (!a) { set_err(err, "arch is NULL"); return DLM_E_ARG; }
+#define REQ(cond) if (!(cond)) { set_err(err, "dlm_init: invalid arch: %s", #cond); return DLM_E_ARG; }
+  REQ(a->n_layers > 0 && a->d_model > 0 && a->n_heads > 0 && a->n_kv_heads > 0 && a->head_dim > 0 && a->d_ffn > 0);
+  REQ(a->vocab > 1 && a->mask_id >= 0 && a->mask_id < a->vocab);
+  REQ(a->n_heads % a->n_kv_heads == 0 && a->head_dim % 2 == 0 && a->head_dim <= 256);
+  REQ(a->weight_dtype == DLM_DTYPE_F32 || a->weight_dtype == DLM_DTYPE_BF16);
+  REQ(a->max_requests > 0 && a->max_seq > 0 && a->max_block > 0 && a->max_block <= 64);
+  REQ(a->kv_page_tokens > 0 && a->max_batch_tokens > 0);
+  if (a->weight_dtype == DLM_DTYPE_BF16) {
+    REQ(a->d_model % 8 == 0 && a->d_ffn % 8 == 0 && (a->n_heads * a->head_dim) % 8 == 0);
+  }
+#undef REQ
+  return DLM_OK;
+}
+
+extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* mem, dlm_ctx** out) {
+  if (!out) { set_err(&g_init_error, "out is NULL"); return DLM_E_ARG; }
+  *out = nullptr;
+  int rc = validate_arch(arch, &g_init_error);
+  if (rc) return rc;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    set_err(&g_init_error, "no CUDA device: libdlm has no CPU fallback");
+    return DLM_E_CUDA;
+  }
+  dlm_ctx* c = new dlm_ctx();
+  c->a = *arch;
+  c->seed = seed;
+  if (mem) c->mem = *mem; else memset(&c->mem, 0, sizeof c->mem);
+  std::string* err = &g_init_error;
+#define FAIL(code, ...) do { set_err(err, __VA_ARGS__); dlm_destroy(c); return code; } while (0)
+  if (c->mem.cuda_stream) c->st = (cudaStream_t)c->mem.cuda_stream;
+  else { if (cudaStreamCreateWithFlags(&c->st, cudaStreamNonBlocking) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaStreamCreate failed"); c->own_stream = true; }
+  cudaDeviceProp prop;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaGetDeviceProperties(&prop, dev);
+  g_num_sms = prop.multiProcessorCount;
+  const dlm_arch& a = c->a;
+  c->bf16_model = a.weight_dtype == DLM_DTYPE_BF16;
+  c->esize = c->bf16_model ? 2 : 4;
+  if (c->bf16_model && prop.major != 10) FAIL(DLM_E_CUDA, "bf16 path needs an sm_100 device (tcgen05/TMA); found sm_%d%d", prop.major, prop.minor);
+  const size_t es = c->esize;
+  const long long d = a.d_model, F = a.d_ffn, V = a.vocab, HQ = (long long)a.n_heads * a.head_dim, NQKV = nqkv(a);
+#define ALLOC(ptr, bytes) do { ptr = (decltype(ptr))c->dalloc((size_t)(bytes)); if (!ptr) FAIL(DLM_E_CAPACITY, "device allocation of %lld bytes failed (%s)", (long long)(bytes), #ptr); } while (0)
+  // ---- weights (Definition W) ----
+  ALLOC(c->E, V * d * es);
+  ALLOC(c->Wlm, V * d * es);
+  gen_weight_any(c, c->E, V * d, 0);
+  gen_weight_any(c, c->Wlm, V * d, 1);
+  c->L.resize(a.n_layers);
+  const long long HKV = (long long)a.n_kv_heads * a.head_dim;
+  for (int l = 0; l < a.n_layers; ++l) {
+    LayerW& w = c->L[l];
+    ALLOC(w.wqkv, NQKV * d * es);
+    ALLOC(w.wo, d * HQ * es);
+    ALLOC(w.wgu, 2 * F * d * es);
+    ALLOC(w.wd, d * F * es);
+    const int t0 = 16 * (l + 1);
+    char* qkv = (char*)w.wqkv;
+    gen_weight_any(c, qkv, HQ * d, t0 + 0);
+    gen_weight_any(c, qkv + HQ * d * es, HKV * d, t0 + 1);
+    gen_weight_any(c, qkv + (HQ + HKV) * d * es, HKV * d, t0 + 2);
+    gen_weight_any(c, w.wo, d * HQ, t0 + 3);
+    gen_weight_any(c, w.wgu, F * d, t0 + 4);
+    gen_weight_any(c, (char*)w.wgu + F * d * es, F * d, t0 + 5);
+    gen_weight_any(c, w.wd, d * F, t0 + 6);
+  }
+  // ---- RoPE table ----
+  const int half = a.head_dim / 2;
+  ALLOC(c->rope_cos, (size_t)a.max_seq * half * 4);
+  ALLOC(c->rope_sin, (size_t)a.max_seq * half * 4);
+  init_rope_kernel<<<(a.max_seq * half + 255) / 256, 256, 0, c->st>>>(c->rope_cos, c->rope_sin, a.max_seq, half, (double)a.rope_theta);
+  DLM_LAUNCH_CHECK();
+  // ---- request state + paged K/V store ----
+  ALLOC(c->tokens, (size_t)a.max_requests * a.max_seq * 4);
+  c->kg.n_kv_heads = a.n_kv_heads; c->kg.head_dim = a.head_dim; c->kg.page_tokens = a.kv_page_tokens;
+  c->kg.max_pages_per_req = (a.max_seq + a.kv_page_tokens - 1) / a.kv_page_tokens;
+  long long pool_tokens = a.kv_pool_tokens > 0 ? a.kv_pool_tokens : (long long)a.max_requests * a.max_seq;
+  c->kg.n_pages = std::min<long long>((pool_tokens + a.kv_page_tokens - 1) / a.kv_page_tokens + a.max_requests,
+                                      (long long)a.max_requests * c->kg.max_pages_per_req);
+  ALLOC(c->page_table, (size_t)a.max_requests * c->kg.max_pages_per_req * 4);
+  ALLOC(c->kv_store, (size_t)a.n_layers * c->kg.n_pages * c->kg.page_elems() * es);
+  cudaMemsetAsync(c->page_table, 0, (size_t)a.max_requests * c->kg.max_pages_per_req * 4, c->st);
+  c->reqs.resize(a.max_requests);
+  for (long long p = c->kg.n_pages - 1; p >= 0; --p) c->free_pages.push_back((int)p);
+  // ---- activations ----
+  c->Tmax = a.max_batch_tokens;
+  c->Rmax = a.max_requests * a.max_block;
+  c->n_tiles = c->bf16_model ? (int)((V + 127) / 128) : 1;
+  ALLOC(c->x, (size_t)c->Tmax * d * 4);
+  ALLOC(c->qkv, (size_t)c->Tmax * NQKV * 4);
+  ALLOC(c->u, (size_t)c->Tmax * d * es);
+  ALLOC(c->q, (size_t)c->Tmax * HQ * es);
+  ALLOC(c->attn, (size_t)c->Tmax * HQ * es);
+  ALLOC(c->act, (size_t)c->Tmax * F * es);
+  ALLOC(c->hf, (size_t)std::max(c->Rmax, 128) * d * es);
+  ALLOC(c->part, (size_t)c->Rmax * std::max(c->n_tiles, 1) * sizeof(RowPartial));
+  ALLOC(c->row_src, (size_t)c->Rmax * 4);
+  c->desc_cap_ints = (size_t)10 * a.max_requests + c->Tmax + 64;
+  ALLOC(c->desc_dev, c->desc_cap_ints * 4);
+  if (cudaMallocHost(&c->desc_host, c->desc_cap_ints * 4) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
+  c->out_bytes = (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6;
+  ALLOC(c->out_dev, c->out_bytes);
+  if (cudaMallocHost(&c->out_host, c->out_bytes) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
+  cudaEventCreate(&c->ev0);
+  cudaEventCreate(&c->ev1);
+  cudaError_t e = cudaStreamSynchronize(c->st);
+  if (e != cudaSuccess) FAIL(DLM_E_CUDA, "weight generation failed: %s", cudaGetErrorString(e));
+#undef ALLOC
+#undef FAIL
+  *out = c;
+  return DLM_OK;
+}
+
+extern "C" int dlm_init(const dlm_arch* arch, uint64_t seed, dlm_ctx** out) { return dlm_init_ex(arch, seed, nullptr, out); }
+
+extern "C" void dlm_destroy(dlm_ctx* c) {
+  if (!c) return;
+  if (c->st) cudaStreamSynchronize(c->st);
+  for (auto& kv : c->dump) cudaFree(kv.second);
+  if (c->tmp) cudaFree(c->tmp);
+  if (c->logits) cudaFree(c->logits);
+  if (c->attn_ws) cudaFree(c->attn_ws);
+  c->dfree_all();
+  if (c->desc_host) cudaFreeHost(c->desc_host);
+  if (c->out_host) cudaFreeHost(c->out_host);
+  if (c->ev0) cudaEventDestroy(c->ev0);
+  if (c->ev1) cudaEventDestroy(c->ev1);
+  if (c->own_stream && c->st) cudaStreamDestroy(c->st);
+  delete c;
+}
+
+extern "C" const char* dlm_last_error(dlm_ctx* c) { return c ? c->err.c_str() : g_init_error.c_str(); }
+extern "C" int64_t dlm_launch_count(dlm_ctx*) { return g_launches; }
+extern "C" float dlm_last_step_usec(dlm_ctx* c) { return c ? c->last_usec : 0.f; }
+
+extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
+  if (!c) return DLM_E_ARG;
+  switch (key) {
+    case DLM_OPT_SIMPLE_KERNELS: c->opt_simple = value; return DLM_OK;
+    case DLM_OPT_DEBUG_DUMP: c->opt_dump = value; return DLM_OK;
+    case DLM_OPT_CUDA_GRAPH: c->opt_graph = value; return DLM_OK;
+    case DLM_OPT_FLASH_ATTENTION: c->opt_flash = value; return DLM_OK;
+  }
+  set_err(&c->err, "unknown option %d", key);
+  return DLM_E_ARG;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Requests
+// ------------------------------------------------------------------------------------------------
+static Req* get_req(dlm_ctx* c, int r) {
+  if (!c || r < 0 || r >= (int)c->reqs.size() || !c->reqs[r].used) return nullptr;
+  return &c->reqs[r];
+}
+
+static void recount(const dlm_arch& a, Req& q, const int* tok) {
+  q.n_masked = 0;
+  q.cur_block = q.G / q.B;
+  q.n_masked_block = 0;
+  for (int b = 0; b < q.G / q.B; ++b) {
+    int m = 0;
+    for (int j = 0; j < q.B; ++j) m += tok[q.P + b * q.B + j] == a.mask_id;
+    q.n_masked += m;
+    if (m && q.cur_block == q.G / q.B) { q.cur_block = b; q.n_masked_block = m; }
+  }
+}
+
+extern "C" int dlm_request_add(dlm_ctx* c, const int32_t* prompt, int32_t P, int32_t G, int32_t B, float tau, int32_t* out_req) {
+  if (!c) return DLM_E_ARG;
+  const dlm_arch& a = c->a;
+  if (!prompt || !out_req || P < 0 || G <= 0 || B <= 0 || B > a.max_block || G % B) {
+    set_err(&c->err, "dlm_request_add: bad arguments (P=%d G=%d B=%d; G %% B must be 0, B <= max_block=%d)", P, G, B, a.max_block);
+    return DLM_E_ARG;
+  }
+  const int S = P + G;
+  if (S > a.max_seq) { set_err(&c->err, "dlm_request_add: S=%d exceeds max_seq=%d", S, a.max_seq); return DLM_E_CAPACITY; }
+  for (int i = 0; i < P; ++i)
+    if (prompt[i] < 0 || prompt[i] >= a.vocab) { set_err(&c->err, "dlm_request_add: prompt id %d out of range", prompt[i]); return DLM_E_ARG; }
+  int slot = -1;
+  for (int i = 0; i < (int)c->reqs.size(); ++i) if (!c->reqs[i].used) { slot = i; break; }
+  if (slot < 0) { set_err(&c->err, "dlm_request_add: all %d request slots in use", a.max_requests); return DLM_E_CAPACITY; }
+  const int need = (S + a.kv_page_tokens - 1) / a.kv_page_tokens;
+  if ((int)c->free_pages.size() < need) { set_err(&c->err, "dlm_request_add: K/V pool exhausted (%d pages needed, %zu free)", need, c->free_pages.size()); return DLM_E_CAPACITY; }
+  Req& q = c->reqs[slot];
+  q = Req();
+  q.used = true; q.P = P; q.G = G; q.B = B; q.S = S; q.tau = tau;
+  q.cur_block = 0; q.cache_valid = false; q.n_masked = G; q.n_masked_block = B;
+  std::vector<int> row(c->kg.max_pages_per_req, 0);
+  for (int i = 0; i < need; ++i) { q.pages.push_back(c->free_pages.back()); c->free_pages.pop_back(); row[i] = q.pages[i]; }
+  std::vector<int> tok(S);
+  for (int i = 0; i < P; ++i) tok[i] = prompt[i];
+  for (int i = P; i < S; ++i) tok[i] = a.mask_id;
+  CU_TRY(&c->err, cudaMemcpyAsync(c->tokens + (size_t)slot * a.max_seq, tok.data(), (size_t)S * 4, cudaMemcpyHostToDevice, c->st));
+  CU_TRY(&c->err, cudaMemcpyAsync(c->page_table + (size_t)slot * c->kg.max_pages_per_req, row.data(), row.size() * 4, cudaMemcpyHostToDevice, c->st));
+  CU_TRY(&c->err, cudaStreamSynchronize(c->st));
+  *out_req = slot;
+  return DLM_OK;
+}
+
+extern "C" int dlm_request_set_tokens(dlm_ctx* c, int32_t r, const int32_t* tokens, int32_t n, int32_t keep_cache) {
+  Req* q = get_req(c, r);
+  if (!q || !tokens) { if (c) set_err(&c->err, "dlm_request_set_tokens: bad request %d", r); return DLM_E_ARG; }
+  if (n != q->S) { set_err(&c->err, "dlm_request_set_tokens: n=%d != S=%d", n, q->S); return DLM_E_ARG; }
+  for (int i = 0; i < n; ++i)
+    if (tokens[i] < 0 || tokens[i] >= c->a.vocab || (i < q->P && tokens[i] == c->a.mask_id)) { set_err(&c->err, "dlm_request_set_tokens: bad id at %d", i); return DLM_E_ARG; }
+  CU_TRY(&c->err, cudaMemcpyAsync(c->tokens + (size_t)r * c->a.max_seq, tokens, (size_t)n * 4, cudaMemcpyHostToDevice, c->st));
+  CU_TRY(&c->err, cudaStreamSynchronize(c->st));
+  const int old_block = q->cur_block;
+  recount(c->a, *q, tokens);
+  if (!keep_cache || q->cur_block != old_block) q->cache_valid = false;
+  return DLM_OK;
+}
+
+extern "C" int dlm_request_remove(dlm_ctx* c, int32_t r) {
+  Req* q = get_req(c, r);
+  if (!q) { if (c) set_err(&c->err, "dlm_request_remove: bad request %d", r); return DLM_E_ARG; }
+  for (int p : q->pages) c->free_pages.push_back(p);
+  *q = Req();
+  return DLM_OK;
+}
+
+extern "C" int dlm_request_tokens(dlm_ctx* c, int32_t r, int32_t* out, int32_t cap) {
+  Req* q = get_req(c, r);
+  if (!q || !out) { if (c) set_err(&c->err, "dlm_request_tokens: bad request %d", r); return DLM_E_ARG; }
+  if (cap < q->S) { set_err(&c->err, "dlm_request_tokens: cap=%d < S=%d", cap, q->S); return DLM_E_CAPACITY; }
+  CU_TRY(&c->err, cudaMemcpyAsync(out, c->tokens + (size_t)r * c->a.max_seq, (size_t)q->S * 4, cudaMemcpyDeviceToHost, c->st));
+  CU_TRY(&c->err, cudaStreamSynchronize(c->st));
+  return q->S;
+}
+
+extern "C" int dlm_request_info(dlm_ctx* c, int32_t r, int32_t* cur_block, int32_t* cache_valid, int32_t* n_masked) {
+  Req* q = get_req(c, r);
+  if (!q) { if (c) set_err(&c->err, "dlm_request_info: bad request %d", r); return DLM_E_ARG; }
+  if (cur_block) *cur_block = q->cur_block;
+  if (cache_valid) *cache_valid = q->cache_valid;
+  if (n_masked) *n_masked = q->n_masked;
+  return DLM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// One step
+// ------------------------------------------------------------------------------------------------
+static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override, bool refresh, HostBatch& hb) {
+  const dlm_arch& a = c->a;
+  if (!b || b->n <= 0 || !b->req) { set_err(&c->err, "step: empty batch"); return DLM_E_ARG; }
+  if (b->n > a.max_requests) { set_err(&c->err, "step: batch of %d exceeds max_requests", b->n); return DLM_E_CAPACITY; }
+  hb = HostBatch();
+  hb.n = b->n;
+  std::vector<char> seen(c->reqs.size(), 0);
+  for (int i = 0; i < b->n; ++i) {
+    int r = b->req[i];
+    Req* q = get_req(c, r);
+    if (!q) { set_err(&c->err, "step: unknown request %d", r); return DLM_E_ARG; }
+    if (seen[r]) { set_err(&c->err, "step: request %d appears twice in the batch", r); return DLM_E_ARG; }
+    seen[r] = 1;
+    const bool done = q->cur_block >= q->G / q->B;
+    if (!refresh && !done && !q->cache_valid) {
+      set_err(&c->err, "dlm_cached_step: request %d has no valid K/V cache (a refresh step is due)", r);
+      return DLM_E_STATE;
+    }
+    const int blk_lo = q->P + std::min(q->cur_block, q->G / q->B - 1) * q->B;
+    int qlen, qpos0;
+    if (refresh) { qlen = q->S; qpos0 = 0; }
+    else { qlen = done ? 0 : q->B; qpos0 = blk_lo; }
+    float tau = thr_override ? thr_override[i] : (b->threshold ? b->threshold[i] : q->tau);
+    hb.slot.push_back(r); hb.q_off.push_back(hb.T); hb.q_len.push_back(qlen); hb.q_pos0.push_back(qpos0);
+    hb.kv_len.push_back(q->S); hb.blk_lo.push_back(blk_lo); hb.blk_len.push_back(done ? 0 : q->B);
+    hb.row_off.push_back(hb.R); hb.tau.push_back(tau);
+    for (int t = 0; t < qlen; ++t) hb.tok_bi.push_back(i);
+    hb.T += qlen; hb.R += done ? 0 : q->B;
+    hb.max_q = std::max(hb.max_q, qlen); hb.max_kv = std::max(hb.max_kv, q->S);
+  }
+  if (hb.T > c->Tmax) { set_err(&c->err, "step: %d tokens exceed max_batch_tokens=%d", hb.T, c->Tmax); return DLM_E_CAPACITY; }
+  return DLM_OK;
+}
+
+static BatchDesc upload_batch(dlm_ctx* c, const HostBatch& hb) {
+  int* h = c->desc_host;
+  const int n = hb.n;
+  size_t o = 0;
+  auto put = [&](const std::vector<int>& v) { memcpy(h + o, v.data(), v.size() * 4); size_t at = o; o += v.size(); return at; };
+  size_t o_slot = put(hb.slot), o_qoff = put(hb.q_off), o_qlen = put(hb.q_len), o_qpos = put(hb.q_pos0), o_kv = put(hb.kv_len),
+         o_lo = put(hb.blk_lo), o_len = put(hb.blk_len), o_row = put(hb.row_off);
+  size_t o_tau = o; memcpy(h + o, hb.tau.data(), n * 4); o += n;
+  size_t o_bi = put(hb.tok_bi);
+  cudaMemcpyAsync(c->desc_dev, h, o * 4, cudaMemcpyHostToDevice, c->st);
+  BatchDesc d;
+  d.n = n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv;
+  d.slot = c->desc_dev + o_slot; d.q_off = c->desc_dev + o_qoff; d.q_len = c->desc_dev + o_qlen; d.q_pos0 = c->desc_dev + o_qpos;
+  d.kv_len = c->desc_dev + o_kv; d.blk_lo = c->desc_dev + o_lo; d.blk_len = c->desc_dev + o_len; d.row_off = c->desc_dev + o_row;
+  d.tau = (const float*)(c->desc_dev + o_tau); d.tok_bi = c->desc_dev + o_bi;
+  return d;
+}
+
+static void dump_stage(dlm_ctx* c, int layer, int which, const void* src, size_t row_bytes, int rows) {
+  if (!c->opt_dump || rows <= 0) return;
+  auto key = std::make_pair(layer, which);
+  void*& p = c->dump[key];
+  if (p) cudaFree(p);
+  p = nullptr;
+  if (cudaMalloc(&p, row_bytes * rows) != cudaSuccess) { p = nullptr; return; }
+  cudaMemcpyAsync(p, src, row_bytes * rows, cudaMemcpyDeviceToDevice, c->st);
+}
+
+template <typename TE>
+static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
+  const dlm_arch& a = c->a;
+  cudaStream_t st = c->st;
+  const int T = bd.T, d = a.d_model, F = a.d_ffn, V = a.vocab, HQ = a.n_heads * a.head_dim, NQKV = nqkv(a);
+  const int HKV = a.n_kv_heads * a.head_dim;
+  const bool tc = c->bf16_model && !c->opt_simple;
+  const float scale = 1.f / sqrtf((float)a.head_dim);
+  std::string* err = &c->err;
+  if (!tc) {   // scratch of the plain path, allocated on first use
+    if (!c->tmp) CU_TRY(err, cudaMalloc(&c->tmp, (size_t)c->Tmax * std::max(d, 2 * F) * 4));
+    if (!c->logits) CU_TRY(err, cudaMalloc(&c->logits, (size_t)c->Rmax * V * 4));
+  }
+  if (T > 0) {
+    embed_kernel<TE><<<T, 256, 0, st>>>(c->x, (const TE*)c->E, c->tokens, a.max_seq, bd, d);
+    DLM_LAUNCH_CHECK();
+  }
+  for (int l = 0; l < a.n_layers && T > 0; ++l) {
+    const LayerW& w = c->L[l];
+    dump_stage(c, l, DLM_T_X_IN, c->x, (size_t)d * 4, T);
+    rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
+    DLM_LAUNCH_CHECK();
+    dump_stage(c, l, DLM_T_NORM1, c->u, (size_t)d * sizeof(TE), T);
+    if (tc) {
+      GemmTcParams p = {};
+      p.out_f32 = c->qkv; p.ldc = NQKV;
+      int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, 0, p, st);
+      if (rc) return rc;
+    } else {
+      gemm_plain<TE, TE>(c->qkv, (const TE*)c->u, (const TE*)w.wqkv, T, NQKV, d, st);
+    }
+    rope_kv_write_kernel<TE><<<T, 256, 0, st>>>((TE*)c->q, (TE*)c->kv_store, c->qkv, c->rope_cos, c->rope_sin, c->page_table, bd, c->kg, l, a.n_heads);
+    DLM_LAUNCH_CHECK();
+    dump_stage(c, l, DLM_T_Q, c->q, (size_t)HQ * sizeof(TE), T);
+    bool flash_done = false;
+    if (tc && c->opt_flash) {
+      int rc = attn_flash_launch((bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, c->page_table, bd, c->kg, l,
+                                 a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, err, &flash_done);
+      if (rc) return rc;
+    }
+    if (!flash_done) {
+      attention_plain_kernel<TE><<<dim3(T, a.n_heads), 128, (size_t)bd.max_kv_len * 4, st>>>(
+          (TE*)c->attn, (const TE*)c->q, (const TE*)c->kv_store, c->page_table, bd, c->kg, l, a.n_heads, scale);
+      DLM_LAUNCH_CHECK();
+    }
+    dump_stage(c, l, DLM_T_ATTN, c->attn, (size_t)HQ * sizeof(TE), T);
+    if (tc) {
+      GemmTcParams p = {};
+      p.out_f32 = c->x; p.ldc = d;
+      int rc = gemm_tc(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, EPI_RESID, 0, p, st);
+      if (rc) return rc;
+    } else {
+      gemm_plain<TE, TE>(c->tmp, (const TE*)c->attn, (const TE*)w.wo, T, d, HQ, st);
+      add_residual_kernel<<<(unsigned)(((long long)T * d + 255) / 256), 256, 0, st>>>(c->x, c->tmp, (long long)T * d);
+      DLM_LAUNCH_CHECK();
+    }
+    dump_stage(c, l, DLM_T_X_MID, c->x, (size_t)d * 4, T);
+    rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
+    DLM_LAUNCH_CHECK();
+    dump_stage(c, l, DLM_T_NORM2, c->u, (size_t)d * sizeof(TE), T);
+    if (tc) {
+      GemmTcParams p = {};
+      p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F;
+      int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, EPI_SWIGLU, 0, p, st);
+      if (rc) return rc;
+    } else {
+      gemm_plain<TE, TE>(c->tmp, (const TE*)c->u, (const TE*)w.wgu, T, 2 * F, d, st);
+      swiglu_kernel<TE><<<(unsigned)(((long long)T * F + 255) / 256), 256, 0, st>>>((TE*)c->act, c->tmp, T, F);
+      DLM_LAUNCH_CHECK();
+    }
+    dump_stage(c, l, DLM_T_ACT, c->act, (size_t)F * sizeof(TE), T);
+    if (tc) {
+      GemmTcParams p = {};
+      p.out_f32 = c->x; p.ldc = d;
+      int rc = gemm_tc(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, EPI_RESID, 0, p, st);
+      if (rc) return rc;
+    } else {
+      gemm_plain<TE, TE>(c->tmp, (const TE*)c->act, (const TE*)w.wd, T, d, F, st);
+      add_residual_kernel<<<(unsigned)(((long long)T * d + 255) / 256), 256, 0, st>>>(c->x, c->tmp, (long long)T * d);
+      DLM_LAUNCH_CHECK();
+    }
+    dump_stage(c, l, DLM_T_X_OUT, c->x, (size_t)d * 4, T);
+  }
+  // ---- head: a10 final norm on the block rows, a11 LM head statistics, a12+a13 combine + unmask ----
+  const int R = bd.R;
+  StepOut so;
+  char* ob = c->out_dev;
+  so.n_committed = (int*)ob; ob += (size_t)a.max_requests * 4;
+  const size_t rb = (size_t)c->Rmax * 4;
+  so.pos = (int*)ob; ob += rb; so.tok = (int*)ob; ob += rb; so.conf = (float*)ob; ob += rb;
+  so.row_lse = (float*)ob; ob += rb; so.row_conf = (float*)ob; ob += rb; so.row_tok = (int*)ob;
+  int n_tiles = 1;
+  if (R > 0) {
+    build_row_src_kernel<<<bd.n, 64, 0, st>>>(c->row_src, bd);
+    DLM_LAUNCH_CHECK();
+    rmsnorm_kernel<TE><<<R, 256, 0, st>>>((TE*)c->hf, c->x, c->row_src, d, a.rms_eps);
+    DLM_LAUNCH_CHECK();
+    dump_stage(c, 0, DLM_T_FINAL_NORM, c->hf, (size_t)d * sizeof(TE), R);
+    if (tc) {
+      n_tiles = c->n_tiles;
+      GemmTcParams p = {};
+      p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale;
+      int rc = gemm_tc(c->tmaps, err, c->hf, std::max(c->Rmax, 128), c->Wlm, V, R, V, d, EPI_LMHEAD, 128, p, st);
+      if (rc) return rc;
+    } else {
+      gemm_plain<TE, TE>(c->logits, (const TE*)c->hf, (const TE*)c->Wlm, R, V, d, st);
+      row_stats_plain_kernel<<<R, 256, 0, st>>>(c->part, c->logits, V, a.mask_id, a.logit_scale);
+      DLM_LAUNCH_CHECK();
+    }
+  }
+  combine_unmask_kernel<<<bd.n, 128, 0, st>>>(so, c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd, dry_run ? 1 : 0);
+  DLM_LAUNCH_CHECK();
+  CU_TRY(err, cudaGetLastError());
+  return DLM_OK;
+}
+
+static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, dlm_result* res, bool refresh) {
+  if (!c) return DLM_E_ARG;
+  if (!res || !res->n_committed || !res->pos || !res->tok || !res->conf) { set_err(&c->err, "step: result buffers missing"); return DLM_E_ARG; }
+  HostBatch hb;
+  int rc = build_batch(c, b, thr_override, refresh, hb);
+  if (rc) return rc;
+  const dlm_arch& a = c->a;
+  const bool dry = (b->flags & DLM_DRY_RUN) != 0;
+  if (res->capacity < hb.R) { set_err(&c->err, "step: result capacity %d < %d block rows", res->capacity, hb.R); return DLM_E_CAPACITY; }
+  std::string* err = &c->err;
+  CU_TRY(err, cudaEventRecord(c->ev0, c->st));
+  BatchDesc bd = upload_batch(c, hb);
+  rc = c->bf16_model ? forward<bf16>(c, bd, dry) : forward<float>(c, bd, dry);
+  if (rc) { cudaStreamSynchronize(c->st); return rc; }
+  CU_TRY(err, cudaMemcpyAsync(c->out_host, c->out_dev, c->out_bytes, cudaMemcpyDeviceToHost, c->st));
+  CU_TRY(err, cudaEventRecord(c->ev1, c->st));
+  CU_TRY(err, cudaStreamSynchronize(c->st));
+  cudaEventElapsedTime(&c->last_usec, c->ev0, c->ev1);
+  c->last_usec *= 1000.f;
+  // ---- unpack, update host-side request state ----
+  const char* ob = c->out_host;
+  const int* n_comm = (const int*)ob; ob += (size_t)a.max_requests * 4;
+  const size_t rb = (size_t)c->Rmax * 4;
+  const int* pos = (const int*)ob; ob += rb; const int* tok = (const int*)ob; ob += rb; const float* conf = (const float*)ob; ob += rb;
+  const float* rlse = (const float*)ob; ob += rb; const float* rconf = (const float*)ob; ob += rb; const int* rtok = (const int*)ob;
+  int total = 0;
+  for (int i = 0; i < hb.n; ++i) {
+    Req& q = c->reqs[hb.slot[i]];
+    const int k = hb.blk_len[i] ? n_comm[i] : 0;
+    res->n_committed[i] = k;
+    for (int j = 0; j < k; ++j) {
+      res->pos[total + j] = pos[i * a.max_block + j];
+      res->tok[total + j] = tok[i * a.max_block + j];
+      res->conf[total + j] = conf[i * a.max_block + j];
+    }
+    total += k;
+    for (int j = 0; j < a.max_block; ++j) {
+      const bool v = j < hb.blk_len[i];
+      if (res->lse) res->lse[i * a.max_block + j] = v ? rlse[i * a.max_block + j] : 0.f;
+      if (res->row_conf) res->row_conf[i * a.max_block + j] = v ? rconf[i * a.max_block + j] : 0.f;
+      if (res->row_tok) res->row_tok[i * a.max_block + j] = v ? rtok[i * a.max_block + j] : -1;
+    }
+    if (refresh && hb.blk_len[i]) q.cache_valid = true;      // K/V of all positions now match the pre-step tokens
+    if (!dry && hb.blk_len[i]) {
+      q.n_masked -= k; q.n_masked_block -= k;
+      if (q.n_masked_block == 0) {                            // P:109 block complete -> recompute before the next block
+        q.cache_valid = false;
+        q.cur_block++;
+        q.n_masked_block = q.cur_block < q.G / q.B ? q.B : 0;
+      }
+    }
+    if (res->n_masked_left) res->n_masked_left[i] = q.n_masked;
+  }
+  res->total = total;
+  c->last_batch = hb;
+  c->last_refresh = refresh;
+  return DLM_OK;
+}
+
+extern "C" int dlm_refresh_step(dlm_ctx* c, const dlm_batch* b, dlm_result* r) { return run_step(c, b, nullptr, r, true); }
+extern "C" int dlm_cached_step(dlm_ctx* c, const dlm_batch* b, const float* thr, dlm_result* r) { return run_step(c, b, thr, r, false); }
+
+// ------------------------------------------------------------------------------------------------
+// Debug tensors
+// ------------------------------------------------------------------------------------------------
+static void to_f32_host(const void* src, float* dst, size_t n, bool is_bf16) {
+  if (!is_bf16) { memcpy(dst, src, n * 4); return; }
+  const uint16_t* s = (const uint16_t*)src;
+  for (size_t i = 0; i < n; ++i) { uint32_t u = (uint32_t)s[i] << 16; memcpy(dst + i, &u, 4); }
+}
+
+extern "C" int64_t dlm_debug_tensor(dlm_ctx* c, int32_t r, int32_t layer, int32_t which, float* out, int64_t cap) {
+  Req* q = get_req(c, r);
+  if (!q || !out) { if (c) set_err(&c->err, "dlm_debug_tensor: bad request %d", r); return DLM_E_ARG; }
+  const dlm_arch& a = c->a;
+  const int HQ = a.n_heads * a.head_dim, HKV = a.n_kv_heads * a.head_dim;
+  if (which == DLM_T_KCACHE || which == DLM_T_VCACHE) {
+    if (layer < 0 || layer >= a.n_layers) { set_err(&c->err, "dlm_debug_tensor: bad layer"); return DLM_E_ARG; }
+    const int64_t n = (int64_t)q->S * HKV;
+    if (cap < n) { set_err(&c->err, "dlm_debug_tensor: cap too small"); return DLM_E_CAPACITY; }
+    std::vector<char> page((size_t)c->kg.page_elems() * c->esize);
+    const int PT = a.kv_page_tokens, kv = which == DLM_T_VCACHE;
+    for (int pi = 0; pi * PT < q->S; ++pi) {
+      const char* src = (const char*)c->kv_store + (size_t)c->kg.offset(layer, q->pages[pi], 0, 0, 0) * c->esize;
+      if (cudaMemcpy(page.data(), src, page.size(), cudaMemcpyDeviceToHost) != cudaSuccess) { set_err(&c->err, "dlm_debug_tensor: copy failed"); return DLM_E_CUDA; }
+      for (int h = 0; h < a.n_kv_heads; ++h)
+        for (int t = 0; t < PT && pi * PT + t < q->S; ++t) {
+          size_t so = ((size_t)(kv * a.n_kv_heads + h) * PT + t) * a.head_dim;
+          to_f32_host(page.data() + so * c->esize, out + ((size_t)(pi * PT + t) * HKV + (size_t)h * a.head_dim), a.head_dim, c->bf16_model);
+        }
+    }
+    return n;
+  }
+  // stage tensors of the last step
+  int bi = -1;
+  for (int i = 0; i < c->last_batch.n; ++i) if (c->last_batch.slot[i] == r) bi = i;
+  if (bi < 0) { set_err(&c->err, "dlm_debug_tensor: request %d was not in the last step", r); return DLM_E_STATE; }
+  int width, rows, off;
+  bool f32 = false;
+  switch (which) {
+    case DLM_T_X_IN: case DLM_T_X_MID: case DLM_T_X_OUT: width = a.d_model; f32 = true; break;
+    case DLM_T_NORM1: case DLM_T_NORM2: case DLM_T_FINAL_NORM: width = a.d_model; break;
+    case DLM_T_Q: case DLM_T_ATTN: width = HQ; break;
+    case DLM_T_ACT: width = a.d_ffn; break;
+    default: set_err(&c->err, "dlm_debug_tensor: unsupported tensor %d", which); return DLM_E_ARG;
+  }
+  if (which == DLM_T_FINAL_NORM) { rows = c->last_batch.blk_len[bi]; off = c->last_batch.row_off[bi]; layer = 0; }
+  else { rows = c->last_batch.q_len[bi]; off = c->last_batch.q_off[bi]; }
+  auto it = c->dump.find(std::make_pair(layer, which));
+  if (it == c->dump.end() || !it->second) { set_err(&c->err, "dlm_debug_tensor: nothing dumped for layer %d tensor %d (set DLM_OPT_DEBUG_DUMP before the step)", layer, which); return DLM_E_STATE; }
+  const int64_t n = (int64_t)rows * width;
+  if (cap < n) { set_err(&c->err, "dlm_debug_tensor: cap too small"); return DLM_E_CAPACITY; }
+  const size_t es = f32 ? 4 : c->esize;
+  std::vector<char> buf((size_t)n * es);
+  if (cudaMemcpy(buf.data(), (const char*)it->second + (size_t)off * width * es, buf.size(), cudaMemcpyDeviceToHost) != cudaSuccess) { set_err(&c->err, "dlm_debug_tensor: copy failed"); return DLM_E_CUDA; }
+  to_f32_host(buf.data(), out, (size_t)n, !f32 && c->bf16_model);
+  return n;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a15  cost table (P:123 one-time latency profiling; P:599-618 LP[tp][tokens], tp = 1)
+// ------------------------------------------------------------------------------------------------
+extern "C" int dlm_profile_step_costs(dlm_ctx* c, dlm_cost_row* rows, int32_t cap, int32_t* n_rows) {
+  if (!c || !rows || !n_rows) return DLM_E_ARG;
+  const dlm_arch& a = c->a;
+  *n_rows = 0;
+  const int B = std::min(32, a.max_block);
+  static const int kv_lens[] = {512, 1024, 2048, 4608};
+  static const int ns[] = {1, 2, 4, 8, 16, 32, 64};
+  int free_slots = 0;
+  for (auto& q : c->reqs) free_slots += !q.used;
+  std::vector<int32_t> n_comm(a.max_requests), pos(c->Rmax), tok(c->Rmax);
+  std::vector<float> conf(c->Rmax);
+  dlm_result res = {};
+  res.n_committed = n_comm.data(); res.pos = pos.data(); res.tok = tok.data(); res.conf = conf.data(); res.capacity = c->Rmax;
+  const int reps = 5;
+  for (int kv : kv_lens) {
+    if (kv > a.max_seq) continue;
+    for (int n : ns) {
+      if (n > free_slots || (long long)n * kv > c->Tmax) continue;
+      if ((long long)n * ((kv + a.kv_page_tokens - 1) / a.kv_page_tokens) > (long long)c->free_pages.size()) continue;
+      if (*n_rows + 2 > cap) return DLM_OK;
+      std::vector<int32_t> ids;
+      std::vector<int32_t> prompt(kv - B);
+      for (int i = 0; i < n; ++i) {
+        for (int j = 0; j < kv - B; ++j) prompt[j] = (int32_t)(mix64(0x5eedULL + 977ULL * i + j) % (unsigned)(a.vocab - 1));
+        for (auto& t : prompt) if (t >= a.mask_id) t++;
+        int32_t id;
+        int rc = dlm_request_add(c, prompt.data(), kv - B, B, B, 2.0f, &id);
+        if (rc) { for (int r : ids) dlm_request_remove(c, r); return rc; }
+        ids.push_back(id);
+      }
+      dlm_batch b = {n, ids.data(), nullptr, DLM_DRY_RUN};
+      float best_r = 1e30f, best_c = 1e30f;
+      int rc = DLM_OK;
+      for (int it = 0; it < reps + 1 && !rc; ++it) {
+        rc = dlm_refresh_step(c, &b, &res);
+        if (it) best_r = std::min(best_r, c->last_usec);
+      }
+      for (int it = 0; it < reps + 1 && !rc; ++it) {
+        rc = dlm_cached_step(c, &b, nullptr, &res);
+        if (it) best_c = std::min(best_c, c->last_usec);
+      }
+      for (int r : ids) dlm_request_remove(c, r);
+      if (rc) return rc;
+      rows[*n_rows] = {DLM_KIND_REFRESH, n, n * kv, kv, best_r}; (*n_rows)++;
+      rows[*n_rows] = {DLM_KIND_CACHED, n, n * B, kv, best_c}; (*n_rows)++;
+    }
+  }
+  return DLM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Kernel-level entry points (include/dlm_ops.h)
+// ------------------------------------------------------------------------------------------------
+static TmapCache g_op_tmaps;
+
+static int op_check_device() {
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    set_err(&g_init_error, "no CUDA device: libdlm has no CPU fallback");
+    return DLM_E_CUDA;
+  }
+  static bool init = false;
+  if (!init) { cudaDeviceProp p; int d = 0; cudaGetDevice(&d); cudaGetDeviceProperties(&p, d); g_num_sms = p.multiProcessorCount; init = true; }
+  return DLM_OK;
+}
+
+extern "C" int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epi, int32_t bn, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!A || !W || !out || M <= 0 || N <= 0 || K <= 0 || epi < 0 || epi > 3) { set_err(&g_init_error, "dlm_op_gemm_bf16: bad arguments"); return DLM_E_ARG; }
+  GemmTcParams p = {};
+  p.ldc = N;
+  p.up_row0 = N;
+  if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
+  g_op_tmaps.m.clear();   // caller buffers come and go; never reuse a stale map
+  return gemm_tc(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, (cudaStream_t)stream);
+}
+
+extern "C" int dlm_op_gemm_plain_bf16(const void* A, const void* W, float* out, int32_t M, int32_t N, int32_t K, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!A || !W || !out || M <= 0 || N <= 0 || K <= 0) { set_err(&g_init_error, "dlm_op_gemm_plain_bf16: bad arguments"); return DLM_E_ARG; }
+  gemm_plain<bf16, bf16>(out, (const bf16*)A, (const bf16*)W, M, N, K, (cudaStream_t)stream);
+  return cudaGetLastError() == cudaSuccess ? DLM_OK : DLM_E_CUDA;
+}
+
+extern "C" int64_t dlm_op_lmhead_scratch_bytes(int32_t R, int32_t V) {
+  return (int64_t)std::max(R, 1) * ((V + 127) / 128) * (int64_t)sizeof(RowPartial) + (int64_t)R * 64 + 4096;
+}
+
+// batch descriptor for the stand-alone head ops: n requests of B rows, block = positions [0, B) of a private token row
+static int op_head(const void* hidden, const void* Wlm, int n, int B, int V, int K, float scale, int mask_id, const float* tau,
+                   int* tokens_io, StepOut so, void* scratch, cudaStream_t st, int dry) {
+  const int R = n * B;
+  const int n_tiles = (V + 127) / 128;
+  RowPartial* part = (RowPartial*)scratch;
+  int* meta = (int*)((char*)scratch + (size_t)R * n_tiles * sizeof(RowPartial));
+  // meta: slot[n], blk_lo[n], blk_len[n], row_off[n]  (+ tau passed separately)
+  std::vector<int> h(4 * n);
+  for (int i = 0; i < n; ++i) { h[i] = i; h[n + i] = 0; h[2 * n + i] = B; h[3 * n + i] = i * B; }
+  cudaMemcpyAsync(meta, h.data(), h.size() * 4, cudaMemcpyHostToDevice, st);
+  cudaStreamSynchronize(st);   // h is a stack-lifetime staging buffer
+  GemmTcParams p = {};
+  p.part = part; p.n_tiles = n_tiles; p.mask_id = mask_id; p.scale = scale;
+  g_op_tmaps.m.clear();
+  int rc = gemm_tc(g_op_tmaps, &g_init_error, hidden, R, Wlm, V, R, V, K, EPI_LMHEAD, 128, p, st);
+  if (rc) return rc;
+  BatchDesc bd = {};
+  bd.n = n; bd.R = R; bd.slot = meta; bd.blk_lo = meta + n; bd.blk_len = meta + 2 * n; bd.row_off = meta + 3 * n; bd.tau = tau;
+  combine_unmask_kernel<<<n, 128, 0, st>>>(so, part, n_tiles, tokens_io, B, B, mask_id, bd, dry);
+  DLM_LAUNCH_CHECK();
+  return cudaGetLastError() == cudaSuccess ? DLM_OK : DLM_E_CUDA;
+}
+
+extern "C" int dlm_op_lmhead_unmask_bf16(const void* hidden, const void* Wlm, int32_t n, int32_t B, int32_t V, int32_t K, float scale,
+                                          int32_t mask_id, const float* tau, int32_t* tokens_io, int32_t* n_committed, int32_t* pos,
+                                          int32_t* tok, float* conf, void* scratch, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!hidden || !Wlm || !tau || !tokens_io || !n_committed || !pos || !tok || !conf || !scratch || n <= 0 || B <= 0 || B > 64 || K % 8) {
+    set_err(&g_init_error, "dlm_op_lmhead_unmask_bf16: bad arguments"); return DLM_E_ARG;
+  }
+  // row statistics land after the metadata in scratch
+  const int R = n * B;
+  char* extra = (char*)scratch + (size_t)R * ((V + 127) / 128) * sizeof(RowPartial) + (size_t)16 * n + 256;
+  StepOut so;
+  so.n_committed = n_committed; so.pos = pos; so.tok = tok; so.conf = conf;
+  so.row_lse = (float*)extra; so.row_conf = (float*)extra + R; so.row_tok = (int*)extra + 2 * R;
+  return op_head(hidden, Wlm, n, B, V, K, scale, mask_id, tau, tokens_io, so, scratch, (cudaStream_t)stream, 0);
+}
+
+extern "C" int dlm_op_lmhead_bf16(const void* hidden, const void* Wlm, int32_t R, int32_t V, int32_t K, float scale, int32_t mask_id,
+                                   int32_t* tok, float* conf, float* lse, void* scratch, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!hidden || !Wlm || !tok || !conf || !lse || !scratch || R <= 0 || K % 8) { set_err(&g_init_error, "dlm_op_lmhead_bf16: bad arguments"); return DLM_E_ARG; }
+  // every row is its own "request" of one block row; commits are discarded (dry run), only row stats are kept
+  const int n_tiles = (V + 127) / 128;
+  char* extra = (char*)scratch + (size_t)R * n_tiles * sizeof(RowPartial) + (size_t)16 * R + 256;
+  int* dummy = (int*)extra;                 // n_committed[R], pos[R], tok[R], conf[R], tokens[R], tau[R]
+  StepOut so;
+  so.n_committed = dummy; so.pos = dummy + R; so.tok = dummy + 2 * R; so.conf = (float*)(dummy + 3 * R);
+  so.row_lse = lse; so.row_conf = conf; so.row_tok = tok;
+  int* tokens = dummy + 4 * R;
+  float* tau = (float*)(dummy + 5 * R);
+  cudaMemsetAsync(tokens, 0, (size_t)R * 4, (cudaStream_t)stream);
+  cudaMemsetAsync(tau, 0, (size_t)R * 4, (cudaStream_t)stream);
+  return op_head(hidden, Wlm, R, 1, V, K, scale, mask_id, tau, tokens, so, scratch, (cudaStream_t)stream, 1);
+}
+
+extern "C" int dlm_op_attention_bf16(const void* q, const void* k, const void* v, void* out, int32_t Tq, int32_t S, int32_t H,
+                                      int32_t Hkv, int32_t dh, int32_t flash, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  return attn_op_contiguous(q, k, v, out, Tq, S, H, Hkv, dh, flash, (cudaStream_t)stream, &g_init_error);
+}

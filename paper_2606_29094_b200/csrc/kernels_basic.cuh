@@ -1,0 +1,362 @@
+// Plain CUDA kernels of the denoising step: weight generation (Definition W), embedding gather, RMSNorm,
+// RoPE + paged K/V write, SIMT GEMM / attention (the all-fp32 path of config 1 and the on-device debugging
+// reference of the bf16 path), SwiGLU, residual add, LM-head row statistics, combine + threshold unmask.
+// Row numbers a0..a13 refer to DESIGN.md's hot-path table.
+#pragma once
+#include <math_constants.h>
+
+#include "common.cuh"
+
+namespace dlm {
+
+// ------------------------------------------------------------------------------------------------
+// Definition W: counter-based weight generation, bit-identical to the written definition.
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  return z ^ (z >> 31);
+}
+#define DLM_GOLD 0x9E3779B97F4A7C15ULL
+
+template <typename TW>
+__global__ void init_weight_kernel(TW* __restrict__ w, long long n, unsigned long long key, float c) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long stride = (long long)gridDim.x * blockDim.x;
+  for (; i < n; i += stride) {
+    unsigned long long h = mix64(key + DLM_GOLD * (unsigned long long)(i + 1));
+    int s = (int)(h & 0xFFFF) + (int)((h >> 16) & 0xFFFF) + (int)((h >> 32) & 0xFFFF) + (int)(h >> 48) - 131070;
+    w[i] = from_f32<TW>(__fmul_rn((float)s, c));
+  }
+}
+
+// RoPE table: cos/sin(pos * theta^(-2i/d_h)) computed in double, stored fp32. [max_seq, d_h/2]
+__global__ void init_rope_kernel(float* __restrict__ cs, float* __restrict__ sn, int max_seq, int half, double theta) {
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= max_seq * half) return;
+  int pos = idx / half, i = idx % half;
+  double ang = (double)pos * pow(theta, -2.0 * (double)i / (double)(2 * half));
+  cs[idx] = (float)cos(ang);
+  sn[idx] = (float)sin(ang);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1  embedding gather: x[t, :] = E[token_t, :]   (residual stream is fp32 in both paths)
+// ------------------------------------------------------------------------------------------------
+template <typename TW>
+__global__ void embed_kernel(float* __restrict__ x, const TW* __restrict__ E, const int* __restrict__ tokens,
+                             int max_seq, BatchDesc b, int d) {
+  int t = blockIdx.x;
+  int bi = b.tok_bi[t];
+  int pos = b.q_pos0[bi] + (t - b.q_off[bi]);
+  int tok = tokens[(long long)b.slot[bi] * max_seq + pos];
+  const TW* e = E + (long long)tok * d;
+  float* xr = x + (long long)t * d;
+  for (int i = threadIdx.x; i < d; i += blockDim.x) xr[i] = to_f32(e[i]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2/a7/a10  RMSNorm: u = x * rsqrt(mean(x^2) + eps), gains 1.  One block per row.  row_src (optional)
+// gathers rows (a10: the block rows of each request).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float block_sum(float v, float* red) {
+  v = warp_sum(v);
+  int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  __syncthreads();
+  if (l == 0) red[w] = v;
+  __syncthreads();
+  float t = (threadIdx.x < (blockDim.x >> 5)) ? red[threadIdx.x] : 0.f;
+  if (w == 0) { t = warp_sum(t); if (l == 0) red[0] = t; }
+  __syncthreads();
+  return red[0];
+}
+
+template <typename TA>
+__global__ void rmsnorm_kernel(TA* __restrict__ u, const float* __restrict__ x, const int* __restrict__ row_src,
+                               int d, float eps) {
+  __shared__ float red[33];
+  int r = blockIdx.x;
+  const float* xr = x + (long long)(row_src ? row_src[r] : r) * d;
+  float ss = 0.f;
+  for (int i = threadIdx.x; i < d; i += blockDim.x) { float v = xr[i]; ss += v * v; }
+  ss = block_sum(ss, red);
+  float rs = rsqrtf(ss / (float)d + eps);
+  TA* ur = u + (long long)r * d;
+  for (int i = threadIdx.x; i < d; i += blockDim.x) ur[i] = from_f32<TA>(xr[i] * rs);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4  RoPE + K/V write.  qkv fp32 [T, (H+2H_kv) d_h] -> q [T, H d_h] (TA), K (rotated) and V into the pages.
+// Half-split pairing (i, i + d_h/2), angle = pos * theta^(-2i/d_h) from the table.  One block per token.
+// ------------------------------------------------------------------------------------------------
+template <typename TA>
+__global__ void rope_kv_write_kernel(TA* __restrict__ q, TA* __restrict__ kv_store, const float* __restrict__ qkv,
+                                     const float* __restrict__ rope_cos, const float* __restrict__ rope_sin,
+                                     const int* __restrict__ page_table, BatchDesc b, KvGeom g, int layer,
+                                     int n_heads) {
+  int t = blockIdx.x;
+  int bi = b.tok_bi[t];
+  int pos = b.q_pos0[bi] + (t - b.q_off[bi]);
+  int dh = g.head_dim, half = dh >> 1;
+  int nq = n_heads * dh, nkv = g.n_kv_heads * dh;
+  const float* row = qkv + (long long)t * (nq + 2 * nkv);
+  const float* cs = rope_cos + (long long)pos * half;
+  const float* sn = rope_sin + (long long)pos * half;
+  int page = page_table[(long long)b.slot[bi] * g.max_pages_per_req + pos / g.page_tokens];
+  int off = pos % g.page_tokens;
+  // Q and K: one thread per (head, i) pair
+  for (int p = threadIdx.x; p < (n_heads + g.n_kv_heads) * half; p += blockDim.x) {
+    int h = p / half, i = p % half;
+    float a = row[h * dh + i], c = row[h * dh + i + half];
+    float ra = a * cs[i] - c * sn[i];
+    float rc = c * cs[i] + a * sn[i];
+    if (h < n_heads) {
+      TA* qo = q + (long long)t * nq + h * dh;
+      qo[i] = from_f32<TA>(ra);
+      qo[i + half] = from_f32<TA>(rc);
+    } else {
+      TA* ko = kv_store + g.offset(layer, page, 0, h - n_heads, off);
+      ko[i] = from_f32<TA>(ra);
+      ko[i + half] = from_f32<TA>(rc);
+    }
+  }
+  for (int p = threadIdx.x; p < nkv; p += blockDim.x) {
+    int h = p / dh, e = p % dh;
+    kv_store[g.offset(layer, page, 1, h, off) + e] = from_f32<TA>(row[nq + nkv + p]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5 (plain)  attention, one block per (query token, head): softmax_j(q.k_j / sqrt(d_h)) v_j over ALL
+// j in [0, S_r), no mask; K/V read from the pages (the block's own slots were just rewritten by a4).
+// Scores live in dynamic shared memory ([max_kv_len] floats).
+// ------------------------------------------------------------------------------------------------
+template <typename TA>
+__global__ void attention_plain_kernel(TA* __restrict__ out, const TA* __restrict__ q, const TA* __restrict__ kv_store,
+                                       const int* __restrict__ page_table, BatchDesc b, KvGeom g, int layer,
+                                       int n_heads, float scale) {
+  extern __shared__ float sc[];
+  __shared__ float red[33];
+  __shared__ float qs[256];
+  int t = blockIdx.x, h = blockIdx.y;
+  int bi = b.tok_bi[t];
+  int S = b.kv_len[bi];
+  int dh = g.head_dim;
+  int kvh = (h * g.n_kv_heads) / n_heads;
+  const int* pt = page_table + (long long)b.slot[bi] * g.max_pages_per_req;
+  const TA* qr = q + ((long long)t * n_heads + h) * dh;
+  for (int e = threadIdx.x; e < dh; e += blockDim.x) qs[e] = to_f32(qr[e]);
+  __syncthreads();
+  float lmax = -CUDART_INF_F;
+  for (int j = threadIdx.x; j < S; j += blockDim.x) {
+    const TA* kr = kv_store + g.offset(layer, pt[j / g.page_tokens], 0, kvh, j % g.page_tokens);
+    float s = 0.f;
+    for (int e = 0; e < dh; ++e) s += qs[e] * to_f32(kr[e]);
+    s *= scale;
+    sc[j] = s;
+    lmax = fmaxf(lmax, s);
+  }
+  lmax = warp_max(lmax);
+  int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) red[w] = lmax;
+  __syncthreads();
+  float m = red[0];
+  for (int i = 1; i < (int)(blockDim.x >> 5); ++i) m = fmaxf(m, red[i]);
+  float lsum = 0.f;
+  for (int j = threadIdx.x; j < S; j += blockDim.x) {
+    float p = expf(sc[j] - m);
+    sc[j] = p;
+    lsum += p;
+  }
+  float tot = block_sum(lsum, red);
+  float inv = 1.f / tot;
+  for (int e = threadIdx.x; e < dh; e += blockDim.x) {
+    float acc = 0.f;
+    for (int j = 0; j < S; ++j) {
+      const TA* vr = kv_store + g.offset(layer, pt[j / g.page_tokens], 1, kvh, j % g.page_tokens);
+      acc += sc[j] * to_f32(vr[e]);
+    }
+    out[((long long)t * n_heads + h) * dh + e] = from_f32<TA>(acc * inv);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3/a6/a8/a9/a11 (plain)  C[M,N] = A[M,K] . W[N,K]^T, fp32 accumulate, fp32 out.  64x64 tile, 4x4 per thread.
+// ------------------------------------------------------------------------------------------------
+template <typename TA, typename TW>
+__global__ void __launch_bounds__(256) gemm_plain_kernel(float* __restrict__ C, const TA* __restrict__ A,
+                                                         const TW* __restrict__ W, int M, int N, int K, int lda,
+                                                         int ldw, int ldc) {
+  __shared__ float As[16][65];
+  __shared__ float Ws[16][65];
+  int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  int m0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
+  float acc[4][4] = {};
+  for (int k0 = 0; k0 < K; k0 += 16) {
+    for (int i = threadIdx.x; i < 1024; i += 256) {
+      int r = i >> 4, c = i & 15;
+      As[c][r] = (m0 + r < M && k0 + c < K) ? to_f32(A[(long long)(m0 + r) * lda + k0 + c]) : 0.f;
+      Ws[c][r] = (n0 + r < N && k0 + c < K) ? to_f32(W[(long long)(n0 + r) * ldw + k0 + c]) : 0.f;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < 16; ++kk) {
+      float a[4], w[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { a[i] = As[kk][ty * 4 + i]; w[i] = Ws[kk][tx * 4 + i]; }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], w[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+  for (int i = 0; i < 4; ++i)
+    for (int j = 0; j < 4; ++j) {
+      int m = m0 + ty * 4 + i, n = n0 + tx * 4 + j;
+      if (m < M && n < N) C[(long long)m * ldc + n] = acc[i][j];
+    }
+}
+
+// x += y   (fp32 residual stream)
+__global__ void add_residual_kernel(float* __restrict__ x, const float* __restrict__ y, long long n) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) x[i] += y[i];
+}
+
+__device__ __forceinline__ float silu_f(float g) { return g / (1.f + __expf(-g)); }
+
+// act[t, f] = silu(gu[t, f]) * gu[t, F + f]
+template <typename TA>
+__global__ void swiglu_kernel(TA* __restrict__ act, const float* __restrict__ gu, int T, int F) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)T * F) return;
+  int t = (int)(i / F), f = (int)(i % F);
+  const float* r = gu + (long long)t * 2 * F;
+  act[i] = from_f32<TA>(silu_f(r[f]) * r[F + f]);
+}
+
+// row_src[r] for a10: index into [T, d] of each block row
+__global__ void build_row_src_kernel(int* __restrict__ row_src, BatchDesc b) {
+  int bi = blockIdx.x;
+  int base = b.q_off[bi] + (b.blk_lo[bi] - b.q_pos0[bi]);
+  for (int j = threadIdx.x; j < b.blk_len[bi]; j += blockDim.x) row_src[b.row_off[bi] + j] = base + j;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a11 (plain)  per-row statistics of materialised logits: z = scale * logits, z[mask_id] excluded.
+// Writes ONE partial (max, sum exp(z - max), argmax) per row, the format the tcgen05 epilogue writes per tile.
+// ------------------------------------------------------------------------------------------------
+struct RowPartial { float m, s; int idx; int pad; };
+
+__device__ __forceinline__ void partial_merge(float& m, float& s, int& idx, float m2, float s2, int idx2) {
+  // lowest index wins ties (reading G8)
+  if (m2 > m || (m2 == m && idx2 < idx)) idx = idx2;
+  float nm = fmaxf(m, m2);
+  if (nm == -CUDART_INF_F) { s = 0.f; m = nm; return; }
+  s = s * __expf(m - nm) + s2 * __expf(m2 - nm);
+  m = nm;
+}
+
+__global__ void row_stats_plain_kernel(RowPartial* __restrict__ part, const float* __restrict__ logits, int V,
+                                       int mask_id, float scale) {
+  __shared__ float sm[32], ss[32];
+  __shared__ int si[32];
+  int r = blockIdx.x;
+  const float* z = logits + (long long)r * V;
+  float m = -CUDART_INF_F, s = 0.f;
+  int idx = 0x7fffffff;
+  for (int v = threadIdx.x; v < V; v += blockDim.x) {
+    if (v == mask_id) continue;
+    partial_merge(m, s, idx, z[v] * scale, 1.f, v);
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    float m2 = __shfl_xor_sync(0xffffffffu, m, o), s2 = __shfl_xor_sync(0xffffffffu, s, o);
+    int i2 = __shfl_xor_sync(0xffffffffu, idx, o);
+    partial_merge(m, s, idx, m2, s2, i2);
+  }
+  int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { sm[w] = m; ss[w] = s; si[w] = idx; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int i = 1; i < (int)(blockDim.x >> 5); ++i) partial_merge(m, s, idx, sm[i], ss[i], si[i]);
+    part[r].m = m; part[r].s = s; part[r].idx = idx; part[r].pad = 0;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a12 + a13  combine split-vocab partials, then threshold-unmask.  One block (128 threads) per request.
+//   tok = argmax_v z (lowest id on ties), lse = m + log(sum), conf = 1 / sum = exp(z_tok - lse)
+//   M = MASK positions of the current block; C = {i in M : conf_i >= tau} U {argmax_{i in M} conf_i, lowest i}
+//   tokens[i] = tok_i for i in C (unless dry run); commits written in ascending position.
+// ------------------------------------------------------------------------------------------------
+struct StepOut {              // device-side result arrays, fixed stride max_block per request
+  int* n_committed;           // [n]
+  int* pos;                   // [n, max_block]
+  int* tok;                   // [n, max_block]
+  float* conf;                // [n, max_block]
+  float* row_lse;             // [n, max_block]
+  float* row_conf;            // [n, max_block]
+  int* row_tok;               // [n, max_block]
+};
+
+__global__ void __launch_bounds__(128) combine_unmask_kernel(StepOut o, const RowPartial* __restrict__ part,
+                                                             int n_tiles, int* __restrict__ tokens, int max_seq,
+                                                             int max_block, int mask_id, BatchDesc b, int dry_run) {
+  __shared__ float s_conf[64];
+  __shared__ int s_tok[64];
+  int bi = blockIdx.x;
+  int B = b.blk_len[bi];
+  int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  for (int j = w; j < B; j += 4) {
+    const RowPartial* p = part + (long long)(b.row_off[bi] + j) * n_tiles;
+    float m = -CUDART_INF_F, s = 0.f;
+    int idx = 0x7fffffff;
+    for (int t = l; t < n_tiles; t += 32) partial_merge(m, s, idx, p[t].m, p[t].s, p[t].idx);
+    for (int off = 16; off > 0; off >>= 1) {
+      float m2 = __shfl_xor_sync(0xffffffffu, m, off), s2 = __shfl_xor_sync(0xffffffffu, s, off);
+      int i2 = __shfl_xor_sync(0xffffffffu, idx, off);
+      partial_merge(m, s, idx, m2, s2, i2);
+    }
+    if (l == 0) {
+      float conf = 1.f / s;
+      s_conf[j] = conf;
+      s_tok[j] = idx;
+      o.row_lse[bi * max_block + j] = m + logf(s);
+      o.row_conf[bi * max_block + j] = conf;
+      o.row_tok[bi * max_block + j] = idx;
+    }
+  }
+  __syncthreads();
+  if (w != 0) return;
+  int* trow = tokens + (long long)b.slot[bi] * max_seq + b.blk_lo[bi];
+  float tau = b.tau[bi];
+  // best MASK position: max conf, lowest j on ties
+  float bc = -1.f;
+  int bj = 0x7fffffff;
+  for (int j = l; j < B; j += 32)
+    if (trow[j] == mask_id && (s_conf[j] > bc)) { bc = s_conf[j]; bj = j; }   // ascending j keeps the lowest on ties
+  for (int off = 16; off > 0; off >>= 1) {
+    float c2 = __shfl_xor_sync(0xffffffffu, bc, off);
+    int j2 = __shfl_xor_sync(0xffffffffu, bj, off);
+    if (c2 > bc || (c2 == bc && j2 < bj)) { bc = c2; bj = j2; }
+  }
+  int count = 0;
+  for (int j0 = 0; j0 < B; j0 += 32) {
+    int j = j0 + l;
+    bool masked = (j < B) && trow[j] == mask_id;
+    bool commit = masked && (s_conf[j] >= tau || j == bj);
+    unsigned bal = __ballot_sync(0xffffffffu, commit);
+    if (commit) {
+      int k = count + __popc(bal & ((1u << l) - 1));
+      o.pos[bi * max_block + k] = b.blk_lo[bi] + j;
+      o.tok[bi * max_block + k] = s_tok[j];
+      o.conf[bi * max_block + k] = s_conf[j];
+      if (!dry_run) trow[j] = s_tok[j];
+    }
+    count += __popc(bal);
+  }
+  if (l == 0) o.n_committed[bi] = count;
+}
+
+}  // namespace dlm

@@ -1,0 +1,294 @@
+"""End-to-end parity of the CUDA path (through the C ABI) with the fp64 oracle (-m gpu).
+
+Protocols:
+  P-A  config 1, fp32 weights, all-fp32 CUDA path, FREE-RUNNING to completion: commits bit-exact outside the
+       1e-3 band (resync after a step with an exclusion), hidden / lse within 1e-4.
+  P-B  bf16 models, TEACHER-FORCED per step: hidden and lse within 2e-2 relative are pass/fail; commit
+       agreement is reported (agree / excluded / mismatch).
+  P-C  bf16 models, stage-wise from the GPU's own dumped stage inputs.
+"""
+import numpy as np
+import pytest
+
+from oracle import compare, model as omodel, step as ostep, weights as ow
+from synth_inputs import ARCH_C1, ARCH_LLADA8B, ARCH_QWEN7B, WEIGHT_SEED, RequestSpec, initial_tokens, random_tokens, workload_c1
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def _pkg():
+    import paper_2606_29094_b200 as pkg
+    return pkg
+
+
+def _gpu_hidden_block_rows(pkg, eng, rid, arch, o, refresh):
+    """last layer's residual output on the block rows, from the debug dump"""
+    S = len(eng.tokens(rid))
+    rows = S if refresh else len(o.conf)
+    x = eng.debug_tensor(rid, arch.n_layers - 1, pkg.binding.T_X_OUT, rows, arch.d_model)
+    return x[o.block_lo:o.block_lo + len(o.conf)] if refresh else x
+
+
+def _run_parity(arch, seed, spec, max_steps, teacher_forced, hid_tol, lse_tol, simple=False, flash=True, kv_page_tokens=64):
+    """Step the GPU engine and the oracle side by side; returns counters.  teacher_forced: GPU tokens are reset
+    to the oracle's before every step (cache kept)."""
+    pkg = _pkg()
+    S = len(spec.prompt) + spec.gen_len
+    eng = pkg.Engine(arch, seed, max_requests=1, max_seq=S, max_block=spec.block_len, kv_page_tokens=kv_page_tokens)
+    eng.set_option(pkg.OPT_DEBUG_DUMP, 1)
+    eng.set_option(pkg.OPT_SIMPLE_KERNELS, 1 if simple else 0)
+    eng.set_option(pkg.OPT_FLASH_ATTENTION, 1 if flash else 0)
+    rid = eng.add_request(spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
+    wts = ow.Weights(arch, seed)
+    oreq = ostep.Request(arch, spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
+    if spec.filled is not None:
+        oreq.tokens[:] = initial_tokens(spec, arch.mask_id)
+        eng.set_tokens(rid, oreq.tokens.astype(np.int32))
+    stats = dict(steps=0, exact=0, excluded=0, mismatch=0, max_hid=0.0, max_lse=0.0, resync=0)
+    while oreq.current_block() is not None and stats["steps"] < max_steps:
+        if eng.info(rid)["cache_valid"] != oreq.cache_valid:      # a resync moved one side across a block boundary
+            oreq.cache_valid = False
+            eng.set_tokens(rid, oreq.tokens.astype(np.int32), keep_cache=False)
+        refresh = not oreq.cache_valid
+        lo, hi = oreq.block_range(oreq.current_block())
+        masked_before = oreq.tokens[lo:hi] == arch.mask_id
+        o = ostep.refresh_step(oreq, wts) if refresh else ostep.cached_step(oreq, wts)
+        g = eng.refresh_step([rid]) if refresh else eng.cached_step([rid])
+        hid = _gpu_hidden_block_rows(pkg, eng, rid, arch, o, refresh)
+        stats["max_hid"] = max(stats["max_hid"], float(compare.rel_rows(hid, o.hidden).max()))
+        stats["max_lse"] = max(stats["max_lse"], float(np.abs(g.lse[0][:hi - lo] - o.lse).max() / np.abs(o.lse).max()))
+        assert stats["max_hid"] <= hid_tol, f"hidden rel err {stats['max_hid']} at step {stats['steps']}"
+        assert stats["max_lse"] <= lse_tol, f"lse rel err {stats['max_lse']} at step {stats['steps']}"
+        d = compare.compare_commits(o, masked_before, spec.threshold, [(p, t) for p, t, _ in g.commits[0]])
+        stats["exact"] += d.exact
+        stats["excluded"] += d.n_excluded
+        stats["mismatch"] += d.n_mismatch
+        stats["steps"] += 1
+        assert g.n_masked_left[0] == eng.info(rid)["n_masked"]
+        if teacher_forced or not d.exact:
+            eng.set_tokens(rid, oreq.tokens.astype(np.int32), keep_cache=True)
+            stats["resync"] += (not d.exact)
+        assert np.array_equal(eng.tokens(rid), oreq.tokens)
+        if not teacher_forced:
+            assert d.n_mismatch == 0, d.detail
+    eng.close()
+    return stats
+
+
+# ------------------------------------------------------------------------------------------------------------------
+def test_c1_fp32_free_running_trajectory():
+    """P-A: the literal north_star criterion on config 1 (fp32 weights, all-fp32 CUDA path), run to completion."""
+    spec = workload_c1()[0]
+    s = _run_parity(ARCH_C1, WEIGHT_SEED["C1"], spec, 10 ** 6, teacher_forced=False, hid_tol=1e-4, lse_tol=1e-4)
+    print("P-A", s)
+    assert s["mismatch"] == 0 and s["steps"] >= 2 * 1 and s["steps"] <= 64
+
+
+@pytest.mark.parametrize("tau,steps_per_block", [(1.5, 32), (0.0, 1)])
+def test_c1_threshold_extremes_on_gpu(tau, steps_per_block):
+    """north_star pins on the CUDA path: tau > 1 commits exactly one token per step, tau = 0 the whole block."""
+    pkg = _pkg()
+    spec = workload_c1()[0]
+    eng = pkg.Engine(ARCH_C1, WEIGHT_SEED["C1"], max_requests=1, max_seq=128, max_block=32)
+    rid = eng.add_request(spec.prompt, 64, 32, tau)
+    n_steps, seen = 0, {}
+    prev = eng.tokens(rid)
+    while eng.info(rid)["n_masked"] > 0:
+        cached = eng.info(rid)["cache_valid"]
+        blk = eng.info(rid)["cur_block"]
+        g = eng.cached_step([rid]) if cached else eng.refresh_step([rid])
+        assert g.n_committed[0] == (1 if tau > 1 else 32)
+        cur = eng.tokens(rid)
+        changed = np.flatnonzero(cur != prev)
+        assert sorted(changed.tolist()) == [p for p, _, _ in g.commits[0]]          # only commits change tokens
+        assert (prev[changed] == ARCH_C1.mask_id).all() and (cur[changed] != ARCH_C1.mask_id).all()
+        assert all(64 + blk * 32 <= p < 64 + (blk + 1) * 32 for p, _, _ in g.commits[0])
+        prev = cur
+        seen[blk] = seen.get(blk, 0) + 1
+        n_steps += 1
+        assert n_steps <= 64
+    assert seen == {0: steps_per_block, 1: steps_per_block}
+    g = eng.refresh_step([rid])                      # finished request commits 0
+    assert g.total == 0
+    eng.close()
+
+
+def test_state_errors_and_dry_run():
+    pkg = _pkg()
+    spec = workload_c1()[0]
+    eng = pkg.Engine(ARCH_C1, WEIGHT_SEED["C1"], max_requests=2, max_seq=128, max_block=32)
+    rid = eng.add_request(spec.prompt, 64, 32, 0.9)
+    with pytest.raises(pkg.DlmError) as e:
+        eng.cached_step([rid])                        # no valid cache yet (G19)
+    assert e.value.code == pkg.binding.DLM_E_STATE
+    with pytest.raises(pkg.DlmError):
+        eng.add_request(spec.prompt, 60, 32, 0.9)     # G % B != 0 (G20)
+    with pytest.raises(pkg.DlmError):
+        eng.refresh_step([rid, rid])
+    with pytest.raises(pkg.DlmError):
+        eng.refresh_step([5])
+    before = eng.tokens(rid)
+    a = eng.refresh_step([rid], dry_run=True)          # fills the cache, commits reported, nothing mutated
+    assert a.total >= 1 and np.array_equal(eng.tokens(rid), before) and eng.info(rid)["cache_valid"]
+    b = eng.cached_step([rid], dry_run=True)           # G15: cached right after refresh == full recompute
+    assert [(p, t) for p, t, _ in a.commits[0]] == [(p, t) for p, t, _ in b.commits[0]]
+    assert np.allclose(a.lse, b.lse, rtol=1e-5, atol=1e-5) and np.allclose(a.row_conf, b.row_conf, rtol=1e-4, atol=1e-7)
+    c = eng.cached_step([rid], thresholds=[0.0])       # per-step threshold override: whole block
+    assert c.n_committed[0] == 32 and not eng.info(rid)["cache_valid"] and eng.info(rid)["cur_block"] == 1
+    eng.remove_request(rid)
+    with pytest.raises(pkg.DlmError):
+        eng.refresh_step([rid])
+    eng.close()
+
+
+def test_batch_independence_ragged():
+    """A request's result does not depend on its batch-mates or on batch order (ragged lengths, mixed B)."""
+    pkg = _pkg()
+    a = ARCH_C1
+    rng = np.random.default_rng(77)
+    specs = [(random_tokens(rng, P, a.vocab, a.mask_id), G, B, tau) for P, G, B, tau in
+             [(64, 64, 32, 0.9), (17, 32, 16, 0.05), (100, 24, 8, 0.5), (5, 64, 32, 1.5)]]
+    eng = pkg.Engine(a, WEIGHT_SEED["C1"], max_requests=4, max_seq=128, max_block=32)
+    ids = [eng.add_request(*s) for s in specs]
+    solo = []
+    for i in ids:
+        r = eng.refresh_step([i], dry_run=True)
+        c = eng.cached_step([i], dry_run=True)
+        solo.append((r, c))
+    for order in ([0, 1, 2, 3], [3, 1, 0, 2]):
+        r = eng.refresh_step([ids[k] for k in order], dry_run=True)
+        c = eng.cached_step([ids[k] for k in order], dry_run=True)
+        for j, k in enumerate(order):
+            for got, want in ((r, solo[k][0]), (c, solo[k][1])):
+                assert got.commits[j] == want.commits[0]
+                assert np.array_equal(got.lse[j], want.lse[0]) and np.array_equal(got.row_tok[j], want.row_tok[0])
+    # mixed kinds back to back (config 3 pattern): one refresh + the rest cached, then real commits
+    eng.refresh_step([ids[0]])
+    eng.cached_step([ids[1], ids[2], ids[3]])
+    eng.close()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+ARCH_C1_BF16 = ARCH_C1.replace(weight_dtype=1)
+
+
+@pytest.mark.parametrize("simple", [False, True])
+def test_c1_bf16_teacher_forced(simple):
+    """G16(ii) / P-B: config 1 with weights rounded to bf16 on BOTH sides, through the tcgen05 path (K tails:
+    d_ffn 688; head_dim 64 -> plain attention) and through the plain-kernel path."""
+    spec = workload_c1()[0]
+    s = _run_parity(ARCH_C1_BF16, WEIGHT_SEED["C1"], spec, 24, teacher_forced=True, hid_tol=2e-2, lse_tol=2e-2, simple=simple)
+    print("P-B C1/bf16", "plain" if simple else "tcgen05", s)
+
+
+def _reduced(arch, layers):
+    return arch.replace(n_layers=layers)
+
+
+@pytest.mark.parametrize("simple,flash", [(False, True), (False, False), (True, False)])
+def test_c2_reduced_depth_teacher_forced(simple, flash):
+    """P-B on the LLaDA-8B shape at depth 2 (full widths: d 4096, 32 heads x 128, FFN 12288, vocab 126464)."""
+    arch = _reduced(ARCH_LLADA8B, 2)
+    rng = np.random.default_rng(2002)
+    spec = RequestSpec(random_tokens(rng, 96, arch.vocab, arch.mask_id), 64, 32, 0.9)
+    s = _run_parity(arch, WEIGHT_SEED["C2"], spec, 5, teacher_forced=True, hid_tol=2e-2, lse_tol=2e-2, simple=simple, flash=flash)
+    print("P-B C2/L2", dict(simple=simple, flash=flash), s)
+
+
+def test_c5_reduced_depth_gqa_teacher_forced():
+    """P-B on the Qwen2.5-7B shape (GQA 28/4, FFN 18944, vocab 152064) at depth 2."""
+    arch = _reduced(ARCH_QWEN7B, 2)
+    rng = np.random.default_rng(2005)
+    spec = RequestSpec(random_tokens(rng, 200, arch.vocab, arch.mask_id), 64, 32, 0.9)
+    s = _run_parity(arch, WEIGHT_SEED["C5"], spec, 4, teacher_forced=True, hid_tol=2e-2, lse_tol=2e-2)
+    print("P-B C5/L2", s)
+
+
+def test_stagewise_from_gpu_inputs():
+    """P-C: every stage of one layer recomputed by the oracle FROM THE GPU'S OWN STAGE INPUTS (bf16 rounding
+    points cut the step); tolerances are those of a single fp32-accumulated stage, not of the whole bf16 path."""
+    pkg = _pkg()
+    B = pkg.binding
+    arch = _reduced(ARCH_LLADA8B, 2)
+    seed = WEIGHT_SEED["C2"]
+    rng = np.random.default_rng(9)
+    prompt = random_tokens(rng, 70, arch.vocab, arch.mask_id)
+    S, G, Bk = 70 + 64, 64, 32
+    eng = pkg.Engine(arch, seed, max_requests=1, max_seq=S, max_block=Bk)
+    eng.set_option(pkg.OPT_DEBUG_DUMP, 1)
+    rid = eng.add_request(prompt, G, Bk, 0.9)
+    wts = ow.Weights(arch, seed)
+    HQ, HKV, d, F = arch.n_heads * arch.head_dim, arch.n_kv_heads * arch.head_dim, arch.d_model, arch.d_ffn
+    eng.refresh_step([rid], dry_run=True)
+    for kind in ("refresh", "cached"):
+        if kind == "cached":
+            eng.cached_step([rid], dry_run=True)
+        rows, lo = (S, 0) if kind == "refresh" else (Bk, 70)
+        pos = np.arange(lo, lo + rows, dtype=np.float64)
+        for l in range(arch.n_layers):
+            t = lambda which, w: eng.debug_tensor(rid, l, which, rows, w).astype(np.float64)
+            x_in, u1, q, attn, x_mid, u2, act, x_out = (t(B.T_X_IN, d), t(B.T_NORM1, d), t(B.T_Q, HQ), t(B.T_ATTN, HQ),
+                                                        t(B.T_X_MID, d), t(B.T_NORM2, d), t(B.T_ACT, F), t(B.T_X_OUT, d))
+            kc = eng.debug_tensor(rid, l, B.T_KCACHE, S, HKV).astype(np.float64)
+            vc = eng.debug_tensor(rid, l, B.T_VCACHE, S, HKV).astype(np.float64)
+            bf = lambda want, got, extra=0.0: np.all(np.abs(got - want) <= np.abs(want) * 2 ** -8 + extra)   # one bf16 rounding
+            # S0/S4 norms
+            assert bf(omodel.rmsnorm(x_in, arch.rms_eps), u1, 1e-6) and bf(omodel.rmsnorm(x_mid, arch.rms_eps), u2, 1e-6)
+            # S1 QKV + RoPE from the GPU's normed input; K/V as stored
+            wq, wk, wv = (wts.get(ow.layer_tid(l, s)) for s in (ow.SUB_Q, ow.SUB_K, ow.SUB_V))
+            q_o = omodel.rope((u1 @ wq.T).reshape(rows, arch.n_heads, arch.head_dim), pos, arch.rope_theta).reshape(rows, HQ)
+            k_o = omodel.rope((u1 @ wk.T).reshape(rows, arch.n_kv_heads, arch.head_dim), pos, arch.rope_theta).reshape(rows, HKV)
+            assert bf(q_o, q, 2e-4) and bf(k_o, kc[lo:lo + rows], 2e-4) and bf(u1 @ wv.T, vc[lo:lo + rows], 2e-4)
+            # S2 attention from the GPU's q and stored K/V
+            a_o = omodel.attention(q.reshape(rows, arch.n_heads, -1), kc.reshape(S, arch.n_kv_heads, -1), vc.reshape(S, arch.n_kv_heads, -1))
+            assert np.abs(a_o.reshape(rows, HQ) - attn).max() <= 2e-3 * max(1.0, np.abs(a_o).max())
+            # S3 O-proj + residual, S5 gate/up + SwiGLU, S6 down + residual
+            xm_o = x_in + attn @ wts.get(ow.layer_tid(l, ow.SUB_O)).T
+            assert np.abs(xm_o - x_mid).max() <= 1e-4 * max(1.0, np.abs(xm_o).max())
+            act_o = omodel.silu(u2 @ wts.get(ow.layer_tid(l, ow.SUB_G)).T) * (u2 @ wts.get(ow.layer_tid(l, ow.SUB_U)).T)
+            assert bf(act_o, act, 1e-5)
+            xo_o = x_mid + act @ wts.get(ow.layer_tid(l, ow.SUB_D)).T
+            assert np.abs(xo_o - x_out).max() <= 1e-4 * max(1.0, np.abs(xo_o).max())
+    # S7: LM head from the GPU's final-normed rows
+    g = eng.cached_step([rid], dry_run=True)
+    hf = eng.debug_tensor(rid, 0, B.T_FINAL_NORM, Bk, d).astype(np.float64)
+    z = arch.logit_scale * (hf @ wts.get(ow.TID_LMHEAD).T)
+    z[:, arch.mask_id] = -np.inf
+    tok_o, conf_o, lse_o, margin = omodel.confidence(z)
+    clear = margin >= 1e-3
+    assert np.array_equal(g.row_tok[0][clear], tok_o[clear])
+    assert np.abs(g.row_conf[0] - conf_o).max() < 2e-5 and np.abs(g.lse[0] - lse_o).max() < 1e-4 * np.abs(lse_o).max()
+    # S8: unmask from the GPU's own (tok, conf): bit-exact, no band
+    toks = eng.tokens(rid).astype(np.int64)
+    want = ostep.unmask(toks, 70, 70 + Bk, g.row_tok[0], g.row_conf[0], np.float32(0.9), arch.mask_id, dry_run=True)
+    assert [(p, t) for p, t, _ in g.commits[0]] == [(c.pos, c.tok) for c in want]
+    eng.close()
+
+
+def test_embedding_rows_bit_exact():
+    """Definition W on the device: layer-0 residual input == E[token] exactly (bf16 values are exact in fp32)."""
+    pkg = _pkg()
+    arch = _reduced(ARCH_LLADA8B, 1)
+    rng = np.random.default_rng(4)
+    prompt = random_tokens(rng, 40, arch.vocab, arch.mask_id)
+    eng = pkg.Engine(arch, 1234, max_requests=1, max_seq=72, max_block=32)
+    eng.set_option(pkg.OPT_DEBUG_DUMP, 1)
+    rid = eng.add_request(prompt, 32, 32, 0.9)
+    eng.refresh_step([rid], dry_run=True)
+    x = eng.debug_tensor(rid, 0, pkg.binding.T_X_IN, 72, arch.d_model)
+    want = ow.Weights(arch, 1234).rows(ow.TID_EMBED, eng.tokens(rid))
+    assert np.array_equal(x.astype(np.float64), want)
+    eng.close()
+
+
+def test_cost_table_rows():
+    pkg = _pkg()
+    eng = pkg.Engine(ARCH_C1, WEIGHT_SEED["C1"], max_requests=4, max_seq=1024, max_block=32, max_batch_tokens=4096)
+    rows = eng.profile_step_costs()
+    assert rows and all(r["usec"] > 0 for r in rows)
+    kinds = {(r["kind"], r["n_requests"], r["kv_tokens"]) for r in rows}
+    assert ("refresh", 1, 512) in kinds and ("cached", 4, 1024) in kinds
+    for r in rows:
+        assert r["n_tokens"] == (r["n_requests"] * r["kv_tokens"] if r["kind"] == "refresh" else r["n_requests"] * 32)
+    eng.close()
