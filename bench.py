@@ -1,0 +1,440 @@
+#!/usr/bin/env python3
+"""bench.py -- denoising-step throughput of libdlm on B200 (BASELINE.json metric: denoise steps/s and committed
+tokens/s on 1 B200, LLaDA-8B shape; % of roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3|C4|C5] [--impl ours|reference]
+
+A "step" is one denoising step of the workload's batch through the whole hot path (DESIGN.md rows a0-a14): refresh
+steps where a block starts, cached steps inside a block, exactly as the free-running trajectory demands.
+`value`  = steps / device time (CUDA events on the library's stream around each step's kernels, inputs resident).
+`e2e`    = steps / wall time of the same C-ABI calls with HOST buffers (request upload, per-step descriptor H2D,
+           result D2H and the synchronize all inside the timed region).
+`roofline` = the tcgen05 GEMM kernel (the dominant kernel) inside cached steps, from per-launch CUDA events.
+`cpu_baseline` = the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample.
+N > 1: one process per GPU (torchrun), independent replicas of the workload (requests are independent, P:426
+"16 TP-1 workers"), no data-path collective; time = max over ranks; scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from synth_inputs import (ARCH_LLADA8B, ARCH_QWEN7B, WEIGHT_SEED, initial_tokens, workload_c2, workload_c3,  # noqa: E402
+                          workload_c4, workload_c5)
+
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), "source": "measured"}
+    return dict(FALLBACK_PEAKS, source="fallback")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# algorithmic work of a step: what the method must move / multiply
+# ---------------------------------------------------------------------------------------------------------
+def layer_params(a):
+    return a.d_model * (a.n_heads + 2 * a.n_kv_heads) * a.head_dim + a.n_heads * a.head_dim * a.d_model + 3 * a.d_model * a.d_ffn
+
+
+def step_work(a, q_lens, kv_lens, rows):
+    """FLOPs and HBM bytes of one step: q_lens[i] tokens of request i computed against kv_lens[i] positions."""
+    T, R = sum(q_lens), rows
+    L = a.n_layers
+    kv_tok = 4 * a.n_kv_heads * a.head_dim                       # bytes of K and V per token per layer (bf16)
+    flops_lin = 2 * T * layer_params(a) * L
+    flops_lm = 2 * R * a.d_model * a.vocab
+    flops_attn = 4 * sum(q * s for q, s in zip(q_lens, kv_lens)) * a.n_heads * a.head_dim * L
+    bytes_w = 2 * (layer_params(a) * L + a.vocab * a.d_model)
+    bytes_kv_rd = sum(kv_lens) * kv_tok * L
+    bytes_kv_wr = T * kv_tok * L
+    return {"flops": flops_lin + flops_lm + flops_attn, "bytes": bytes_w + bytes_kv_rd + bytes_kv_wr,
+            "weight_bytes": bytes_w, "kv_read_bytes": bytes_kv_rd, "flops_linear": flops_lin + flops_lm, "flops_attn": flops_attn}
+
+
+def roofline_ms(work, peaks, sustained=True):
+    tf = peaks["bf16_tflops_sustained" if sustained else "bf16_tflops"] * 1e12
+    t_f = work["flops"] / tf
+    t_b = work["bytes"] / (peaks["hbm_gbs"] * 1e9)
+    return 1e3 * max(t_f, t_b), ("tensor" if t_f > t_b else "hbm")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ---------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": int(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# workloads
+# ---------------------------------------------------------------------------------------------------------
+def get_workload(name: str):
+    if name == "C2":
+        return ARCH_LLADA8B, WEIGHT_SEED["C2"], workload_c2(), "configs[1]: LLaDA-8B shape, batch 1, prompt 256, gen 256, block 32, tau 0.9"
+    if name == "C3":
+        return ARCH_LLADA8B, WEIGHT_SEED["C3"], workload_c3(), "configs[2]: LLaDA-8B shape, ragged batch 32, prompts U[128,1024], gen 256, block 32, mixed tau/phases"
+    if name == "C4":
+        return ARCH_LLADA8B, WEIGHT_SEED["C4"], workload_c4(), "configs[3]: LLaDA-8B shape, batch 8, prompt 4096, gen 512, block 64, tau 0.9"
+    if name == "C5":
+        return ARCH_QWEN7B, WEIGHT_SEED["C5"], workload_c5(), "configs[4]: Qwen2.5-7B shape (GQA 28/4), batch 64, prompts U[256,2048], gen 256, block 32"
+    raise SystemExit(f"unknown workload {name}")
+
+
+class Runner:
+    """Drives a batch of requests through libdlm the way the paper's scheduler would: every
+    request gets the step kind that is due; refresh and cached requests of one iteration go in two calls."""
+
+    def __init__(self, pkg, arch, seed, specs):
+        self.pkg, self.arch, self.specs = pkg, arch, specs
+        max_seq = max(len(s.prompt) + s.gen_len for s in specs)
+        max_seq = (max_seq + 63) // 64 * 64
+        self.max_block = max(s.block_len for s in specs)
+        tot = sum(len(s.prompt) + s.gen_len for s in specs)
+        self.eng = pkg.Engine(arch, seed, max_requests=len(specs), max_seq=max_seq, max_block=self.max_block,
+                              max_batch_tokens=max(tot, 128))
+        self.ids = [None] * len(specs)
+        self.h2d = 0
+        self.d2h = 0
+        for i in range(len(specs)):
+            self._add(i)
+
+    def _add(self, i):
+        s = self.specs[i]
+        if self.ids[i] is not None:
+            self.eng.remove_request(self.ids[i])
+        self.ids[i] = self.eng.add_request(s.prompt, s.gen_len, s.block_len, s.threshold)
+        self.h2d += 4 * (len(s.prompt) + s.gen_len)
+        if s.filled is not None and len(s.filled):
+            self.eng.set_tokens(self.ids[i], initial_tokens(s, self.arch.mask_id))
+            self.h2d += 4 * (len(s.prompt) + s.gen_len)
+
+    def step(self):
+        """One denoising step of the whole batch.  Returns (device_usec, commits, n_refresh_reqs, n_cached_reqs, work)."""
+        eng = self.eng
+        refresh, cached = [], []
+        for i, rid in enumerate(self.ids):
+            st = eng.info(rid)
+            if st["n_masked"] == 0:             # finished: the client submits it again (prompt upload inside the region)
+                self._add(i)
+                rid = self.ids[i]
+                st = eng.info(rid)
+            (cached if st["cache_valid"] else refresh).append(i)
+        usec, commits = 0.0, 0
+        q_lens, kv_lens, rows = [], [], 0
+        for kind, idx in (("refresh", refresh), ("cached", cached)):
+            if not idx:
+                continue
+            rids = [self.ids[i] for i in idx]
+            g = eng.refresh_step(rids) if kind == "refresh" else eng.cached_step(rids)
+            usec += g.usec
+            commits += g.total
+            self.h2d += 4 * (10 * len(rids) + sum((len(self.specs[i].prompt) + self.specs[i].gen_len) if kind == "refresh"
+                                                   else self.specs[i].block_len for i in idx))
+            self.d2h += 4 * (len(self.specs) + 6 * len(self.specs) * self.max_block)
+            for i in idx:
+                s = self.specs[i]
+                S = len(s.prompt) + s.gen_len
+                q_lens.append(S if kind == "refresh" else s.block_len)
+                kv_lens.append(S)
+                rows += s.block_len
+        return usec, commits, len(refresh), len(cached), step_work(self.arch, q_lens, kv_lens, rows)
+
+    def close(self):
+        self.eng.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the CPU oracle, timed as it stands on a bounded sample (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------------------
+def oracle_sample(arch, seed, spec, layers: int, n_cached: int):
+    """Time the fp64 oracle on the first `layers` layers (+ the LM head) of one request: one refresh step and
+    `n_cached` cached steps.  Returns per-step seconds extrapolated to the full depth (layer time x L/layers)."""
+    from oracle import model as omodel, step as ostep, weights as ow
+    sub = arch.replace(n_layers=layers)
+    wts = ow.Weights(sub, seed)
+    t0 = time.perf_counter()
+    for l in range(layers):                       # weight generation is set-up, not part of the step
+        for s in range(7):
+            wts.f32(ow.layer_tid(l, s))
+    wts.f32(ow.TID_LMHEAD)
+    t_gen = time.perf_counter() - t0
+    req = ostep.Request(sub, spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
+    if spec.filled is not None and len(spec.filled):
+        req.tokens[:] = initial_tokens(spec, arch.mask_id)
+    lo, hi = req.block_range(req.current_block())
+    t0 = time.perf_counter()
+    hidden, kv = omodel.full_forward(sub, wts, req.tokens)
+    t_ref_layers = time.perf_counter() - t0
+    req.cache, req.cache_valid = kv, True
+    t0 = time.perf_counter()
+    tok, conf, lse, margin = omodel.head(sub, wts, hidden[lo:hi])
+    ostep.unmask(req.tokens, lo, hi, tok, conf, spec.threshold, arch.mask_id)
+    t_head = time.perf_counter() - t0
+    t_cached_layers = []
+    for _ in range(n_cached):
+        if req.current_block() is None or not (req.tokens[lo:hi] == arch.mask_id).any():
+            break
+        t0 = time.perf_counter()
+        hidden, _ = omodel.cached_forward(sub, wts, req.tokens, lo, hi, req.cache)
+        t_cached_layers.append(time.perf_counter() - t0)
+        tok, conf, lse, margin = omodel.head(sub, wts, hidden)
+        ostep.unmask(req.tokens, lo, hi, tok, conf, spec.threshold, arch.mask_id)
+    f = arch.n_layers / layers
+    t_cached = (float(np.mean(t_cached_layers)) if t_cached_layers else 0.0) * f + t_head
+    return {"t_refresh": t_ref_layers * f + t_head, "t_cached": t_cached, "t_gen": t_gen, "n_cached": len(t_cached_layers)}
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        return max([int(p.get("num_threads", 1)) for p in threadpool_info()] or [os.cpu_count() or 1])
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def mix_steps_per_s(spec, t_refresh, t_cached):
+    """steps/s of the block cycle the workload runs: 1 refresh + (B - 1) cached steps."""
+    b = spec.block_len
+    return b / (t_refresh + (b - 1) * t_cached)
+
+
+def cpu_baseline(arch, seed, specs, layers=1, n_cached=2):
+    spec = specs[0]
+    o = oracle_sample(arch, seed, spec, layers, n_cached)
+    n = len(specs)
+    return {"value": mix_steps_per_s(spec, o["t_refresh"], o["t_cached"]) / n, "unit": "steps/s", "cores": blas_threads(), "kind": "oracle",
+            "sample": f"fp64 numpy oracle, request 0 of {n}, first {layers} of {arch.n_layers} layers + LM head: 1 refresh step and "
+                      f"{o['n_cached']} cached steps timed, layer time x{arch.n_layers // layers}, block cycle 1 refresh + {spec.block_len - 1} cached"
+                      + (f", divided by {n} requests processed serially" if n > 1 else ""),
+            "t_refresh_s": round(o["t_refresh"], 3), "t_cached_s": round(o["t_cached"], 3), "weight_gen_s": round(o["t_gen"], 1)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores; each step = one bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    arch, seed, specs, desc = get_workload(args.workload)
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    vals = []
+    for i in range(warm + steps):
+        cb = cpu_baseline(arch, seed, specs, layers=1, n_cached=1)
+        if i >= warm:
+            vals.append(cb)
+    v = float(np.mean([c["value"] for c in vals]))
+    out = {"impl": "reference", "metric": "denoise_steps_per_s", "value": v, "unit": "steps/s", "n_gpus": args.gpus, "steps": steps,
+           "warmup": warm, "ms_per_step": 1e3 / v, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": {"workload": f"{args.workload}: {desc}"},
+           "cpu_baseline": {"value": v, "unit": "steps/s", "cores": vals[-1]["cores"], "kind": "oracle", "sample": vals[-1]["sample"]},
+           "e2e": {"value": v, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=128)
+    ap.add_argument("--warmup", type=int, default=16)
+    ap.add_argument("--workload", default="C2")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-kernel-pass", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libdlm has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2606_29094_b200 as pkg
+    arch, seed, specs, desc = get_workload(args.workload)
+    peaks = load_peaks()
+    K, W = max(1, args.steps), max(3, args.warmup)
+
+    run = Runner(pkg, arch, seed, specs)
+    for _ in range(W):
+        run.step()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    run.h2d = run.d2h = 0
+    launches0 = run.eng.launch_count()
+    dev_us, commits, per_kind = 0.0, 0, {"refresh": [], "cached": [], "mixed": []}
+    work_by_kind = {}
+    with ClockSampler(local) as clk:
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(K):
+            us, cm, nr, nc, work = run.step()
+            dev_us += us
+            commits += cm
+            kind = "mixed" if (nr and nc) else ("refresh" if nr else "cached")
+            per_kind[kind].append(us)
+            work_by_kind.setdefault(kind, work)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+    launches = run.eng.launch_count() - launches0
+    if dist:
+        t = torch.tensor([dev_us, wall], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_us, wall = float(t[0]), float(t[1])
+        c = torch.tensor([commits, launches], device="cuda", dtype=torch.float64)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        commits, launches = int(c[0]), int(c[1])
+    n_req = len(specs)
+    value = world * K / (dev_us * 1e-6)
+    out = {"metric": "denoise_steps_per_s", "value": value, "unit": "steps/s", "n_gpus": world, "steps": K, "warmup": W,
+           "ms_per_step": dev_us / K * 1e-3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+           "data": "synthetic",
+           "config": {"workload": f"{args.workload}: {desc}", "requests_per_gpu": n_req, "parallelism": f"replicas x{world}, no collective",
+                      "l2": "every step streams all weights (15 GB >> 126 MB L2): inputs larger than L2, no flush",
+                      "timing": "value: sum over steps of CUDA-event time around each step's kernels (library stream); e2e: wall clock of the same calls"},
+           "committed_tokens_per_s": commits / (dev_us * 1e-6), "request_steps_per_s": value * n_req,
+           "e2e": {"value": world * K / wall, "unit": "steps/s", "h2d_bytes_per_step": run.h2d // K, "d2h_bytes_per_step": run.d2h // K,
+                   "committed_tokens_per_s": commits / wall},
+           "gpu_launches": int(launches), "clocks": clk.summary()}
+    # ---- per step kind: measured vs the step's roofline (north_star: >= 60 %) ----
+    steps_rf = {}
+    for kind, us in per_kind.items():
+        if not us:
+            continue
+        t_roof, bound = roofline_ms(work_by_kind[kind], peaks)
+        steps_rf[kind] = {"n": len(us), "ms": float(np.mean(us)) * 1e-3, "ms_min": float(np.min(us)) * 1e-3, "roofline_ms": t_roof, "bound": bound,
+                          "frac": t_roof / (float(np.mean(us)) * 1e-3), "gflop": work_by_kind[kind]["flops"] * 1e-9,
+                          "gbytes": work_by_kind[kind]["bytes"] * 1e-9}
+    out["step_roofline"] = steps_rf
+    out["peaks"] = peaks
+
+    # ---- dominant kernel: the tcgen05 GEMM inside cached steps, per-launch CUDA events ----
+    if rank == 0 and not args.no_kernel_pass:
+        out["roofline"], out["kernels"] = kernel_pass(run, pkg, arch, peaks)
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        try:
+            out["cpu_baseline"] = cpu_baseline(arch, seed, specs)
+        except Exception as e:      # the oracle must never take the GPU line down
+            out["cpu_baseline"] = {"value": None, "unit": "steps/s", "cores": os.cpu_count(), "kind": "oracle", "sample": f"failed: {e!r}"}
+    run.close()
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def kernel_pass(run, pkg, arch, peaks, n_steps=24):
+    """Second pass with an event pair around every launch (DLM_OPT_KERNEL_TIMING): per-kernel-class time inside
+    cached steps.  The GEMM classes are one kernel (gemm_tc_kernel) with different epilogues; they stream the
+    weights, so their roofline is HBM for small batches and tensor for large ones."""
+    eng = run.eng
+    eng.set_option(pkg.OPT_KERNEL_TIMING, 1)
+    eng.kernel_times(reset=True)
+    n_cached, works, kt = 0, None, {}
+    guard = 0
+    while n_cached < n_steps and guard < 8 * n_steps:
+        guard += 1
+        us, cm, nr, nc, work = run.step()
+        step_kt = eng.kernel_times(reset=True)
+        if nr:                                   # keep only pure cached steps in the accumulators
+            continue
+        n_cached += 1
+        works = work
+        for k, (n, t) in step_kt.items():
+            a = kt.get(k, (0, 0.0))
+            kt[k] = (a[0] + n, a[1] + t)
+    eng.set_option(pkg.OPT_KERNEL_TIMING, 0)
+    if not n_cached:
+        return None, None
+    tot = sum(us for _, us in kt.values())
+    kernels = {k: {"launches_per_step": n / n_cached, "us_per_step": us / n_cached, "share": us / tot} for k, (n, us) in kt.items()}
+    gemm = [k for k in kt if k.startswith("gemm_") or k == "lmhead"]
+    g_launch = sum(kt[k][0] for k in gemm)
+    g_us = sum(kt[k][1] for k in gemm)
+    T = sum(s.block_len for s in run.specs)
+    w_bytes = works["weight_bytes"]
+    flops = works["flops_linear"]
+    t_b = w_bytes / (peaks["hbm_gbs"] * 1e9)
+    t_f = flops / (peaks["bf16_tflops_sustained"] * 1e12)
+    per_launch_s = g_us * 1e-6 / g_launch
+    if t_b >= t_f:
+        ach = w_bytes / (g_launch / n_cached) / per_launch_s * 1e-9
+        rf = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"]}
+    else:
+        ach = flops / (g_launch / n_cached) / per_launch_s * 1e-12
+        rf = {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"]}
+    rf.update({"traffic": None, "kernel": "gemm_tc_kernel (QKV, O, gate/up+SwiGLU, down, LM-head epilogues) inside cached steps",
+               "launches_per_step": g_launch / n_cached, "avg_launch_us": per_launch_s * 1e6, "share_of_step": g_us / tot,
+               "algorithmic": f"weights streamed once per step ({w_bytes * 1e-9:.2f} GB bf16) / GEMM launches; tokens per step T={T}",
+               "peak_source": peaks["source"], "steps_sampled": n_cached})
+    return rf, kernels
+
+
+if __name__ == "__main__":
+    main()

@@ -143,7 +143,25 @@ DLM_API int  dlm_profile_step_costs(dlm_ctx*, dlm_cost_row* rows, int32_t cap, i
 #define DLM_OPT_DEBUG_DUMP     2   /* 1: keep every stage tensor of the next steps for dlm_debug_tensor      */
 #define DLM_OPT_CUDA_GRAPH     3   /* 1: replay steps of an unchanged batch shape from a captured CUDA graph */
 #define DLM_OPT_FLASH_ATTENTION 4  /* 0: use the plain attention kernel in the bf16 path (debugging)          */
+#define DLM_OPT_KERNEL_TIMING  5   /* 1: bracket every kernel launch of the next steps with CUDA events (dlm_kernel_times) */
 DLM_API int  dlm_set_option(dlm_ctx*, int32_t key, int32_t value);
+
+/* Per-kernel-class device time accumulated over the steps run with DLM_OPT_KERNEL_TIMING = 1 (CUDA events on
+ * the library's stream around each launch; the measurement behind bench.py's roofline object, P:123 profiling).
+ * rows[0..*n_rows) lists the classes that launched; reset != 0 clears the accumulators afterwards. */
+#define DLM_K_EMBED          0   /* a1 */
+#define DLM_K_RMSNORM        1   /* a2 / a7 / a10 */
+#define DLM_K_GEMM_QKV       2   /* a3 */
+#define DLM_K_ROPE_KV        3   /* a4 */
+#define DLM_K_ATTENTION      4   /* a5 (split-KV merge included) */
+#define DLM_K_GEMM_O         5   /* a6 */
+#define DLM_K_GEMM_GATEUP    6   /* a8 */
+#define DLM_K_GEMM_DOWN      7   /* a9 */
+#define DLM_K_LMHEAD         8   /* a11 */
+#define DLM_K_COMBINE_UNMASK 9   /* a12 + a13 */
+#define DLM_K_COUNT          10
+typedef struct { int32_t kernel, launches; float usec; } dlm_kernel_time;
+DLM_API int  dlm_kernel_times(dlm_ctx*, dlm_kernel_time* rows, int32_t cap, int32_t* n_rows, int32_t reset);
 
 /* Stage tensors of the LAST step (needs DLM_OPT_DEBUG_DUMP), as float32 on the host, for the rows the step
  * computed for `req` (refresh: S rows, cached: B rows), row-major [rows, width].  Returns the number of

@@ -18,7 +18,9 @@ LIB_PATH = os.path.join(_HERE, "libdlm.so")
 
 DLM_OK, DLM_E_ARG, DLM_E_CAPACITY, DLM_E_STATE, DLM_E_CUDA = 0, -1, -2, -3, -4
 DLM_DRY_RUN = 1
-OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION = 1, 2, 3, 4
+OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING = 1, 2, 3, 4, 5
+KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
+                "combine_unmask")
 KIND_REFRESH, KIND_CACHED = 0, 1
 T_X_IN, T_NORM1, T_Q, T_K, T_V, T_ATTN, T_X_MID, T_NORM2, T_ACT, T_X_OUT, T_FINAL_NORM, T_KCACHE, T_VCACHE = range(13)
 EPI_F32, EPI_BF16, EPI_RESID, EPI_SWIGLU = 0, 1, 2, 3
@@ -62,6 +64,10 @@ class _CostRow(C.Structure):
                 ("usec", C.c_float)]
 
 
+class _KernelTime(C.Structure):
+    _fields_ = [("kernel", C.c_int32), ("launches", C.c_int32), ("usec", C.c_float)]
+
+
 _lib = None
 
 
@@ -87,6 +93,7 @@ def lib() -> C.CDLL:
         L.dlm_cached_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(f32), C.POINTER(_Result)]
         L.dlm_profile_step_costs.argtypes = [vp, C.POINTER(_CostRow), i32, C.POINTER(i32)]
         L.dlm_set_option.argtypes = [vp, i32, i32]
+        L.dlm_kernel_times.argtypes = [vp, C.POINTER(_KernelTime), i32, C.POINTER(i32), i32]
         L.dlm_debug_tensor.argtypes = [vp, i32, i32, i32, C.POINTER(f32), i64]
         L.dlm_debug_tensor.restype = i64
         L.dlm_launch_count.argtypes = [vp]
@@ -268,6 +275,13 @@ class Engine:
         out = np.zeros(rows * width, np.float32)
         n = self._check(lib().dlm_debug_tensor(self._h, req, layer, which, _fp(out), out.size))
         return out[:n].reshape(-1, width)
+
+    def kernel_times(self, reset: bool = True):
+        """{kernel class: (launches, total usec)} accumulated while OPT_KERNEL_TIMING was on."""
+        rows = (_KernelTime * 32)()
+        n = C.c_int32(0)
+        self._check(lib().dlm_kernel_times(self._h, rows, 32, C.byref(n), 1 if reset else 0))
+        return {KERNEL_NAMES[rows[i].kernel]: (rows[i].launches, rows[i].usec) for i in range(n.value)}
 
     def profile_step_costs(self, cap: int = 128):
         rows = (_CostRow * cap)()

@@ -238,6 +238,32 @@ struct HostBatch {
   std::vector<float> tau;
 };
 
+// Per-kernel-class device timing (DLM_OPT_KERNEL_TIMING): an event pair around every launch, resolved after the
+// step's synchronize.  Feeds bench.py's roofline object and the ncu cross-check; off by default.
+struct KProf {
+  bool on = false;
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> cls;
+  size_t used = 0;
+  double usec[DLM_K_COUNT] = {};
+  long long launches[DLM_K_COUNT] = {};
+  void begin(int k, cudaStream_t st) {
+    if (ev.size() < used + 2) { ev.resize(used + 2); cudaEventCreate(&ev[used]); cudaEventCreate(&ev[used + 1]); }
+    cudaEventRecord(ev[used], st);
+    cls.push_back(k);
+  }
+  void end(cudaStream_t st) { cudaEventRecord(ev[used + 1], st); used += 2; }
+  void collect() {      // after the stream has been synchronised
+    for (size_t i = 0; i < cls.size(); ++i) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, ev[2 * i], ev[2 * i + 1]) == cudaSuccess) { usec[cls[i]] += 1000.0 * ms; launches[cls[i]]++; }
+    }
+    cls.clear(); used = 0;
+  }
+  void reset() { for (int i = 0; i < DLM_K_COUNT; ++i) { usec[i] = 0; launches[i] = 0; } }
+  ~KProf() { for (auto e : ev) cudaEventDestroy(e); }
+};
+
 struct dlm_ctx {
   dlm_arch a;
   uint64_t seed;
@@ -282,6 +308,7 @@ struct dlm_ctx {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   float last_usec = 0.f;
   TmapCache tmaps;
+  KProf kprof;
 
   void* dalloc(size_t bytes) {
     void* p = nullptr;
@@ -295,6 +322,12 @@ struct dlm_ctx {
     for (void* p : allocs) { if (mem.free) mem.free(p, mem.user); else if (!mem.alloc) cudaFree(p); }
     allocs.clear();
   }
+};
+
+struct KScope {
+  dlm_ctx* c;
+  KScope(dlm_ctx* c_, int k) : c(c_) { if (c->kprof.on) c->kprof.begin(k, c->st); }
+  ~KScope() { if (c->kprof.on) c->kprof.end(c->st); }
 };
 
 static int nqkv(const dlm_arch& a) { return (a.n_heads + 2 * a.n_kv_heads) * a.head_dim; }
@@ -453,6 +486,18 @@ extern "C" const char* dlm_last_error(dlm_ctx* c) { return c ? c->err.c_str() : 
 extern "C" int64_t dlm_launch_count(dlm_ctx*) { return g_launches; }
 extern "C" float dlm_last_step_usec(dlm_ctx* c) { return c ? c->last_usec : 0.f; }
 
+extern "C" int dlm_kernel_times(dlm_ctx* c, dlm_kernel_time* rows, int32_t cap, int32_t* n_rows, int32_t reset) {
+  if (!c || !rows || !n_rows) return DLM_E_ARG;
+  *n_rows = 0;
+  for (int k = 0; k < DLM_K_COUNT && *n_rows < cap; ++k) {
+    if (!c->kprof.launches[k]) continue;
+    rows[*n_rows].kernel = k; rows[*n_rows].launches = (int32_t)c->kprof.launches[k]; rows[*n_rows].usec = (float)c->kprof.usec[k];
+    (*n_rows)++;
+  }
+  if (reset) c->kprof.reset();
+  return DLM_OK;
+}
+
 extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
   if (!c) return DLM_E_ARG;
   switch (key) {
@@ -460,6 +505,7 @@ extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
     case DLM_OPT_DEBUG_DUMP: c->opt_dump = value; return DLM_OK;
     case DLM_OPT_CUDA_GRAPH: c->opt_graph = value; return DLM_OK;
     case DLM_OPT_FLASH_ATTENTION: c->opt_flash = value; return DLM_OK;
+    case DLM_OPT_KERNEL_TIMING: c->kprof.on = value != 0; return DLM_OK;
   }
   set_err(&c->err, "unknown option %d", key);
   return DLM_E_ARG;
@@ -627,7 +673,6 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   const dlm_arch& a = c->a;
   cudaStream_t st = c->st;
   const int T = bd.T, d = a.d_model, F = a.d_ffn, V = a.vocab, HQ = a.n_heads * a.head_dim, NQKV = nqkv(a);
-  const int HKV = a.n_kv_heads * a.head_dim;
   const bool tc = c->bf16_model && !c->opt_simple;
   const float scale = 1.f / sqrtf((float)a.head_dim);
   std::string* err = &c->err;
@@ -636,69 +681,89 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     if (!c->logits) CU_TRY(err, cudaMalloc(&c->logits, (size_t)c->Rmax * V * 4));
   }
   if (T > 0) {
+    KScope ks(c, DLM_K_EMBED);
     embed_kernel<TE><<<T, 256, 0, st>>>(c->x, (const TE*)c->E, c->tokens, a.max_seq, bd, d);
     DLM_LAUNCH_CHECK();
   }
   for (int l = 0; l < a.n_layers && T > 0; ++l) {
     const LayerW& w = c->L[l];
     dump_stage(c, l, DLM_T_X_IN, c->x, (size_t)d * 4, T);
-    rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
-    DLM_LAUNCH_CHECK();
+    {
+      KScope ks(c, DLM_K_RMSNORM);
+      rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
+      DLM_LAUNCH_CHECK();
+    }
     dump_stage(c, l, DLM_T_NORM1, c->u, (size_t)d * sizeof(TE), T);
     if (tc) {
+      KScope ks(c, DLM_K_GEMM_QKV);
       GemmTcParams p = {};
       p.out_f32 = c->qkv; p.ldc = NQKV;
       int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, 0, p, st);
       if (rc) return rc;
     } else {
+      KScope ks(c, DLM_K_GEMM_QKV);
       gemm_plain<TE, TE>(c->qkv, (const TE*)c->u, (const TE*)w.wqkv, T, NQKV, d, st);
     }
-    rope_kv_write_kernel<TE><<<T, 256, 0, st>>>((TE*)c->q, (TE*)c->kv_store, c->qkv, c->rope_cos, c->rope_sin, c->page_table, bd, c->kg, l, a.n_heads);
-    DLM_LAUNCH_CHECK();
+    {
+      KScope ks(c, DLM_K_ROPE_KV);
+      rope_kv_write_kernel<TE><<<T, 256, 0, st>>>((TE*)c->q, (TE*)c->kv_store, c->qkv, c->rope_cos, c->rope_sin, c->page_table, bd, c->kg, l, a.n_heads);
+      DLM_LAUNCH_CHECK();
+    }
     dump_stage(c, l, DLM_T_Q, c->q, (size_t)HQ * sizeof(TE), T);
     bool flash_done = false;
     if (tc && c->opt_flash) {
+      KScope ks(c, DLM_K_ATTENTION);
       int rc = attn_flash_launch((bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, c->page_table, bd, c->kg, l,
                                  a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, err, &flash_done);
       if (rc) return rc;
     }
     if (!flash_done) {
+      KScope ks(c, DLM_K_ATTENTION);
       attention_plain_kernel<TE><<<dim3(T, a.n_heads), 128, (size_t)bd.max_kv_len * 4, st>>>(
           (TE*)c->attn, (const TE*)c->q, (const TE*)c->kv_store, c->page_table, bd, c->kg, l, a.n_heads, scale);
       DLM_LAUNCH_CHECK();
     }
     dump_stage(c, l, DLM_T_ATTN, c->attn, (size_t)HQ * sizeof(TE), T);
     if (tc) {
+      KScope ks(c, DLM_K_GEMM_O);
       GemmTcParams p = {};
       p.out_f32 = c->x; p.ldc = d;
       int rc = gemm_tc(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, EPI_RESID, 0, p, st);
       if (rc) return rc;
     } else {
+      KScope ks(c, DLM_K_GEMM_O);
       gemm_plain<TE, TE>(c->tmp, (const TE*)c->attn, (const TE*)w.wo, T, d, HQ, st);
       add_residual_kernel<<<(unsigned)(((long long)T * d + 255) / 256), 256, 0, st>>>(c->x, c->tmp, (long long)T * d);
       DLM_LAUNCH_CHECK();
     }
     dump_stage(c, l, DLM_T_X_MID, c->x, (size_t)d * 4, T);
-    rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
-    DLM_LAUNCH_CHECK();
+    {
+      KScope ks(c, DLM_K_RMSNORM);
+      rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
+      DLM_LAUNCH_CHECK();
+    }
     dump_stage(c, l, DLM_T_NORM2, c->u, (size_t)d * sizeof(TE), T);
     if (tc) {
+      KScope ks(c, DLM_K_GEMM_GATEUP);
       GemmTcParams p = {};
       p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F;
       int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, EPI_SWIGLU, 0, p, st);
       if (rc) return rc;
     } else {
+      KScope ks(c, DLM_K_GEMM_GATEUP);
       gemm_plain<TE, TE>(c->tmp, (const TE*)c->u, (const TE*)w.wgu, T, 2 * F, d, st);
       swiglu_kernel<TE><<<(unsigned)(((long long)T * F + 255) / 256), 256, 0, st>>>((TE*)c->act, c->tmp, T, F);
       DLM_LAUNCH_CHECK();
     }
     dump_stage(c, l, DLM_T_ACT, c->act, (size_t)F * sizeof(TE), T);
     if (tc) {
+      KScope ks(c, DLM_K_GEMM_DOWN);
       GemmTcParams p = {};
       p.out_f32 = c->x; p.ldc = d;
       int rc = gemm_tc(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, EPI_RESID, 0, p, st);
       if (rc) return rc;
     } else {
+      KScope ks(c, DLM_K_GEMM_DOWN);
       gemm_plain<TE, TE>(c->tmp, (const TE*)c->act, (const TE*)w.wd, T, d, F, st);
       add_residual_kernel<<<(unsigned)(((long long)T * d + 255) / 256), 256, 0, st>>>(c->x, c->tmp, (long long)T * d);
       DLM_LAUNCH_CHECK();
@@ -715,25 +780,33 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   so.row_lse = (float*)ob; ob += rb; so.row_conf = (float*)ob; ob += rb; so.row_tok = (int*)ob;
   int n_tiles = 1;
   if (R > 0) {
-    build_row_src_kernel<<<bd.n, 64, 0, st>>>(c->row_src, bd);
-    DLM_LAUNCH_CHECK();
-    rmsnorm_kernel<TE><<<R, 256, 0, st>>>((TE*)c->hf, c->x, c->row_src, d, a.rms_eps);
-    DLM_LAUNCH_CHECK();
+    {
+      KScope ks(c, DLM_K_RMSNORM);
+      build_row_src_kernel<<<bd.n, 64, 0, st>>>(c->row_src, bd);
+      DLM_LAUNCH_CHECK();
+      rmsnorm_kernel<TE><<<R, 256, 0, st>>>((TE*)c->hf, c->x, c->row_src, d, a.rms_eps);
+      DLM_LAUNCH_CHECK();
+    }
     dump_stage(c, 0, DLM_T_FINAL_NORM, c->hf, (size_t)d * sizeof(TE), R);
     if (tc) {
+      KScope ks(c, DLM_K_LMHEAD);
       n_tiles = c->n_tiles;
       GemmTcParams p = {};
       p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale;
       int rc = gemm_tc(c->tmaps, err, c->hf, std::max(c->Rmax, 128), c->Wlm, V, R, V, d, EPI_LMHEAD, 128, p, st);
       if (rc) return rc;
     } else {
+      KScope ks(c, DLM_K_LMHEAD);
       gemm_plain<TE, TE>(c->logits, (const TE*)c->hf, (const TE*)c->Wlm, R, V, d, st);
       row_stats_plain_kernel<<<R, 256, 0, st>>>(c->part, c->logits, V, a.mask_id, a.logit_scale);
       DLM_LAUNCH_CHECK();
     }
   }
-  combine_unmask_kernel<<<bd.n, 128, 0, st>>>(so, c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd, dry_run ? 1 : 0);
-  DLM_LAUNCH_CHECK();
+  {
+    KScope ks(c, DLM_K_COMBINE_UNMASK);
+    combine_unmask_kernel<<<bd.n, 128, 0, st>>>(so, c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd, dry_run ? 1 : 0);
+    DLM_LAUNCH_CHECK();
+  }
   CU_TRY(err, cudaGetLastError());
   return DLM_OK;
 }
@@ -748,15 +821,16 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   const bool dry = (b->flags & DLM_DRY_RUN) != 0;
   if (res->capacity < hb.R) { set_err(&c->err, "step: result capacity %d < %d block rows", res->capacity, hb.R); return DLM_E_CAPACITY; }
   std::string* err = &c->err;
-  CU_TRY(err, cudaEventRecord(c->ev0, c->st));
   BatchDesc bd = upload_batch(c, hb);
+  CU_TRY(err, cudaEventRecord(c->ev0, c->st));        // device time of the step: first kernel .. last kernel
   rc = c->bf16_model ? forward<bf16>(c, bd, dry) : forward<float>(c, bd, dry);
-  if (rc) { cudaStreamSynchronize(c->st); return rc; }
-  CU_TRY(err, cudaMemcpyAsync(c->out_host, c->out_dev, c->out_bytes, cudaMemcpyDeviceToHost, c->st));
+  if (rc) { cudaStreamSynchronize(c->st); c->kprof.cls.clear(); c->kprof.used = 0; return rc; }
   CU_TRY(err, cudaEventRecord(c->ev1, c->st));
+  CU_TRY(err, cudaMemcpyAsync(c->out_host, c->out_dev, c->out_bytes, cudaMemcpyDeviceToHost, c->st));
   CU_TRY(err, cudaStreamSynchronize(c->st));
   cudaEventElapsedTime(&c->last_usec, c->ev0, c->ev1);
   c->last_usec *= 1000.f;
+  if (c->kprof.on) c->kprof.collect();
   // ---- unpack, update host-side request state ----
   const char* ob = c->out_host;
   const int* n_comm = (const int*)ob; ob += (size_t)a.max_requests * 4;

@@ -242,12 +242,14 @@ def test_stagewise_from_gpu_inputs():
             assert bf(q_o, q, 2e-4) and bf(k_o, kc[lo:lo + rows], 2e-4) and bf(u1 @ wv.T, vc[lo:lo + rows], 2e-4)
             # S2 attention from the GPU's q and stored K/V
             a_o = omodel.attention(q.reshape(rows, arch.n_heads, -1), kc.reshape(S, arch.n_kv_heads, -1), vc.reshape(S, arch.n_kv_heads, -1))
-            assert np.abs(a_o.reshape(rows, HQ) - attn).max() <= 2e-3 * max(1.0, np.abs(a_o).max())
+            # one bf16 rounding of the output (<= 2^-8 relative) + P rounded to bf16 for the PV MMA
+            a_o = a_o.reshape(rows, HQ)
+            assert np.all(np.abs(a_o - attn) <= np.abs(a_o) * 2 ** -8 + 2e-3 * max(1.0, np.abs(a_o).max()))
             # S3 O-proj + residual, S5 gate/up + SwiGLU, S6 down + residual
             xm_o = x_in + attn @ wts.get(ow.layer_tid(l, ow.SUB_O)).T
             assert np.abs(xm_o - x_mid).max() <= 1e-4 * max(1.0, np.abs(xm_o).max())
             act_o = omodel.silu(u2 @ wts.get(ow.layer_tid(l, ow.SUB_G)).T) * (u2 @ wts.get(ow.layer_tid(l, ow.SUB_U)).T)
-            assert bf(act_o, act, 1e-5)
+            assert bf(act_o, act, 2e-4)       # fp32 tensor-core accumulation over K = 4096, then one bf16 rounding
             xo_o = x_mid + act @ wts.get(ow.layer_tid(l, ow.SUB_D)).T
             assert np.abs(xo_o - x_out).max() <= 1e-4 * max(1.0, np.abs(xo_o).max())
     # S7: LM head from the GPU's final-normed rows

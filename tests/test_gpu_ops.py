@@ -91,11 +91,11 @@ def test_lmhead_stats(R, V, K, mask_id):
     z = scale * (h @ w.T)
     z[:, mask_id] = -np.inf
     tok_o, conf_o, lse_o, margin = omodel.confidence(z)
-    assert tok_o[0] == min(i1, i2) and margin[0] == 0.0
+    assert tok_o[0] in (i1, i2) and abs(margin[0]) < 1e-12      # a tie up to BLAS summation order in fp64
     tok, conf, lse = pkg.op_lmhead_bf16(H, W, scale, mask_id)
     torch.cuda.synchronize()
     tok, conf, lse = tok.cpu().numpy(), conf.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
-    assert tok[0] == min(i1, i2)
+    assert tok[0] == min(i1, i2)                                 # exact tie on the device -> lowest id (G8)
     clear = margin >= 1e-3
     assert np.array_equal(tok[clear], tok_o[clear])
     assert (tok != mask_id).all() and (tok >= 0).all() and (tok < V).all()
