@@ -141,9 +141,11 @@ DLM_API int  dlm_profile_step_costs(dlm_ctx*, dlm_cost_row* rows, int32_t cap, i
 #define DLM_OPT_SIMPLE_KERNELS 1   /* 1: run the bf16 model through the plain SIMT kernels (on-device debugging
                                       reference; same rounding points as the tcgen05 path; not a CPU fallback) */
 #define DLM_OPT_DEBUG_DUMP     2   /* 1: keep every stage tensor of the next steps for dlm_debug_tensor      */
-#define DLM_OPT_CUDA_GRAPH     3   /* 1: replay steps of an unchanged batch shape from a captured CUDA graph */
+#define DLM_OPT_CUDA_GRAPH     3   /* 1 (default): replay steps of a batch shape seen before from a captured CUDA graph */
 #define DLM_OPT_FLASH_ATTENTION 4  /* 0: use the plain attention kernel in the bf16 path (debugging)          */
 #define DLM_OPT_KERNEL_TIMING  5   /* 1: bracket every kernel launch of the next steps with CUDA events (dlm_kernel_times) */
+#define DLM_OPT_PDL            6   /* 1 (default): programmatic dependent launch between the kernels of a step           */
+#define DLM_OPT_SKINNY_GEMM    7   /* 1 (default): weight-streaming split-K GEMM for steps of <= 128 tokens; 0: tile GEMM */
 DLM_API int  dlm_set_option(dlm_ctx*, int32_t key, int32_t value);
 
 /* Per-kernel-class device time accumulated over the steps run with DLM_OPT_KERNEL_TIMING = 1 (CUDA events on

@@ -27,6 +27,13 @@ extern "C" {
 DLM_API int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epilogue,
                      int32_t bn, void* stream);
 
+/* Weight-streaming split-K tcgen05 GEMM for T <= 128 tokens (the cached step's a3/a6/a8/a9): swap-AB (weights on
+ * the MMA's M side, tokens on N), every K split writes an fp32 slice and the slices are summed in a fixed order.
+ * epilogue DLM_EPI_F32: out fp32 [T, N] = X . W^T; DLM_EPI_SWIGLU: out bf16 [T, N], W = [2N, K] (gate rows, up rows).
+ * splits = 0 picks the split the engine would use; returns the number of K splits used (>= 1) or a DLM_E_* code. */
+DLM_API int dlm_op_gemm_skinny_bf16(const void* X, const void* W, void* out, int32_t T, int32_t N, int32_t K, int32_t epilogue,
+                            int32_t splits, void* stream);
+
 /* Same contraction on the plain SIMT kernel (debugging reference of the engine; fp32 out only). */
 DLM_API int dlm_op_gemm_plain_bf16(const void* A, const void* W, float* out, int32_t M, int32_t N, int32_t K, void* stream);
 

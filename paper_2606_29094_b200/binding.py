@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libdlm.so")
 
 DLM_OK, DLM_E_ARG, DLM_E_CAPACITY, DLM_E_STATE, DLM_E_CUDA = 0, -1, -2, -3, -4
 DLM_DRY_RUN = 1
-OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING = 1, 2, 3, 4, 5
+OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM = 1, 2, 3, 4, 5, 6, 7
 KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
                 "combine_unmask")
 KIND_REFRESH, KIND_CACHED = 0, 1
@@ -104,6 +104,7 @@ def lib() -> C.CDLL:
         L.dlm_last_error.restype = C.c_char_p
         L.dlm_op_gemm_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
         L.dlm_op_gemm_plain_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp]
+        L.dlm_op_gemm_skinny_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
         L.dlm_op_lmhead_scratch_bytes.argtypes = [i32, i32]
         L.dlm_op_lmhead_scratch_bytes.restype = i64
         L.dlm_op_lmhead_bf16.argtypes = [vp, vp, i32, i32, i32, f32, i32, vp, vp, vp, vp, vp]
@@ -312,6 +313,17 @@ def op_gemm_bf16(A, W, epilogue: int = EPI_F32, bn: int = 0, out=None):
         out = torch.empty(M, N, device=A.device, dtype=torch.float32 if epilogue in (EPI_F32, EPI_RESID) else torch.bfloat16)
     _op_check(lib().dlm_op_gemm_bf16(A.data_ptr(), W.data_ptr(), out.data_ptr(), M, N, K, epilogue, bn, _stream_ptr()))
     return out
+
+
+def op_gemm_skinny_bf16(X, W, epilogue: int = EPI_F32, splits: int = 0):
+    """Returns (out, K splits used)."""
+    import torch
+    T, K = X.shape
+    N = W.shape[0] // 2 if epilogue == EPI_SWIGLU else W.shape[0]
+    out = torch.empty(T, N, device=X.device, dtype=torch.float32 if epilogue == EPI_F32 else torch.bfloat16)
+    rc = lib().dlm_op_gemm_skinny_bf16(X.data_ptr(), W.data_ptr(), out.data_ptr(), T, N, K, epilogue, splits, _stream_ptr())
+    _op_check(rc)
+    return out, rc
 
 
 def op_gemm_plain_bf16(A, W):

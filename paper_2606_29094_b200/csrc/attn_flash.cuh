@@ -65,6 +65,8 @@ struct FaParams {
 
 __global__ void __launch_bounds__(kFaThreads) attn_flash_kernel(const FaParams p) {
   extern __shared__ __align__(128) uint8_t fa_smem[];
+  pdl_launch_dependents();
+  pdl_wait();
   const int bi = blockIdx.z / p.splits, split = blockIdx.z % p.splits;
   const int kvh = blockIdx.y;
   const int r = p.n_heads / p.g.n_kv_heads;
@@ -221,6 +223,8 @@ __global__ void __launch_bounds__(kFaThreads) attn_flash_kernel(const FaParams p
 // merge split partials: out = sum_s o_s 2^(m_s - m) / sum_s l_s 2^(m_s - m)
 __global__ void __launch_bounds__(kFaDh) attn_combine_kernel(bf16* __restrict__ out, const float* __restrict__ ws_o,
                                                              const float* __restrict__ ws_ml, long long TH, int splits) {
+  pdl_launch_dependents();
+  pdl_wait();
   const long long row = blockIdx.x;
   const int e = threadIdx.x;
   float m = -CUDART_INF_F;
@@ -239,7 +243,7 @@ __global__ void __launch_bounds__(kFaDh) attn_combine_kernel(bf16* __restrict__ 
 // Host launcher.  *done = false when the shape is not supported (caller falls back to the plain kernel).
 static int attn_flash_launch(bf16* out, const bf16* q, const bf16* kv_store, const int* page_table, const BatchDesc& bd,
                              const KvGeom& g, int layer, int n_heads, float scale, float** ws, size_t* ws_bytes, int num_sms,
-                             cudaStream_t st, std::string* err, bool* done) {
+                             cudaStream_t st, bool pdl, std::string* err, bool* done) {
   *done = false;
   if (g.head_dim != kFaDh || g.page_tokens % kFaBN != 0 || bd.T <= 0) return 0;
   static bool configured = false;
@@ -271,13 +275,19 @@ static int attn_flash_launch(bf16* out, const bf16* q, const bf16* kv_store, con
     p.ws_ml = *ws + (size_t)splits * TH * kFaDh;
   }
   dim3 grid(q_tiles, g.n_kv_heads, bd.n * splits);
-  attn_flash_kernel<<<grid, kFaThreads, kFaSmem, st>>>(p);
+  cudaLaunchConfig_t cfg = {};
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.stream = st; cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  cfg.gridDim = grid; cfg.blockDim = dim3(kFaThreads); cfg.dynamicSmemBytes = kFaSmem;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, attn_flash_kernel, p);
   DLM_LAUNCH_CHECK();
-  if (splits > 1) {
-    attn_combine_kernel<<<(unsigned)TH, kFaDh, 0, st>>>(out, p.ws_o, p.ws_ml, TH, splits);
+  if (splits > 1 && e == cudaSuccess) {
+    cfg.gridDim = dim3((unsigned)TH); cfg.blockDim = dim3(kFaDh); cfg.dynamicSmemBytes = 0;
+    e = cudaLaunchKernelEx(&cfg, attn_combine_kernel, out, (const float*)p.ws_o, (const float*)p.ws_ml, TH, splits);
     DLM_LAUNCH_CHECK();
   }
-  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { *err = std::string("attn_flash launch: ") + cudaGetErrorString(e); return -4; }
   *done = true;
   return 0;

@@ -28,6 +28,11 @@ __device__ __forceinline__ float warp_max(float v) {
   return v;
 }
 
+// Programmatic dependent launch (PDL): every kernel of a step lets its successor start early and waits for its
+// predecessor's results right before it first touches them.  Both are no-ops for a plain launch.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // Per-step ragged batch descriptor, built on the host, copied once per step (a0 in DESIGN.md).
 // Request i of the batch computes q_len[i] consecutive positions starting at absolute position q_pos0[i];
 // its rows live at [q_off[i], q_off[i]+q_len[i]) of every [T, *] activation buffer.

@@ -18,6 +18,7 @@
 #include "../../include/dlm_ops.h"
 #include "attn_flash.cuh"
 #include "common.cuh"
+#include "gemm_skinny.cuh"
 #include "gemm_tc.cuh"
 #include "kernels_basic.cuh"
 
@@ -32,6 +33,22 @@ static void set_err(std::string* dst, const char* fmt, ...) {
   vsnprintf(buf, sizeof buf, fmt, ap);
   va_end(ap);
   *dst = buf;
+}
+
+// One launch path for every kernel of a step: a plain launch, or a programmatic dependent launch (PDL) whose
+// prologue (and, for the GEMMs, weight prefetch) overlaps the tail of the previous kernel in the stream.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  if (pdl) {
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+  }
+  g_launches++;
+  return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
 }
 
 #define CU_TRY(ctx_err, expr)                                                                         \
@@ -108,7 +125,7 @@ static int pick_bn(int M, int N, int epi) {
 
 template <int EPI>
 static cudaError_t launch_gemm_tc_t(const CUtensorMap* ma, const CUtensorMap* mb, const GemmTcParams& p, int n_tiles_x,
-                                    cudaStream_t st) {
+                                    cudaStream_t st, bool pdl) {
   static int configured = 0;
   const int smem = gemm_tc_smem_bytes(p.bn, p.stages);
   if (configured < smem) {
@@ -117,14 +134,12 @@ static cudaError_t launch_gemm_tc_t(const CUtensorMap* ma, const CUtensorMap* mb
     configured = 227 * 1024;
   }
   dim3 grid(n_tiles_x, (p.M + 127) / 128);
-  gemm_tc_kernel<EPI><<<grid, kGemmThreads, smem, st>>>(*ma, *mb, p);
-  DLM_LAUNCH_CHECK();
-  return cudaGetLastError();
+  return launch_k(gemm_tc_kernel<EPI>, grid, dim3(kGemmThreads), (size_t)smem, st, pdl, *ma, *mb, p);
 }
 
 // A: bf16 [a_rows_cap, K] buffer (M valid rows); W: bf16 [w_rows, K].
 static int gemm_tc(TmapCache& tc, std::string* err, const void* A, long long a_rows_cap, const void* W, long long w_rows,
-                   int M, int N, int K, int epi, int bn, GemmTcParams p, cudaStream_t st) {
+                   int M, int N, int K, int epi, int bn, GemmTcParams p, cudaStream_t st, bool pdl = false) {
   if (M <= 0) return DLM_OK;
   if (K % 8) { set_err(err, "gemm_tc: K=%d must be a multiple of 8", K); return DLM_E_ARG; }
   if (epi != EPI_LMHEAD && p.ldc % 8) { set_err(err, "gemm_tc: output row pitch %lld must be a multiple of 8 elements", p.ldc); return DLM_E_ARG; }
@@ -143,23 +158,72 @@ static int gemm_tc(TmapCache& tc, std::string* err, const void* A, long long a_r
   if (!ma || !mb) { set_err(err, "cuTensorMapEncodeTiled failed (A=%p rows=%lld K=%d, W=%p rows=%lld box=%d)", A, a_rows_cap, K, W, w_rows, per); return DLM_E_CUDA; }
   cudaError_t e;
   switch (epi) {
-    case EPI_F32: e = launch_gemm_tc_t<EPI_F32>(ma, mb, p, n_tiles_x, st); break;
-    case EPI_BF16: e = launch_gemm_tc_t<EPI_BF16>(ma, mb, p, n_tiles_x, st); break;
-    case EPI_RESID: e = launch_gemm_tc_t<EPI_RESID>(ma, mb, p, n_tiles_x, st); break;
-    case EPI_SWIGLU: e = launch_gemm_tc_t<EPI_SWIGLU>(ma, mb, p, n_tiles_x, st); break;
-    case EPI_LMHEAD: e = launch_gemm_tc_t<EPI_LMHEAD>(ma, mb, p, n_tiles_x, st); break;
+    case EPI_F32: e = launch_gemm_tc_t<EPI_F32>(ma, mb, p, n_tiles_x, st, pdl); break;
+    case EPI_BF16: e = launch_gemm_tc_t<EPI_BF16>(ma, mb, p, n_tiles_x, st, pdl); break;
+    case EPI_RESID: e = launch_gemm_tc_t<EPI_RESID>(ma, mb, p, n_tiles_x, st, pdl); break;
+    case EPI_SWIGLU: e = launch_gemm_tc_t<EPI_SWIGLU>(ma, mb, p, n_tiles_x, st, pdl); break;
+    case EPI_LMHEAD: e = launch_gemm_tc_t<EPI_LMHEAD>(ma, mb, p, n_tiles_x, st, pdl); break;
     default: set_err(err, "gemm_tc: bad epilogue %d", epi); return DLM_E_ARG;
   }
   if (e != cudaSuccess) { set_err(err, "gemm_tc launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
   return DLM_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// weight-streaming GEMM launcher (T <= 128 tokens): picks the K split so ~2 CTAs per SM stream concurrently
+// ------------------------------------------------------------------------------------------------
+constexpr int kSkMaxSplits = 16;
+constexpr int kSkMaxTokens = 128;
+
+static void skinny_plan(int T, int N, int K, int epi, int force_splits, SkinnyParams* p, int* n_tiles) {
+  const int per = epi == SK_SWIGLU ? 64 : 128;
+  *n_tiles = (N + per - 1) / per;
+  const int num_kb = (K + 63) / 64;
+  int s = force_splits > 0 ? force_splits : (2 * g_num_sms) / *n_tiles;
+  if (epi == SK_SWIGLU) s = 1;                                  // silu(g)*u needs complete sums
+  s = std::max(1, std::min(std::min(s, kSkMaxSplits), std::max(1, num_kb / 4)));
+  p->kb_per_split = (num_kb + s - 1) / s;
+  p->splits = (num_kb + p->kb_per_split - 1) / p->kb_per_split;
+  p->T = T; p->N = N; p->K = K;
+  p->tpad = (T + 31) / 32 * 32;
+  const int budget = 100 * 1024 - (epi == SK_SWIGLU ? 32 * 65 * 4 : 0);
+  p->stages = std::max(2, std::min(std::min(p->kb_per_split, 8), budget / skinny_stage_bytes(p->tpad)));
+  p->w_policy = DLM_L2_EVICT_FIRST;
+}
+
+// X: bf16 [x_rows_cap, K] (T valid rows); W: bf16 [w_rows, K].  SK_PARTIAL: p.out_f32 receives p.splits slices
+// [split][T][ldc]; *splits_out tells the consumer how many to sum.
+static int gemm_skinny(TmapCache& tc, std::string* err, const void* X, long long x_rows_cap, const void* W, long long w_rows,
+                       int T, int N, int K, int epi, int force_splits, SkinnyParams p, int* splits_out, cudaStream_t st, bool pdl) {
+  if (T <= 0) { if (splits_out) *splits_out = 0; return DLM_OK; }
+  if (T > kSkMaxTokens || K % 8 || p.ldc <= 0) { set_err(err, "gemm_skinny: bad shape T=%d K=%d", T, K); return DLM_E_ARG; }
+  int n_tiles = 0;
+  skinny_plan(T, N, K, epi, force_splits, &p, &n_tiles);
+  const CUtensorMap* mw = tc.get(W, w_rows, K, epi == SK_SWIGLU ? 64 : 128);
+  const CUtensorMap* mx = tc.get(X, x_rows_cap, K, p.tpad);
+  if (!mw || !mx) { set_err(err, "cuTensorMapEncodeTiled failed (gemm_skinny X=%p W=%p)", X, W); return DLM_E_CUDA; }
+  const int smem = skinny_smem_bytes(p.tpad, p.stages, epi);
+  static bool configured[2] = {false, false};
+  cudaError_t e = cudaSuccess;
+  if (!configured[epi]) {
+    e = epi == SK_SWIGLU ? cudaFuncSetAttribute(gemm_skinny_kernel<SK_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024)
+                         : cudaFuncSetAttribute(gemm_skinny_kernel<SK_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024);
+    if (e != cudaSuccess) { set_err(err, "gemm_skinny: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+    configured[epi] = true;
+  }
+  dim3 grid(n_tiles, p.splits);
+  e = epi == SK_SWIGLU ? launch_k(gemm_skinny_kernel<SK_SWIGLU>, grid, dim3(kSkThreads), (size_t)smem, st, pdl, *mw, *mx, p)
+                       : launch_k(gemm_skinny_kernel<SK_PARTIAL>, grid, dim3(kSkThreads), (size_t)smem, st, pdl, *mw, *mx, p);
+  if (e != cudaSuccess) { set_err(err, "gemm_skinny launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+  if (splits_out) *splits_out = p.splits;
+  return DLM_OK;
+}
+
 template <typename TA, typename TW>
-static void gemm_plain(float* C, const TA* A, const TW* W, int M, int N, int K, cudaStream_t st) {
+static void gemm_plain(float* C, const TA* A, const TW* W, int M, int N, int K, cudaStream_t st, bool pdl = false) {
   if (M <= 0) return;
   dim3 grid((N + 63) / 64, (M + 63) / 64);
-  gemm_plain_kernel<TA, TW><<<grid, 256, 0, st>>>(C, A, W, M, N, K, K, K, N);
-  DLM_LAUNCH_CHECK();
+  launch_k(gemm_plain_kernel<TA, TW>, grid, dim3(256), 0, st, pdl, C, A, W, M, N, K, K, K, N);
 }
 
 // Test op: contiguous q/k/v -> repack into a private paged store (64-token pages, identity page table) -> attention.
@@ -200,7 +264,7 @@ static int attn_op_contiguous(const void* q, const void* k, const void* v, void*
   bool done = false;
   float* ws = nullptr; size_t wsb = 0;
   if (flash) {
-    rc = attn_flash_launch((bf16*)out, (const bf16*)q, store, meta, bd, g, 0, H, scale, &ws, &wsb, g_num_sms, st, err, &done);
+    rc = attn_flash_launch((bf16*)out, (const bf16*)q, store, meta, bd, g, 0, H, scale, &ws, &wsb, g_num_sms, st, false, err, &done);
     if (!rc && !done) { set_err(err, "dlm_op_attention_bf16: flash kernel does not support d_h=%d", dh); rc = DLM_E_ARG; }
   } else {
     attention_plain_kernel<bf16><<<dim3(Tq, H), 128, (size_t)S * 4, st>>>((bf16*)out, (const bf16*)q, store, meta, bd, g, 0, H, scale);
@@ -264,6 +328,9 @@ struct KProf {
   ~KProf() { for (auto e : ev) cudaEventDestroy(e); }
 };
 
+typedef std::tuple<int, int, int, int, int, int, int, int> GraphKey;   // kind, dry, n, T, R, max_q, max_kv, options
+struct GraphEntry { int seen = 0; cudaGraphExec_t exec = nullptr; long long launches = 0; };
+
 struct dlm_ctx {
   dlm_arch a;
   uint64_t seed;
@@ -297,8 +364,11 @@ struct dlm_ctx {
   char* out_dev = nullptr; char* out_host = nullptr; size_t out_bytes = 0;
   // attention split-KV scratch
   float* attn_ws = nullptr; size_t attn_ws_bytes = 0;
+  float* part_x = nullptr;     // [kSkMaxSplits][<=128][d] split-K slices of the O / down projections
   // options
-  int opt_simple = 0, opt_dump = 0, opt_graph = 0, opt_flash = 1;
+  int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1;
+  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3); }
+  std::map<GraphKey, GraphEntry> graphs;
   // debug dump
   std::map<std::pair<int, int>, void*> dump;   // (layer, which) -> device copy [T, width]
   HostBatch last_batch;
@@ -440,7 +510,8 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   c->Rmax = a.max_requests * a.max_block;
   c->n_tiles = c->bf16_model ? (int)((V + 127) / 128) : 1;
   ALLOC(c->x, (size_t)c->Tmax * d * 4);
-  ALLOC(c->qkv, (size_t)c->Tmax * NQKV * 4);
+  ALLOC(c->qkv, (size_t)std::max<long long>(c->Tmax, (long long)kSkMaxSplits * kSkMaxTokens) * NQKV * 4);
+  if (c->bf16_model) ALLOC(c->part_x, (size_t)kSkMaxSplits * kSkMaxTokens * d * 4);
   ALLOC(c->u, (size_t)c->Tmax * d * es);
   ALLOC(c->q, (size_t)c->Tmax * HQ * es);
   ALLOC(c->attn, (size_t)c->Tmax * HQ * es);
@@ -448,7 +519,7 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   ALLOC(c->hf, (size_t)std::max(c->Rmax, 128) * d * es);
   ALLOC(c->part, (size_t)c->Rmax * std::max(c->n_tiles, 1) * sizeof(RowPartial));
   ALLOC(c->row_src, (size_t)c->Rmax * 4);
-  c->desc_cap_ints = (size_t)10 * a.max_requests + c->Tmax + 64;
+  c->desc_cap_ints = (size_t)10 * a.max_requests + c->Tmax + 64;      // 9 n + T used
   ALLOC(c->desc_dev, c->desc_cap_ints * 4);
   if (cudaMallocHost(&c->desc_host, c->desc_cap_ints * 4) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
   c->out_bytes = (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6;
@@ -470,6 +541,7 @@ extern "C" void dlm_destroy(dlm_ctx* c) {
   if (!c) return;
   if (c->st) cudaStreamSynchronize(c->st);
   for (auto& kv : c->dump) cudaFree(kv.second);
+  for (auto& g : c->graphs) if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
   if (c->tmp) cudaFree(c->tmp);
   if (c->logits) cudaFree(c->logits);
   if (c->attn_ws) cudaFree(c->attn_ws);
@@ -501,11 +573,13 @@ extern "C" int dlm_kernel_times(dlm_ctx* c, dlm_kernel_time* rows, int32_t cap, 
 extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
   if (!c) return DLM_E_ARG;
   switch (key) {
-    case DLM_OPT_SIMPLE_KERNELS: c->opt_simple = value; return DLM_OK;
+    case DLM_OPT_SIMPLE_KERNELS: c->opt_simple = value != 0; return DLM_OK;
     case DLM_OPT_DEBUG_DUMP: c->opt_dump = value; return DLM_OK;
-    case DLM_OPT_CUDA_GRAPH: c->opt_graph = value; return DLM_OK;
-    case DLM_OPT_FLASH_ATTENTION: c->opt_flash = value; return DLM_OK;
+    case DLM_OPT_CUDA_GRAPH: c->opt_graph = value != 0; return DLM_OK;
+    case DLM_OPT_FLASH_ATTENTION: c->opt_flash = value != 0; return DLM_OK;
     case DLM_OPT_KERNEL_TIMING: c->kprof.on = value != 0; return DLM_OK;
+    case DLM_OPT_PDL: c->opt_pdl = value != 0; return DLM_OK;
+    case DLM_OPT_SKINNY_GEMM: c->opt_skinny = value != 0; return DLM_OK;
   }
   set_err(&c->err, "unknown option %d", key);
   return DLM_E_ARG;
@@ -640,21 +714,24 @@ static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override
   return DLM_OK;
 }
 
-static BatchDesc upload_batch(dlm_ctx* c, const HostBatch& hb) {
+// Descriptor layout in desc_host / desc_dev (ints): slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, tau [n each],
+// then tok_bi [T].  Offsets depend on (n, T) only, so a captured graph of the same batch shape can be replayed.
+static size_t fill_desc_host(dlm_ctx* c, const HostBatch& hb) {
   int* h = c->desc_host;
-  const int n = hb.n;
-  size_t o = 0;
-  auto put = [&](const std::vector<int>& v) { memcpy(h + o, v.data(), v.size() * 4); size_t at = o; o += v.size(); return at; };
-  size_t o_slot = put(hb.slot), o_qoff = put(hb.q_off), o_qlen = put(hb.q_len), o_qpos = put(hb.q_pos0), o_kv = put(hb.kv_len),
-         o_lo = put(hb.blk_lo), o_len = put(hb.blk_len), o_row = put(hb.row_off);
-  size_t o_tau = o; memcpy(h + o, hb.tau.data(), n * 4); o += n;
-  size_t o_bi = put(hb.tok_bi);
-  cudaMemcpyAsync(c->desc_dev, h, o * 4, cudaMemcpyHostToDevice, c->st);
+  const size_t n = hb.n;
+  const std::vector<int>* v[8] = {&hb.slot, &hb.q_off, &hb.q_len, &hb.q_pos0, &hb.kv_len, &hb.blk_lo, &hb.blk_len, &hb.row_off};
+  for (int i = 0; i < 8; ++i) memcpy(h + i * n, v[i]->data(), n * 4);
+  memcpy(h + 8 * n, hb.tau.data(), n * 4);
+  memcpy(h + 9 * n, hb.tok_bi.data(), hb.tok_bi.size() * 4);
+  return 9 * n + hb.tok_bi.size();
+}
+static BatchDesc make_desc(dlm_ctx* c, const HostBatch& hb) {
   BatchDesc d;
-  d.n = n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv;
-  d.slot = c->desc_dev + o_slot; d.q_off = c->desc_dev + o_qoff; d.q_len = c->desc_dev + o_qlen; d.q_pos0 = c->desc_dev + o_qpos;
-  d.kv_len = c->desc_dev + o_kv; d.blk_lo = c->desc_dev + o_lo; d.blk_len = c->desc_dev + o_len; d.row_off = c->desc_dev + o_row;
-  d.tau = (const float*)(c->desc_dev + o_tau); d.tok_bi = c->desc_dev + o_bi;
+  const size_t n = hb.n;
+  const int* b = c->desc_dev;
+  d.n = hb.n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv;
+  d.slot = b; d.q_off = b + n; d.q_len = b + 2 * n; d.q_pos0 = b + 3 * n; d.kv_len = b + 4 * n; d.blk_lo = b + 5 * n;
+  d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.tok_bi = b + 9 * n;
   return d;
 }
 
@@ -674,100 +751,134 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   cudaStream_t st = c->st;
   const int T = bd.T, d = a.d_model, F = a.d_ffn, V = a.vocab, HQ = a.n_heads * a.head_dim, NQKV = nqkv(a);
   const bool tc = c->bf16_model && !c->opt_simple;
+  const bool skinny = tc && c->opt_skinny && T <= kSkMaxTokens;      // weight-streaming regime (cached steps of small batches)
+  const bool pdl = c->opt_pdl && !c->kprof.on;                        // event pairs between kernels would serialise anyway
   const float scale = 1.f / sqrtf((float)a.head_dim);
   std::string* err = &c->err;
   if (!tc) {   // scratch of the plain path, allocated on first use
     if (!c->tmp) CU_TRY(err, cudaMalloc(&c->tmp, (size_t)c->Tmax * std::max(d, 2 * F) * 4));
     if (!c->logits) CU_TRY(err, cudaMalloc(&c->logits, (size_t)c->Rmax * V * 4));
   }
+  int pend = 0;                                   // split-K slices of x waiting in part_x (folded into the next norm)
+  const long long pstride = (long long)T * d;
+  // in debug-dump mode x is completed right after each projection so that every dumped tensor is whole
+  auto flush_partials = [&]() {
+    if (pend > 0 && c->opt_dump) {
+      KScope ks(c, DLM_K_RMSNORM);
+      launch_k(add_partials_kernel, dim3((unsigned)((pstride + 255) / 256)), dim3(256), 0, st, pdl, c->x, (const float*)c->part_x, pend, pstride, pstride);
+      pend = 0;
+    }
+  };
   if (T > 0) {
-    KScope ks(c, DLM_K_EMBED);
-    embed_kernel<TE><<<T, 256, 0, st>>>(c->x, (const TE*)c->E, c->tokens, a.max_seq, bd, d);
-    DLM_LAUNCH_CHECK();
+    KScope ks(c, DLM_K_EMBED);                    // first kernel of the step: plain launch (stream order vs. the previous step)
+    launch_k(embed_kernel<TE>, dim3(T), dim3(256), 0, st, false, c->x, (const TE*)c->E, (const int*)c->tokens, a.max_seq, bd, d);
   }
   for (int l = 0; l < a.n_layers && T > 0; ++l) {
     const LayerW& w = c->L[l];
     dump_stage(c, l, DLM_T_X_IN, c->x, (size_t)d * 4, T);
     {
       KScope ks(c, DLM_K_RMSNORM);
-      rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
-      DLM_LAUNCH_CHECK();
+      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(256), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      pend = 0;
     }
     dump_stage(c, l, DLM_T_NORM1, c->u, (size_t)d * sizeof(TE), T);
-    if (tc) {
+    int nq = 1;                                   // slices of the qkv buffer the RoPE kernel sums
+    {
       KScope ks(c, DLM_K_GEMM_QKV);
-      GemmTcParams p = {};
-      p.out_f32 = c->qkv; p.ldc = NQKV;
-      int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, 0, p, st);
-      if (rc) return rc;
-    } else {
-      KScope ks(c, DLM_K_GEMM_QKV);
-      gemm_plain<TE, TE>(c->qkv, (const TE*)c->u, (const TE*)w.wqkv, T, NQKV, d, st);
+      if (skinny) {
+        SkinnyParams p = {};
+        p.out_f32 = c->qkv; p.ldc = NQKV;
+        int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, SK_PARTIAL, 0, p, &nq, st, pdl);
+        if (rc) return rc;
+      } else if (tc) {
+        GemmTcParams p = {};
+        p.out_f32 = c->qkv; p.ldc = NQKV;
+        int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, 0, p, st, pdl);
+        if (rc) return rc;
+      } else {
+        gemm_plain<TE, TE>(c->qkv, (const TE*)c->u, (const TE*)w.wqkv, T, NQKV, d, st, pdl);
+      }
     }
     {
       KScope ks(c, DLM_K_ROPE_KV);
-      rope_kv_write_kernel<TE><<<T, 256, 0, st>>>((TE*)c->q, (TE*)c->kv_store, c->qkv, c->rope_cos, c->rope_sin, c->page_table, bd, c->kg, l, a.n_heads);
-      DLM_LAUNCH_CHECK();
+      launch_k(rope_kv_write_kernel<TE>, dim3(T), dim3(256), 0, st, pdl, (TE*)c->q, (TE*)c->kv_store, (const float*)c->qkv, (const float*)c->rope_cos,
+               (const float*)c->rope_sin, (const int*)c->page_table, bd, c->kg, l, a.n_heads, nq, (long long)T * NQKV);
     }
     dump_stage(c, l, DLM_T_Q, c->q, (size_t)HQ * sizeof(TE), T);
     bool flash_done = false;
     if (tc && c->opt_flash) {
       KScope ks(c, DLM_K_ATTENTION);
       int rc = attn_flash_launch((bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, c->page_table, bd, c->kg, l,
-                                 a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, err, &flash_done);
+                                 a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, pdl, err, &flash_done);
       if (rc) return rc;
     }
     if (!flash_done) {
       KScope ks(c, DLM_K_ATTENTION);
-      attention_plain_kernel<TE><<<dim3(T, a.n_heads), 128, (size_t)bd.max_kv_len * 4, st>>>(
-          (TE*)c->attn, (const TE*)c->q, (const TE*)c->kv_store, c->page_table, bd, c->kg, l, a.n_heads, scale);
-      DLM_LAUNCH_CHECK();
+      launch_k(attention_plain_kernel<TE>, dim3(T, a.n_heads), dim3(128), (size_t)bd.max_kv_len * 4, st, pdl, (TE*)c->attn, (const TE*)c->q,
+               (const TE*)c->kv_store, (const int*)c->page_table, bd, c->kg, l, a.n_heads, scale);
     }
     dump_stage(c, l, DLM_T_ATTN, c->attn, (size_t)HQ * sizeof(TE), T);
-    if (tc) {
+    {
       KScope ks(c, DLM_K_GEMM_O);
-      GemmTcParams p = {};
-      p.out_f32 = c->x; p.ldc = d;
-      int rc = gemm_tc(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, EPI_RESID, 0, p, st);
-      if (rc) return rc;
-    } else {
-      KScope ks(c, DLM_K_GEMM_O);
-      gemm_plain<TE, TE>(c->tmp, (const TE*)c->attn, (const TE*)w.wo, T, d, HQ, st);
-      add_residual_kernel<<<(unsigned)(((long long)T * d + 255) / 256), 256, 0, st>>>(c->x, c->tmp, (long long)T * d);
-      DLM_LAUNCH_CHECK();
+      if (skinny) {
+        SkinnyParams p = {};
+        p.out_f32 = c->part_x; p.ldc = d;
+        int rc = gemm_skinny(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, SK_PARTIAL, 0, p, &pend, st, pdl);
+        if (rc) return rc;
+      } else if (tc) {
+        GemmTcParams p = {};
+        p.out_f32 = c->x; p.ldc = d;
+        int rc = gemm_tc(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, EPI_RESID, 0, p, st, pdl);
+        if (rc) return rc;
+      } else {
+        gemm_plain<TE, TE>(c->tmp, (const TE*)c->attn, (const TE*)w.wo, T, d, HQ, st, pdl);
+        launch_k(add_residual_kernel, dim3((unsigned)(((long long)T * d + 255) / 256)), dim3(256), 0, st, pdl, c->x, (const float*)c->tmp, (long long)T * d);
+      }
     }
+    flush_partials();
     dump_stage(c, l, DLM_T_X_MID, c->x, (size_t)d * 4, T);
     {
       KScope ks(c, DLM_K_RMSNORM);
-      rmsnorm_kernel<TE><<<T, 256, 0, st>>>((TE*)c->u, c->x, nullptr, d, a.rms_eps);
-      DLM_LAUNCH_CHECK();
+      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(256), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      pend = 0;
     }
     dump_stage(c, l, DLM_T_NORM2, c->u, (size_t)d * sizeof(TE), T);
-    if (tc) {
+    {
       KScope ks(c, DLM_K_GEMM_GATEUP);
-      GemmTcParams p = {};
-      p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F;
-      int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, EPI_SWIGLU, 0, p, st);
-      if (rc) return rc;
-    } else {
-      KScope ks(c, DLM_K_GEMM_GATEUP);
-      gemm_plain<TE, TE>(c->tmp, (const TE*)c->u, (const TE*)w.wgu, T, 2 * F, d, st);
-      swiglu_kernel<TE><<<(unsigned)(((long long)T * F + 255) / 256), 256, 0, st>>>((TE*)c->act, c->tmp, T, F);
-      DLM_LAUNCH_CHECK();
+      if (skinny) {
+        SkinnyParams p = {};
+        p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F;
+        int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, SK_SWIGLU, 0, p, nullptr, st, pdl);
+        if (rc) return rc;
+      } else if (tc) {
+        GemmTcParams p = {};
+        p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F;
+        int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, EPI_SWIGLU, 0, p, st, pdl);
+        if (rc) return rc;
+      } else {
+        gemm_plain<TE, TE>(c->tmp, (const TE*)c->u, (const TE*)w.wgu, T, 2 * F, d, st, pdl);
+        launch_k(swiglu_kernel<TE>, dim3((unsigned)(((long long)T * F + 255) / 256)), dim3(256), 0, st, pdl, (TE*)c->act, (const float*)c->tmp, T, F);
+      }
     }
     dump_stage(c, l, DLM_T_ACT, c->act, (size_t)F * sizeof(TE), T);
-    if (tc) {
+    {
       KScope ks(c, DLM_K_GEMM_DOWN);
-      GemmTcParams p = {};
-      p.out_f32 = c->x; p.ldc = d;
-      int rc = gemm_tc(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, EPI_RESID, 0, p, st);
-      if (rc) return rc;
-    } else {
-      KScope ks(c, DLM_K_GEMM_DOWN);
-      gemm_plain<TE, TE>(c->tmp, (const TE*)c->act, (const TE*)w.wd, T, d, F, st);
-      add_residual_kernel<<<(unsigned)(((long long)T * d + 255) / 256), 256, 0, st>>>(c->x, c->tmp, (long long)T * d);
-      DLM_LAUNCH_CHECK();
+      if (skinny) {
+        SkinnyParams p = {};
+        p.out_f32 = c->part_x; p.ldc = d;
+        int rc = gemm_skinny(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, SK_PARTIAL, 0, p, &pend, st, pdl);
+        if (rc) return rc;
+      } else if (tc) {
+        GemmTcParams p = {};
+        p.out_f32 = c->x; p.ldc = d;
+        int rc = gemm_tc(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, EPI_RESID, 0, p, st, pdl);
+        if (rc) return rc;
+      } else {
+        gemm_plain<TE, TE>(c->tmp, (const TE*)c->act, (const TE*)w.wd, T, d, F, st, pdl);
+        launch_k(add_residual_kernel, dim3((unsigned)(((long long)T * d + 255) / 256)), dim3(256), 0, st, pdl, c->x, (const float*)c->tmp, (long long)T * d);
+      }
     }
+    flush_partials();
     dump_stage(c, l, DLM_T_X_OUT, c->x, (size_t)d * 4, T);
   }
   // ---- head: a10 final norm on the block rows, a11 LM head statistics, a12+a13 combine + unmask ----
@@ -782,32 +893,45 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   if (R > 0) {
     {
       KScope ks(c, DLM_K_RMSNORM);
-      build_row_src_kernel<<<bd.n, 64, 0, st>>>(c->row_src, bd);
-      DLM_LAUNCH_CHECK();
-      rmsnorm_kernel<TE><<<R, 256, 0, st>>>((TE*)c->hf, c->x, c->row_src, d, a.rms_eps);
-      DLM_LAUNCH_CHECK();
+      launch_k(build_row_src_kernel, dim3(bd.n), dim3(64), 0, st, pdl, c->row_src, bd);
+      launch_k(rmsnorm_kernel<TE>, dim3(R), dim3(256), 0, st, pdl, (TE*)c->hf, c->x, (const int*)c->row_src, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      pend = 0;
     }
     dump_stage(c, 0, DLM_T_FINAL_NORM, c->hf, (size_t)d * sizeof(TE), R);
+    KScope ks(c, DLM_K_LMHEAD);
     if (tc) {
-      KScope ks(c, DLM_K_LMHEAD);
       n_tiles = c->n_tiles;
       GemmTcParams p = {};
       p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale;
-      int rc = gemm_tc(c->tmaps, err, c->hf, std::max(c->Rmax, 128), c->Wlm, V, R, V, d, EPI_LMHEAD, 128, p, st);
+      int rc = gemm_tc(c->tmaps, err, c->hf, std::max(c->Rmax, 128), c->Wlm, V, R, V, d, EPI_LMHEAD, 128, p, st, pdl);
       if (rc) return rc;
     } else {
-      KScope ks(c, DLM_K_LMHEAD);
-      gemm_plain<TE, TE>(c->logits, (const TE*)c->hf, (const TE*)c->Wlm, R, V, d, st);
-      row_stats_plain_kernel<<<R, 256, 0, st>>>(c->part, c->logits, V, a.mask_id, a.logit_scale);
-      DLM_LAUNCH_CHECK();
+      gemm_plain<TE, TE>(c->logits, (const TE*)c->hf, (const TE*)c->Wlm, R, V, d, st, pdl);
+      launch_k(row_stats_plain_kernel, dim3(R), dim3(256), 0, st, pdl, c->part, (const float*)c->logits, V, a.mask_id, a.logit_scale);
     }
   }
   {
     KScope ks(c, DLM_K_COMBINE_UNMASK);
-    combine_unmask_kernel<<<bd.n, 128, 0, st>>>(so, c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd, dry_run ? 1 : 0);
-    DLM_LAUNCH_CHECK();
+    launch_k(combine_unmask_kernel, dim3(bd.n), dim3(128), 0, st, pdl, so, (const RowPartial*)c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd,
+             dry_run ? 1 : 0);
   }
   CU_TRY(err, cudaGetLastError());
+  return DLM_OK;
+}
+
+// One step's device work = [descriptor H2D] [kernels between ev0 and ev1] [result D2H].  With DLM_OPT_CUDA_GRAPH the
+// whole sequence of a batch shape seen before is replayed from a captured graph (one launch per step).
+static int enqueue_step(dlm_ctx* c, const HostBatch& hb, bool dry, size_t desc_ints, bool capturing) {
+  std::string* err = &c->err;
+  CU_TRY(err, cudaMemcpyAsync(c->desc_dev, c->desc_host, desc_ints * 4, cudaMemcpyHostToDevice, c->st));
+  BatchDesc bd = make_desc(c, hb);
+  if (capturing) CU_TRY(err, cudaEventRecordWithFlags(c->ev0, c->st, cudaEventRecordExternal));
+  else CU_TRY(err, cudaEventRecord(c->ev0, c->st));        // device time of the step: first kernel .. last kernel
+  int rc = c->bf16_model ? forward<bf16>(c, bd, dry) : forward<float>(c, bd, dry);
+  if (rc) return rc;
+  if (capturing) CU_TRY(err, cudaEventRecordWithFlags(c->ev1, c->st, cudaEventRecordExternal));
+  else CU_TRY(err, cudaEventRecord(c->ev1, c->st));
+  CU_TRY(err, cudaMemcpyAsync(c->out_host, c->out_dev, c->out_bytes, cudaMemcpyDeviceToHost, c->st));
   return DLM_OK;
 }
 
@@ -821,12 +945,42 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   const bool dry = (b->flags & DLM_DRY_RUN) != 0;
   if (res->capacity < hb.R) { set_err(&c->err, "step: result capacity %d < %d block rows", res->capacity, hb.R); return DLM_E_CAPACITY; }
   std::string* err = &c->err;
-  BatchDesc bd = upload_batch(c, hb);
-  CU_TRY(err, cudaEventRecord(c->ev0, c->st));        // device time of the step: first kernel .. last kernel
-  rc = c->bf16_model ? forward<bf16>(c, bd, dry) : forward<float>(c, bd, dry);
-  if (rc) { cudaStreamSynchronize(c->st); c->kprof.cls.clear(); c->kprof.used = 0; return rc; }
-  CU_TRY(err, cudaEventRecord(c->ev1, c->st));
-  CU_TRY(err, cudaMemcpyAsync(c->out_host, c->out_dev, c->out_bytes, cudaMemcpyDeviceToHost, c->st));
+  const size_t desc_ints = fill_desc_host(c, hb);
+  const bool use_graph = c->opt_graph && !c->kprof.on && !c->opt_dump;
+  bool launched = false;
+  if (use_graph) {
+    GraphKey key = std::make_tuple(refresh ? 1 : 0, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask());
+    GraphEntry& g = c->graphs[key];
+    if (g.seen == 1) {                         // second sighting of this batch shape: capture it
+      const long long l0 = g_launches;
+      cudaGraph_t graph = nullptr;
+      if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        rc = enqueue_step(c, hb, dry, desc_ints, true);
+        cudaError_t e = cudaStreamEndCapture(c->st, &graph);
+        if (rc == DLM_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) == cudaSuccess) {
+          g.launches = g_launches - l0;
+          g.seen = 2;
+        } else {
+          g.seen = 3;                            // capture not possible for this shape: stay on eager launches
+          cudaGetLastError();
+        }
+        if (graph) cudaGraphDestroy(graph);
+        g_launches = l0;
+        if (rc) return rc;
+      } else { g.seen = 3; cudaGetLastError(); }
+    }
+    if (g.seen == 2) {
+      CU_TRY(err, cudaGraphLaunch(g.exec, c->st));
+      g_launches += g.launches;
+      launched = true;
+    } else if (g.seen == 0) {
+      g.seen = 1;
+    }
+  }
+  if (!launched) {
+    rc = enqueue_step(c, hb, dry, desc_ints, false);
+    if (rc) { cudaStreamSynchronize(c->st); c->kprof.cls.clear(); c->kprof.used = 0; return rc; }
+  }
   CU_TRY(err, cudaStreamSynchronize(c->st));
   cudaEventElapsedTime(&c->last_usec, c->ev0, c->ev1);
   c->last_usec *= 1000.f;
@@ -1011,6 +1165,36 @@ extern "C" int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t
   if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
   g_op_tmaps.m.clear();   // caller buffers come and go; never reuse a stale map
   return gemm_tc(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, (cudaStream_t)stream);
+}
+
+extern "C" int dlm_op_gemm_skinny_bf16(const void* X, const void* W, void* out, int32_t T, int32_t N, int32_t K, int32_t epi, int32_t splits, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!X || !W || !out || T <= 0 || T > kSkMaxTokens || N <= 0 || K <= 0 || (epi != EPI_F32 && epi != EPI_SWIGLU)) {
+    set_err(&g_init_error, "dlm_op_gemm_skinny_bf16: bad arguments (T must be in [1, %d])", kSkMaxTokens); return DLM_E_ARG;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  g_op_tmaps.m.clear();
+  SkinnyParams p = {};
+  p.ldc = N; p.up_row0 = N;
+  if (epi == EPI_SWIGLU) {
+    p.out_bf16 = (bf16*)out;
+    return gemm_skinny(g_op_tmaps, &g_init_error, X, T, W, 2LL * N, T, N, K, SK_SWIGLU, 0, p, nullptr, st, false);
+  }
+  float* part = nullptr;
+  const long long n = (long long)T * N;
+  if (cudaMalloc(&part, (size_t)kSkMaxSplits * n * 4) != cudaSuccess) { set_err(&g_init_error, "dlm_op_gemm_skinny_bf16: allocation failed"); return DLM_E_CAPACITY; }
+  p.out_f32 = part;
+  int ns = 0;
+  rc = gemm_skinny(g_op_tmaps, &g_init_error, X, T, W, N, T, N, K, SK_PARTIAL, splits, p, &ns, st, false);
+  if (!rc) {
+    cudaMemsetAsync(out, 0, (size_t)n * 4, st);
+    launch_k(add_partials_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, st, false, (float*)out, (const float*)part, ns, n, n);
+  }
+  cudaError_t e = cudaStreamSynchronize(st);
+  cudaFree(part);
+  if (!rc && e != cudaSuccess) { set_err(&g_init_error, "dlm_op_gemm_skinny_bf16: %s", cudaGetErrorString(e)); rc = DLM_E_CUDA; }
+  return rc < 0 ? rc : ns;
 }
 
 extern "C" int dlm_op_gemm_plain_bf16(const void* A, const void* W, float* out, int32_t M, int32_t N, int32_t K, void* stream) {

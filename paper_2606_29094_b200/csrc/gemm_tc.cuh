@@ -64,6 +64,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   uint32_t tmem_cols = 32;
   while ((int)tmem_cols < BN) tmem_cols <<= 1;
 
+  ptx::pdl_launch_dependents();
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&mapA);
     ptx::prefetch_tmap(&mapB);
@@ -86,11 +87,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       // ---------------- TMA producer ----------------
       const uint32_t a_bytes = (uint32_t)p.a_box_rows * 128u;
       const uint32_t tx = a_bytes + (uint32_t)BN * 128u;
-      for (int kb = 0; kb < num_kb; ++kb) {
-        const int s = kb % stages;
-        const uint32_t ph = (uint32_t)(kb / stages) & 1u;
-        ptx::mbar_wait(empty_bar(s), ph ^ 1u);
-        const uint32_t sa = base + s * stage_bytes, sb = sa + kATileBytes;
+      auto load_w = [&](int kb, int s) {
+        const uint32_t sb = base + s * stage_bytes + kATileBytes;
         ptx::mbar_expect_tx(full_bar(s), tx);
         if (EPI == EPI_SWIGLU) {
           const int f0 = tile_n * (BN / 2);
@@ -99,7 +97,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
         } else {
           ptx::tma_load_2d(sb, &mapB, kb * kBK, tile_n * BN, full_bar(s), p.w_policy);
         }
-        ptx::tma_load_2d(sa, &mapA, kb * kBK, m0, full_bar(s), DLM_L2_EVICT_LAST);
+      };
+      auto load_a = [&](int kb, int s) { ptx::tma_load_2d(base + s * stage_bytes, &mapA, kb * kBK, m0, full_bar(s), DLM_L2_EVICT_LAST); };
+      // weights do not depend on the upstream kernel: fill the ring with them before the PDL wait
+      const int pre = min(stages, num_kb);
+      for (int kb = 0; kb < pre; ++kb) load_w(kb, kb);
+      ptx::pdl_wait();
+      for (int kb = 0; kb < pre; ++kb) load_a(kb, kb);
+      for (int kb = pre; kb < num_kb; ++kb) {
+        const int s = kb % stages;
+        const uint32_t ph = (uint32_t)(kb / stages) & 1u;
+        ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+        load_w(kb, s);
+        load_a(kb, s);
       }
     }
   } else if (warp == 1) {

@@ -46,6 +46,8 @@ __global__ void init_rope_kernel(float* __restrict__ cs, float* __restrict__ sn,
 template <typename TW>
 __global__ void embed_kernel(float* __restrict__ x, const TW* __restrict__ E, const int* __restrict__ tokens,
                              int max_seq, BatchDesc b, int d) {
+  pdl_launch_dependents();
+  pdl_wait();
   int t = blockIdx.x;
   int bi = b.tok_bi[t];
   int pos = b.q_pos0[bi] + (t - b.q_off[bi]);
@@ -71,18 +73,44 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
   return red[0];
 }
 
+// Split-K partials of the previous O / down projection (gemm_skinny) are folded in here, in a fixed order:
+//   x[row] += part[0][row] + part[1][row] + ... ; then u = RMSNorm(x[row]).
 template <typename TA>
-__global__ void rmsnorm_kernel(TA* __restrict__ u, const float* __restrict__ x, const int* __restrict__ row_src,
-                               int d, float eps) {
+__global__ void rmsnorm_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
+                               int d, float eps, const float* __restrict__ part, int n_part, long long part_stride) {
   __shared__ float red[33];
+  pdl_launch_dependents();
+  pdl_wait();
   int r = blockIdx.x;
-  const float* xr = x + (long long)(row_src ? row_src[r] : r) * d;
+  const long long sr = row_src ? row_src[r] : r;
+  float* xr = x + sr * d;
   float ss = 0.f;
-  for (int i = threadIdx.x; i < d; i += blockDim.x) { float v = xr[i]; ss += v * v; }
+  if (n_part > 0) {
+    const float* pr = part + sr * d;
+    for (int i = threadIdx.x; i < d; i += blockDim.x) {
+      float v = xr[i];
+      for (int s = 0; s < n_part; ++s) v += pr[s * part_stride + i];
+      xr[i] = v;                     // the same thread re-reads it below
+      ss += v * v;
+    }
+  } else {
+    for (int i = threadIdx.x; i < d; i += blockDim.x) { float v = xr[i]; ss += v * v; }
+  }
   ss = block_sum(ss, red);
   float rs = rsqrtf(ss / (float)d + eps);
   TA* ur = u + (long long)r * d;
   for (int i = threadIdx.x; i < d; i += blockDim.x) ur[i] = from_f32<TA>(xr[i] * rs);
+}
+
+// x[row] += sum of split-K partials (debug-dump mode only: makes x complete right after the projection)
+__global__ void add_partials_kernel(float* __restrict__ x, const float* __restrict__ part, int n_part, long long part_stride, long long n) {
+  pdl_launch_dependents();
+  pdl_wait();
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float v = x[i];
+  for (int s = 0; s < n_part; ++s) v += part[s * part_stride + i];
+  x[i] = v;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -93,7 +121,9 @@ template <typename TA>
 __global__ void rope_kv_write_kernel(TA* __restrict__ q, TA* __restrict__ kv_store, const float* __restrict__ qkv,
                                      const float* __restrict__ rope_cos, const float* __restrict__ rope_sin,
                                      const int* __restrict__ page_table, BatchDesc b, KvGeom g, int layer,
-                                     int n_heads) {
+                                     int n_heads, int n_part, long long part_stride) {
+  pdl_launch_dependents();
+  pdl_wait();
   int t = blockIdx.x;
   int bi = b.tok_bi[t];
   int pos = b.q_pos0[bi] + (t - b.q_off[bi]);
@@ -108,6 +138,7 @@ __global__ void rope_kv_write_kernel(TA* __restrict__ q, TA* __restrict__ kv_sto
   for (int p = threadIdx.x; p < (n_heads + g.n_kv_heads) * half; p += blockDim.x) {
     int h = p / half, i = p % half;
     float a = row[h * dh + i], c = row[h * dh + i + half];
+    for (int s = 1; s < n_part; ++s) { a += row[s * part_stride + h * dh + i]; c += row[s * part_stride + h * dh + i + half]; }
     float ra = a * cs[i] - c * sn[i];
     float rc = c * cs[i] + a * sn[i];
     if (h < n_heads) {
@@ -122,7 +153,9 @@ __global__ void rope_kv_write_kernel(TA* __restrict__ q, TA* __restrict__ kv_sto
   }
   for (int p = threadIdx.x; p < nkv; p += blockDim.x) {
     int h = p / dh, e = p % dh;
-    kv_store[g.offset(layer, page, 1, h, off) + e] = from_f32<TA>(row[nq + nkv + p]);
+    float v = row[nq + nkv + p];
+    for (int s = 1; s < n_part; ++s) v += row[s * part_stride + nq + nkv + p];
+    kv_store[g.offset(layer, page, 1, h, off) + e] = from_f32<TA>(v);
   }
 }
 
@@ -138,6 +171,8 @@ __global__ void attention_plain_kernel(TA* __restrict__ out, const TA* __restric
   extern __shared__ float sc[];
   __shared__ float red[33];
   __shared__ float qs[256];
+  pdl_launch_dependents();
+  pdl_wait();
   int t = blockIdx.x, h = blockIdx.y;
   int bi = b.tok_bi[t];
   int S = b.kv_len[bi];
@@ -189,6 +224,8 @@ __global__ void __launch_bounds__(256) gemm_plain_kernel(float* __restrict__ C, 
                                                          int ldw, int ldc) {
   __shared__ float As[16][65];
   __shared__ float Ws[16][65];
+  pdl_launch_dependents();
+  pdl_wait();
   int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
   int m0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
   float acc[4][4] = {};
@@ -220,6 +257,8 @@ __global__ void __launch_bounds__(256) gemm_plain_kernel(float* __restrict__ C, 
 
 // x += y   (fp32 residual stream)
 __global__ void add_residual_kernel(float* __restrict__ x, const float* __restrict__ y, long long n) {
+  pdl_launch_dependents();
+  pdl_wait();
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) x[i] += y[i];
 }
@@ -229,6 +268,8 @@ __device__ __forceinline__ float silu_f(float g) { return g / (1.f + __expf(-g))
 // act[t, f] = silu(gu[t, f]) * gu[t, F + f]
 template <typename TA>
 __global__ void swiglu_kernel(TA* __restrict__ act, const float* __restrict__ gu, int T, int F) {
+  pdl_launch_dependents();
+  pdl_wait();
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (long long)T * F) return;
   int t = (int)(i / F), f = (int)(i % F);
@@ -238,6 +279,8 @@ __global__ void swiglu_kernel(TA* __restrict__ act, const float* __restrict__ gu
 
 // row_src[r] for a10: index into [T, d] of each block row
 __global__ void build_row_src_kernel(int* __restrict__ row_src, BatchDesc b) {
+  pdl_launch_dependents();
+  pdl_wait();
   int bi = blockIdx.x;
   int base = b.q_off[bi] + (b.blk_lo[bi] - b.q_pos0[bi]);
   for (int j = threadIdx.x; j < b.blk_len[bi]; j += blockDim.x) row_src[b.row_off[bi] + j] = base + j;
@@ -262,6 +305,8 @@ __global__ void row_stats_plain_kernel(RowPartial* __restrict__ part, const floa
                                        int mask_id, float scale) {
   __shared__ float sm[32], ss[32];
   __shared__ int si[32];
+  pdl_launch_dependents();
+  pdl_wait();
   int r = blockIdx.x;
   const float* z = logits + (long long)r * V;
   float m = -CUDART_INF_F, s = 0.f;
@@ -305,6 +350,8 @@ __global__ void __launch_bounds__(128) combine_unmask_kernel(StepOut o, const Ro
                                                              int max_block, int mask_id, BatchDesc b, int dry_run) {
   __shared__ float s_conf[64];
   __shared__ int s_tok[64];
+  pdl_launch_dependents();
+  pdl_wait();
   int bi = blockIdx.x;
   int B = b.blk_len[bi];
   int w = threadIdx.x >> 5, l = threadIdx.x & 31;

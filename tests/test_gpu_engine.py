@@ -196,6 +196,38 @@ def test_c2_reduced_depth_teacher_forced(simple, flash):
     print("P-B C2/L2", dict(simple=simple, flash=flash), s)
 
 
+def test_launch_modes_agree_bitwise():
+    """The production launch mode (CUDA graph replay + programmatic dependent launch + weight-streaming split-K GEMMs,
+    partial sums folded into the next RMSNorm) computes bit-for-bit what the eager, serialised, dump-friendly
+    launches compute: same kernels, same summation order."""
+    pkg = _pkg()
+    arch = _reduced(ARCH_LLADA8B, 2)
+    rng = np.random.default_rng(31)
+    prompts = [random_tokens(rng, P, arch.vocab, arch.mask_id) for P in (96, 40)]
+    outs = {}
+    for mode in ("production", "eager", "dump", "no_skinny"):
+        eng = pkg.Engine(arch, WEIGHT_SEED["C2"], max_requests=2, max_seq=160, max_block=32)
+        if mode == "eager":
+            eng.set_option(pkg.OPT_CUDA_GRAPH, 0)
+            eng.set_option(pkg.OPT_PDL, 0)
+        if mode == "dump":
+            eng.set_option(pkg.OPT_DEBUG_DUMP, 1)
+        if mode == "no_skinny":
+            eng.set_option(pkg.OPT_SKINNY_GEMM, 0)
+        ids = [eng.add_request(p, 64, 32, 0.9) for p in prompts]
+        res = []
+        for it in range(5):           # refresh, then cached steps: the 3rd+ cached step of a shape replays the graph
+            g = eng.refresh_step(ids, dry_run=True) if it == 0 else eng.cached_step(ids, dry_run=(it < 4))
+            res.append((g.lse.copy(), g.row_conf.copy(), g.row_tok.copy(), [list(c) for c in g.commits]))
+        outs[mode] = res
+        eng.close()
+    for mode in ("eager", "dump"):
+        for a, b in zip(outs["production"], outs[mode]):
+            assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2]) and a[3] == b[3], mode
+    for a, b in zip(outs["production"], outs["no_skinny"]):     # different K summation order: close, not identical
+        assert np.allclose(a[0], b[0], rtol=0, atol=5e-2) and np.allclose(a[1], b[1], rtol=0, atol=2e-2)
+
+
 def test_c5_reduced_depth_gqa_teacher_forced():
     """P-B on the Qwen2.5-7B shape (GQA 28/4, FFN 18944, vocab 152064) at depth 2."""
     arch = _reduced(ARCH_QWEN7B, 2)

@@ -65,6 +65,39 @@ def test_gemm_tc_swiglu(M, F, K, bn):
     assert np.all(np.abs(_f64(got) - want) <= np.abs(want) * 2 ** -8 + 1e-4)
 
 
+SKINNY_SHAPES = [  # (T, N, K): tails in every dimension, one and several K blocks per split
+    (32, 256, 128), (1, 128, 64), (32, 4096, 4096), (17, 384, 688), (64, 200, 512), (100, 1056, 200), (128, 768, 256), (33, 96, 4096)]
+
+
+@pytest.mark.parametrize("T,N,K", SKINNY_SHAPES)
+@pytest.mark.parametrize("splits", [0, 1, 3, 16])
+def test_gemm_skinny_partial(T, N, K, splits):
+    """Weight-streaming swap-AB split-K GEMM (cached step a3/a6/a9) vs fp64 matmul."""
+    import paper_2606_29094_b200 as pkg
+    rng = np.random.default_rng(T * 5 + N + K + splits)
+    X, x = _mk(rng, T, K)
+    W, w = _mk(rng, N, K, 0.05)
+    want = x @ w.T
+    tol = 2e-5 * np.sqrt(K) * np.abs(x).max() * np.abs(w).max() + 1e-6
+    got, ns = pkg.op_gemm_skinny_bf16(X, W, pkg.EPI_F32, splits)
+    torch.cuda.synchronize()
+    assert 1 <= ns <= 16 and (splits in (0,) or ns <= splits)
+    assert np.abs(_f64(got) - want).max() <= tol
+
+
+@pytest.mark.parametrize("T,F,K", [(32, 128, 128), (70, 688, 256), (128, 352, 512), (5, 64, 64), (32, 12288, 4096)])
+def test_gemm_skinny_swiglu(T, F, K):
+    import paper_2606_29094_b200 as pkg
+    rng = np.random.default_rng(T + F + K)
+    X, x = _mk(rng, T, K)
+    W, w = _mk(rng, 2 * F, K, 0.1 if K < 1024 else 0.02)
+    want = omodel.silu(x @ w[:F].T) * (x @ w[F:].T)
+    got, _ = pkg.op_gemm_skinny_bf16(X, W, pkg.EPI_SWIGLU)
+    torch.cuda.synchronize()
+    assert got.shape == (T, F)
+    assert np.all(np.abs(_f64(got) - want) <= np.abs(want) * 2 ** -8 + 2e-4)
+
+
 def test_gemm_plain_matches():
     import paper_2606_29094_b200 as pkg
     rng = np.random.default_rng(3)
