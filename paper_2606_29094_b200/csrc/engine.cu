@@ -400,6 +400,8 @@ struct KScope {
   ~KScope() { if (c->kprof.on) c->kprof.end(c->st); }
 };
 
+static int norm_threads(int d) { return std::min(1024, ((d / 4) + 31) / 32 * 32); }
+
 static int nqkv(const dlm_arch& a) { return (a.n_heads + 2 * a.n_kv_heads) * a.head_dim; }
 
 // ------------------------------------------------------------------------------------------------
@@ -423,6 +425,7 @@ static int validate_arch(const dlm_arch* a, std::string* err) {
   REQ(a->n_layers > 0 && a->d_model > 0 && a->n_heads > 0 && a->n_kv_heads > 0 && a->head_dim > 0 && a->d_ffn > 0);
   REQ(a->vocab > 1 && a->mask_id >= 0 && a->mask_id < a->vocab);
   REQ(a->n_heads % a->n_kv_heads == 0 && a->head_dim % 2 == 0 && a->head_dim <= 256);
+  REQ(a->d_model % 4 == 0 && a->d_model <= 16384);
   REQ(a->weight_dtype == DLM_DTYPE_F32 || a->weight_dtype == DLM_DTYPE_BF16);
   REQ(a->max_requests > 0 && a->max_seq > 0 && a->max_block > 0 && a->max_block <= 64);
   REQ(a->kv_page_tokens > 0 && a->max_batch_tokens > 0);
@@ -778,7 +781,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     dump_stage(c, l, DLM_T_X_IN, c->x, (size_t)d * 4, T);
     {
       KScope ks(c, DLM_K_RMSNORM);
-      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(256), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(norm_threads(d)), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
       pend = 0;
     }
     dump_stage(c, l, DLM_T_NORM1, c->u, (size_t)d * sizeof(TE), T);
@@ -801,7 +804,8 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     }
     {
       KScope ks(c, DLM_K_ROPE_KV);
-      launch_k(rope_kv_write_kernel<TE>, dim3(T), dim3(256), 0, st, pdl, (TE*)c->q, (TE*)c->kv_store, (const float*)c->qkv, (const float*)c->rope_cos,
+      const int hpb = std::max(1, 256 / (a.head_dim / 2));       // heads per block
+      launch_k(rope_kv_write_kernel<TE>, dim3(T, (a.n_heads + 2 * a.n_kv_heads + hpb - 1) / hpb), dim3(hpb * (a.head_dim / 2)), 0, st, pdl, (TE*)c->q, (TE*)c->kv_store, (const float*)c->qkv, (const float*)c->rope_cos,
                (const float*)c->rope_sin, (const int*)c->page_table, bd, c->kg, l, a.n_heads, nq, (long long)T * NQKV);
     }
     dump_stage(c, l, DLM_T_Q, c->q, (size_t)HQ * sizeof(TE), T);
@@ -839,7 +843,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     dump_stage(c, l, DLM_T_X_MID, c->x, (size_t)d * 4, T);
     {
       KScope ks(c, DLM_K_RMSNORM);
-      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(256), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(norm_threads(d)), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
       pend = 0;
     }
     dump_stage(c, l, DLM_T_NORM2, c->u, (size_t)d * sizeof(TE), T);
@@ -894,7 +898,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     {
       KScope ks(c, DLM_K_RMSNORM);
       launch_k(build_row_src_kernel, dim3(bd.n), dim3(64), 0, st, pdl, c->row_src, bd);
-      launch_k(rmsnorm_kernel<TE>, dim3(R), dim3(256), 0, st, pdl, (TE*)c->hf, c->x, (const int*)c->row_src, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      launch_k(rmsnorm_kernel<TE>, dim3(R), dim3(norm_threads(d)), 0, st, pdl, (TE*)c->hf, c->x, (const int*)c->row_src, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
       pend = 0;
     }
     dump_stage(c, 0, DLM_T_FINAL_NORM, c->hf, (size_t)d * sizeof(TE), R);
@@ -912,7 +916,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   }
   {
     KScope ks(c, DLM_K_COMBINE_UNMASK);
-    launch_k(combine_unmask_kernel, dim3(bd.n), dim3(128), 0, st, pdl, so, (const RowPartial*)c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd,
+    launch_k(combine_unmask_kernel, dim3(bd.n), dim3(1024), 0, st, pdl, so, (const RowPartial*)c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd,
              dry_run ? 1 : 0);
   }
   CU_TRY(err, cudaGetLastError());
@@ -1228,7 +1232,7 @@ static int op_head(const void* hidden, const void* Wlm, int n, int B, int V, int
   if (rc) return rc;
   BatchDesc bd = {};
   bd.n = n; bd.R = R; bd.slot = meta; bd.blk_lo = meta + n; bd.blk_len = meta + 2 * n; bd.row_off = meta + 3 * n; bd.tau = tau;
-  combine_unmask_kernel<<<n, 128, 0, st>>>(so, part, n_tiles, tokens_io, B, B, mask_id, bd, dry);
+  combine_unmask_kernel<<<n, 1024, 0, st>>>(so, part, n_tiles, tokens_io, B, B, mask_id, bd, dry);
   DLM_LAUNCH_CHECK();
   return cudaGetLastError() == cudaSuccess ? DLM_OK : DLM_E_CUDA;
 }

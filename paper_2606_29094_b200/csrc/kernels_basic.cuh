@@ -54,7 +54,17 @@ __global__ void embed_kernel(float* __restrict__ x, const TW* __restrict__ E, co
   int tok = tokens[(long long)b.slot[bi] * max_seq + pos];
   const TW* e = E + (long long)tok * d;
   float* xr = x + (long long)t * d;
-  for (int i = threadIdx.x; i < d; i += blockDim.x) xr[i] = to_f32(e[i]);
+  if (sizeof(TW) == 2 && d % 8 == 0) {           // 16-byte loads of 8 bf16
+    for (int i = threadIdx.x * 8; i < d; i += blockDim.x * 8) {
+      uint4 raw = *reinterpret_cast<const uint4*>(reinterpret_cast<const bf16*>(e) + i);
+      const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&raw);
+      float2 a = __bfloat1622float2(h[0]), bq = __bfloat1622float2(h[1]), cq = __bfloat1622float2(h[2]), dq = __bfloat1622float2(h[3]);
+      *reinterpret_cast<float4*>(xr + i) = make_float4(a.x, a.y, bq.x, bq.y);
+      *reinterpret_cast<float4*>(xr + i + 4) = make_float4(cq.x, cq.y, dq.x, dq.y);
+    }
+  } else {
+    for (int i = threadIdx.x; i < d; i += blockDim.x) xr[i] = to_f32(e[i]);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -74,32 +84,61 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
 }
 
 // Split-K partials of the previous O / down projection (gemm_skinny) are folded in here, in a fixed order:
-//   x[row] += part[0][row] + part[1][row] + ... ; then u = RMSNorm(x[row]).
+//   x[row] = ((x[row] + part[0][row]) + part[1][row]) + ... ; then u = RMSNorm(x[row]).
+// One block per row, one float4 per thread per 4*blockDim chunk (d = 4096 -> 1024 threads, everything in flight at
+// once: the kernel sits on the critical path between two weight-streaming GEMMs and is pure latency).
+constexpr int kNormMaxChunks = 4;     // d <= 4 * 4 * 1024
+
 template <typename TA>
-__global__ void rmsnorm_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
-                               int d, float eps, const float* __restrict__ part, int n_part, long long part_stride) {
+__global__ void __launch_bounds__(1024) rmsnorm_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
+                                                      int d, float eps, const float* __restrict__ part, int n_part,
+                                                      long long part_stride) {
   __shared__ float red[33];
   pdl_launch_dependents();
   pdl_wait();
-  int r = blockIdx.x;
+  const int r = blockIdx.x;
   const long long sr = row_src ? row_src[r] : r;
-  float* xr = x + sr * d;
+  float4* xr = reinterpret_cast<float4*>(x + sr * d);
+  const int nvec = d >> 2;
+  float4 v[kNormMaxChunks];
   float ss = 0.f;
-  if (n_part > 0) {
-    const float* pr = part + sr * d;
-    for (int i = threadIdx.x; i < d; i += blockDim.x) {
-      float v = xr[i];
-      for (int s = 0; s < n_part; ++s) v += pr[s * part_stride + i];
-      xr[i] = v;                     // the same thread re-reads it below
-      ss += v * v;
+#pragma unroll
+  for (int k = 0; k < kNormMaxChunks; ++k) {
+    const int i = threadIdx.x + k * blockDim.x;
+    if (i < nvec) {
+      float4 a = xr[i];
+      if (n_part > 0) {
+        const float4* pr = reinterpret_cast<const float4*>(part + sr * d) + i;
+        const long long ps4 = part_stride >> 2;
+#pragma unroll 4
+        for (int s = 0; s < n_part; ++s) {
+          const float4 q = __ldcg(pr + s * ps4);
+          a.x += q.x; a.y += q.y; a.z += q.z; a.w += q.w;
+        }
+        xr[i] = a;
+      }
+      v[k] = a;
+      ss += a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w;
     }
-  } else {
-    for (int i = threadIdx.x; i < d; i += blockDim.x) { float v = xr[i]; ss += v * v; }
   }
   ss = block_sum(ss, red);
-  float rs = rsqrtf(ss / (float)d + eps);
+  const float rs = rsqrtf(ss / (float)d + eps);
   TA* ur = u + (long long)r * d;
-  for (int i = threadIdx.x; i < d; i += blockDim.x) ur[i] = from_f32<TA>(xr[i] * rs);
+#pragma unroll
+  for (int k = 0; k < kNormMaxChunks; ++k) {
+    const int i = threadIdx.x + k * blockDim.x;
+    if (i < nvec) {
+      const float4 a = v[k];
+      if (sizeof(TA) == 2) {
+        __nv_bfloat162 lo = __floats2bfloat162_rn(a.x * rs, a.y * rs), hi = __floats2bfloat162_rn(a.z * rs, a.w * rs);
+        uint2 w;
+        w.x = *reinterpret_cast<uint32_t*>(&lo); w.y = *reinterpret_cast<uint32_t*>(&hi);
+        *reinterpret_cast<uint2*>(reinterpret_cast<bf16*>(ur) + 4 * i) = w;
+      } else {
+        *reinterpret_cast<float4*>(reinterpret_cast<float*>(ur) + 4 * i) = make_float4(a.x * rs, a.y * rs, a.z * rs, a.w * rs);
+      }
+    }
+  }
 }
 
 // x[row] += sum of split-K partials (debug-dump mode only: makes x complete right after the projection)
@@ -117,46 +156,42 @@ __global__ void add_partials_kernel(float* __restrict__ x, const float* __restri
 // a4  RoPE + K/V write.  qkv fp32 [T, (H+2H_kv) d_h] -> q [T, H d_h] (TA), K (rotated) and V into the pages.
 // Half-split pairing (i, i + d_h/2), angle = pos * theta^(-2i/d_h) from the table.  One block per token.
 // ------------------------------------------------------------------------------------------------
+// Grid (token, group of 256/half heads); thread = (head, pair index i): every load of the kernel is in flight at once.
 template <typename TA>
-__global__ void rope_kv_write_kernel(TA* __restrict__ q, TA* __restrict__ kv_store, const float* __restrict__ qkv,
-                                     const float* __restrict__ rope_cos, const float* __restrict__ rope_sin,
-                                     const int* __restrict__ page_table, BatchDesc b, KvGeom g, int layer,
-                                     int n_heads, int n_part, long long part_stride) {
+__global__ void __launch_bounds__(256) rope_kv_write_kernel(TA* __restrict__ q, TA* __restrict__ kv_store, const float* __restrict__ qkv,
+                                                           const float* __restrict__ rope_cos, const float* __restrict__ rope_sin,
+                                                           const int* __restrict__ page_table, BatchDesc b, KvGeom g, int layer,
+                                                           int n_heads, int n_part, long long part_stride) {
   pdl_launch_dependents();
   pdl_wait();
-  int t = blockIdx.x;
-  int bi = b.tok_bi[t];
-  int pos = b.q_pos0[bi] + (t - b.q_off[bi]);
-  int dh = g.head_dim, half = dh >> 1;
-  int nq = n_heads * dh, nkv = g.n_kv_heads * dh;
-  const float* row = qkv + (long long)t * (nq + 2 * nkv);
-  const float* cs = rope_cos + (long long)pos * half;
-  const float* sn = rope_sin + (long long)pos * half;
-  int page = page_table[(long long)b.slot[bi] * g.max_pages_per_req + pos / g.page_tokens];
-  int off = pos % g.page_tokens;
-  // Q and K: one thread per (head, i) pair
-  for (int p = threadIdx.x; p < (n_heads + g.n_kv_heads) * half; p += blockDim.x) {
-    int h = p / half, i = p % half;
-    float a = row[h * dh + i], c = row[h * dh + i + half];
-    for (int s = 1; s < n_part; ++s) { a += row[s * part_stride + h * dh + i]; c += row[s * part_stride + h * dh + i + half]; }
-    float ra = a * cs[i] - c * sn[i];
-    float rc = c * cs[i] + a * sn[i];
-    if (h < n_heads) {
-      TA* qo = q + (long long)t * nq + h * dh;
-      qo[i] = from_f32<TA>(ra);
-      qo[i + half] = from_f32<TA>(rc);
-    } else {
-      TA* ko = kv_store + g.offset(layer, page, 0, h - n_heads, off);
-      ko[i] = from_f32<TA>(ra);
-      ko[i + half] = from_f32<TA>(rc);
-    }
+  const int t = blockIdx.x;
+  const int dh = g.head_dim, half = dh >> 1;
+  const int h = blockIdx.y * (blockDim.x / half) + threadIdx.x / half;       // 0..H-1 query, then K heads, then V heads
+  const int i = threadIdx.x % half;
+  if (h >= n_heads + 2 * g.n_kv_heads) return;
+  const int bi = b.tok_bi[t];
+  const int pos = b.q_pos0[bi] + (t - b.q_off[bi]);
+  const int nq = n_heads * dh, nkv = g.n_kv_heads * dh;
+  const float* row = qkv + (long long)t * (nq + 2 * nkv) + (long long)h * dh;
+  float a = row[i], c = row[i + half];
+#pragma unroll 4
+  for (int s = 1; s < n_part; ++s) { a += __ldcg(row + s * part_stride + i); c += __ldcg(row + s * part_stride + i + half); }
+  if (h < n_heads + g.n_kv_heads) {               // rotate Q and K
+    const float cs = rope_cos[(long long)pos * half + i], sn = rope_sin[(long long)pos * half + i];
+    const float ra = a * cs - c * sn, rc = c * cs + a * sn;
+    a = ra; c = rc;
   }
-  for (int p = threadIdx.x; p < nkv; p += blockDim.x) {
-    int h = p / dh, e = p % dh;
-    float v = row[nq + nkv + p];
-    for (int s = 1; s < n_part; ++s) v += row[s * part_stride + nq + nkv + p];
-    kv_store[g.offset(layer, page, 1, h, off) + e] = from_f32<TA>(v);
+  TA* dst;
+  if (h < n_heads) {
+    dst = q + (long long)t * nq + h * dh;
+  } else {
+    const int page = page_table[(long long)b.slot[bi] * g.max_pages_per_req + pos / g.page_tokens];
+    const int kvh = h - n_heads;
+    dst = kv_store + (kvh < g.n_kv_heads ? g.offset(layer, page, 0, kvh, pos % g.page_tokens)
+                                         : g.offset(layer, page, 1, kvh - g.n_kv_heads, pos % g.page_tokens));
   }
+  dst[i] = from_f32<TA>(a);
+  dst[i + half] = from_f32<TA>(c);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -345,7 +380,7 @@ struct StepOut {              // device-side result arrays, fixed stride max_blo
   int* row_tok;               // [n, max_block]
 };
 
-__global__ void __launch_bounds__(128) combine_unmask_kernel(StepOut o, const RowPartial* __restrict__ part,
+__global__ void __launch_bounds__(1024) combine_unmask_kernel(StepOut o, const RowPartial* __restrict__ part,
                                                              int n_tiles, int* __restrict__ tokens, int max_seq,
                                                              int max_block, int mask_id, BatchDesc b, int dry_run) {
   __shared__ float s_conf[64];
@@ -355,11 +390,23 @@ __global__ void __launch_bounds__(128) combine_unmask_kernel(StepOut o, const Ro
   int bi = blockIdx.x;
   int B = b.blk_len[bi];
   int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  for (int j = w; j < B; j += 4) {
-    const RowPartial* p = part + (long long)(b.row_off[bi] + j) * n_tiles;
+  const int n_warps = blockDim.x >> 5;
+  for (int j = w; j < B; j += n_warps) {
+    const int4* p = reinterpret_cast<const int4*>(part + (long long)(b.row_off[bi] + j) * n_tiles);
     float m = -CUDART_INF_F, s = 0.f;
     int idx = 0x7fffffff;
-    for (int t = l; t < n_tiles; t += 32) partial_merge(m, s, idx, p[t].m, p[t].s, p[t].idx);
+    int t = l;
+    for (; t + 96 < n_tiles; t += 128) {          // four 16-byte loads in flight per lane
+      const int4 q0 = __ldcg(p + t), q1 = __ldcg(p + t + 32), q2 = __ldcg(p + t + 64), q3 = __ldcg(p + t + 96);
+      partial_merge(m, s, idx, __int_as_float(q0.x), __int_as_float(q0.y), q0.z);
+      partial_merge(m, s, idx, __int_as_float(q1.x), __int_as_float(q1.y), q1.z);
+      partial_merge(m, s, idx, __int_as_float(q2.x), __int_as_float(q2.y), q2.z);
+      partial_merge(m, s, idx, __int_as_float(q3.x), __int_as_float(q3.y), q3.z);
+    }
+    for (; t < n_tiles; t += 32) {
+      const int4 q0 = __ldcg(p + t);
+      partial_merge(m, s, idx, __int_as_float(q0.x), __int_as_float(q0.y), q0.z);
+    }
     for (int off = 16; off > 0; off >>= 1) {
       float m2 = __shfl_xor_sync(0xffffffffu, m, off), s2 = __shfl_xor_sync(0xffffffffu, s, off);
       int i2 = __shfl_xor_sync(0xffffffffu, idx, off);
