@@ -27,6 +27,13 @@ extern "C" {
 DLM_API int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epilogue,
                      int32_t bn, void* stream);
 
+/* Same contraction and epilogues on the persistent CTA-pair kernel the engine uses for M > 128 tokens (refresh
+ * steps, large cached batches): clusters of two CTAs, tcgen05.mma.cta_group::2 on 256 x bn tiles, accumulator
+ * double-buffered in tensor memory.  bn = 0 picks the tile width; otherwise a multiple of 32 in [64, 256]
+ * (multiple of 64 for SwiGLU). */
+DLM_API int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epilogue,
+                          int32_t bn, void* stream);
+
 /* Weight-streaming split-K tcgen05 GEMM for T <= 128 tokens (the cached step's a3/a6/a8/a9): swap-AB (weights on
  * the MMA's M side, tokens on N), every K split writes an fp32 slice and the slices are summed in a fixed order.
  * epilogue DLM_EPI_F32: out fp32 [T, N] = X . W^T; DLM_EPI_SWIGLU: out bf16 [T, N], W = [2N, K] (gate rows, up rows).

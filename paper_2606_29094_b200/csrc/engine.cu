@@ -19,6 +19,7 @@
 #include "attn_flash.cuh"
 #include "common.cuh"
 #include "gemm_skinny.cuh"
+#include "gemm_pair.cuh"
 #include "gemm_tc.cuh"
 #include "kernels_basic.cuh"
 
@@ -166,6 +167,87 @@ static int gemm_tc(TmapCache& tc, std::string* err, const void* A, long long a_r
     default: set_err(err, "gemm_tc: bad epilogue %d", epi); return DLM_E_ARG;
   }
   if (e != cudaSuccess) { set_err(err, "gemm_tc launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+  return DLM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// CTA-pair persistent tcgen05 GEMM launcher (M > 128)
+// ------------------------------------------------------------------------------------------------
+// Tile width.  Measured on B200: with both operands in shared memory one 256 x bn x 16 UMMA takes ~128 cycles for
+// every bn <= 256 (the A-operand read paces it), so a tile costs the same whatever its width: take the widest tile
+// among those with the fewest waves over one pair per TPC.
+static int pick_bn_pair(int M, int N, int epi) {
+  if (epi == EPI_LMHEAD) return 256;
+  const int m_tiles = (M + 255) / 256;
+  const int pairs = std::max(1, g_num_sms / 2);
+  static const int cand_std[] = {256, 224, 192, 160, 128, 96, 64};
+  static const int cand_glu[] = {256, 192, 128, 64};
+  const int* cand = epi == EPI_SWIGLU ? cand_glu : cand_std;
+  const int nc = epi == EPI_SWIGLU ? 4 : 7;
+  long long best_waves = -1;
+  int best = cand[0];
+  for (int i = 0; i < nc; ++i) {
+    const int per = epi == EPI_SWIGLU ? cand[i] / 2 : cand[i];
+    const long long tiles = (long long)m_tiles * ((N + per - 1) / per);
+    const long long waves = (tiles + pairs - 1) / pairs;
+    if (best_waves < 0 || waves < best_waves) { best_waves = waves; best = cand[i]; }
+  }
+  return best;
+}
+
+template <int EPI>
+static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* mb, const GemmPairParams& p, cudaStream_t st, bool pdl) {
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_pair_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int pairs = std::max(1, std::min(g_num_sms / 2, p.m_tiles * p.n_tiles_n));
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2 * pairs); cfg.blockDim = dim3(kPairThreads);
+  cfg.dynamicSmemBytes = (size_t)gemm_pair_smem_bytes(p.bn, p.stages); cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
+  g_launches++;
+  return cudaLaunchKernelEx(&cfg, gemm_pair_kernel<EPI>, *ma, *mb, p);
+}
+
+// A: bf16 [a_rows_cap, K] buffer (M valid rows); W: bf16 [w_rows, K].
+static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a_rows_cap, const void* W, long long w_rows,
+                     int M, int N, int K, int epi, int bn, GemmPairParams p, cudaStream_t st, bool pdl = false) {
+  if (M <= 0) return DLM_OK;
+  if (K % 8) { set_err(err, "gemm_pair: K=%d must be a multiple of 8", K); return DLM_E_ARG; }
+  if (epi != EPI_LMHEAD && p.ldc % 8) { set_err(err, "gemm_pair: output row pitch %lld must be a multiple of 8 elements", p.ldc); return DLM_E_ARG; }
+  if (bn <= 0) bn = pick_bn_pair(M, N, epi);
+  if (bn % 32 || bn < 64 || bn > 256 || (epi == EPI_SWIGLU && bn % 64)) { set_err(err, "gemm_pair: bad bn=%d", bn); return DLM_E_ARG; }
+  p.M = M; p.N = N; p.K = K; p.bn = bn;
+  const int num_kb = (K + kBK - 1) / kBK;
+  p.stages = std::max(2, std::min(std::min(num_kb, 12), (224 * 1024) / gemm_pair_stage_bytes(bn)));
+  const int per = epi == EPI_SWIGLU ? bn / 2 : bn;
+  p.m_tiles = (M + 255) / 256;
+  p.n_tiles_n = (N + per - 1) / per;
+  p.panel = std::min(p.m_tiles, 16);
+  p.w_policy = DLM_L2_EVICT_NORMAL;
+  p.a_policy = DLM_L2_EVICT_NORMAL;
+  if (epi == EPI_LMHEAD && p.n_tiles_n != p.n_tiles) { set_err(err, "gemm_pair: lm-head tile count mismatch"); return DLM_E_ARG; }
+  const CUtensorMap* ma = tc.get(A, a_rows_cap, K, 128);
+  const CUtensorMap* mb = tc.get(W, w_rows, K, bn / 2);
+  if (!ma || !mb) { set_err(err, "cuTensorMapEncodeTiled failed (gemm_pair A=%p rows=%lld K=%d, W=%p rows=%lld box=%d)", A, a_rows_cap, K, W, w_rows, bn / 2); return DLM_E_CUDA; }
+  cudaError_t e;
+  switch (epi) {
+    case EPI_F32: e = launch_gemm_pair_t<EPI_F32>(ma, mb, p, st, pdl); break;
+    case EPI_BF16: e = launch_gemm_pair_t<EPI_BF16>(ma, mb, p, st, pdl); break;
+    case EPI_RESID: e = launch_gemm_pair_t<EPI_RESID>(ma, mb, p, st, pdl); break;
+    case EPI_SWIGLU: e = launch_gemm_pair_t<EPI_SWIGLU>(ma, mb, p, st, pdl); break;
+    case EPI_LMHEAD: e = launch_gemm_pair_t<EPI_LMHEAD>(ma, mb, p, st, pdl); break;
+    default: set_err(err, "gemm_pair: bad epilogue %d", epi); return DLM_E_ARG;
+  }
+  if (e != cudaSuccess) { set_err(err, "gemm_pair launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
   return DLM_OK;
 }
 
@@ -366,8 +448,8 @@ struct dlm_ctx {
   float* attn_ws = nullptr; size_t attn_ws_bytes = 0;
   float* part_x = nullptr;     // [kSkMaxSplits][<=128][d] split-K slices of the O / down projections
   // options
-  int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1;
-  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3); }
+  int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1;
+  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4); }
   std::map<GraphKey, GraphEntry> graphs;
   // debug dump
   std::map<std::pair<int, int>, void*> dump;   // (layer, which) -> device copy [T, width]
@@ -583,6 +665,7 @@ extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
     case DLM_OPT_KERNEL_TIMING: c->kprof.on = value != 0; return DLM_OK;
     case DLM_OPT_PDL: c->opt_pdl = value != 0; return DLM_OK;
     case DLM_OPT_SKINNY_GEMM: c->opt_skinny = value != 0; return DLM_OK;
+    case DLM_OPT_PAIR_GEMM: c->opt_pair = value != 0; return DLM_OK;
   }
   set_err(&c->err, "unknown option %d", key);
   return DLM_E_ARG;
@@ -748,6 +831,19 @@ static void dump_stage(dlm_ctx* c, int layer, int which, const void* src, size_t
   cudaMemcpyAsync(p, src, row_bytes * rows, cudaMemcpyDeviceToDevice, c->st);
 }
 
+// Large-M projection of the bf16 path: the CTA-pair persistent kernel above 128 tokens, the single-CTA kernel below.
+static int gemm_big(dlm_ctx* c, const void* A, long long a_rows_cap, const void* W, long long w_rows, int M, int N, int K, int epi,
+                    float* out_f32, bf16* out_bf16, long long ldc, int up_row0, bool pdl) {
+  if (M > 128 && c->opt_pair) {
+    GemmPairParams p = {};
+    p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0;
+    return gemm_pair(c->tmaps, &c->err, A, a_rows_cap, W, w_rows, M, N, K, epi, 0, p, c->st, pdl);
+  }
+  GemmTcParams p = {};
+  p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0;
+  return gemm_tc(c->tmaps, &c->err, A, a_rows_cap, W, w_rows, M, N, K, epi, 0, p, c->st, pdl);
+}
+
 template <typename TE>
 static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   const dlm_arch& a = c->a;
@@ -794,9 +890,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, SK_PARTIAL, 0, p, &nq, st, pdl);
         if (rc) return rc;
       } else if (tc) {
-        GemmTcParams p = {};
-        p.out_f32 = c->qkv; p.ldc = NQKV;
-        int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, 0, p, st, pdl);
+        int rc = gemm_big(c, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, c->qkv, nullptr, NQKV, 0, pdl);
         if (rc) return rc;
       } else {
         gemm_plain<TE, TE>(c->qkv, (const TE*)c->u, (const TE*)w.wqkv, T, NQKV, d, st, pdl);
@@ -830,9 +924,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         int rc = gemm_skinny(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, SK_PARTIAL, 0, p, &pend, st, pdl);
         if (rc) return rc;
       } else if (tc) {
-        GemmTcParams p = {};
-        p.out_f32 = c->x; p.ldc = d;
-        int rc = gemm_tc(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, EPI_RESID, 0, p, st, pdl);
+        int rc = gemm_big(c, c->attn, c->Tmax, w.wo, d, T, d, HQ, EPI_RESID, c->x, nullptr, d, 0, pdl);
         if (rc) return rc;
       } else {
         gemm_plain<TE, TE>(c->tmp, (const TE*)c->attn, (const TE*)w.wo, T, d, HQ, st, pdl);
@@ -855,9 +947,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, SK_SWIGLU, 0, p, nullptr, st, pdl);
         if (rc) return rc;
       } else if (tc) {
-        GemmTcParams p = {};
-        p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F;
-        int rc = gemm_tc(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, EPI_SWIGLU, 0, p, st, pdl);
+        int rc = gemm_big(c, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, EPI_SWIGLU, nullptr, (bf16*)c->act, F, F, pdl);
         if (rc) return rc;
       } else {
         gemm_plain<TE, TE>(c->tmp, (const TE*)c->u, (const TE*)w.wgu, T, 2 * F, d, st, pdl);
@@ -873,9 +963,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         int rc = gemm_skinny(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, SK_PARTIAL, 0, p, &pend, st, pdl);
         if (rc) return rc;
       } else if (tc) {
-        GemmTcParams p = {};
-        p.out_f32 = c->x; p.ldc = d;
-        int rc = gemm_tc(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, EPI_RESID, 0, p, st, pdl);
+        int rc = gemm_big(c, c->act, c->Tmax, w.wd, d, T, d, F, EPI_RESID, c->x, nullptr, d, 0, pdl);
         if (rc) return rc;
       } else {
         gemm_plain<TE, TE>(c->tmp, (const TE*)c->act, (const TE*)w.wd, T, d, F, st, pdl);
@@ -903,7 +991,13 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     }
     dump_stage(c, 0, DLM_T_FINAL_NORM, c->hf, (size_t)d * sizeof(TE), R);
     KScope ks(c, DLM_K_LMHEAD);
-    if (tc) {
+    if (tc && R > 128 && c->opt_pair) {          // compute-bound head: CTA-pair kernel, 256-wide vocabulary tiles
+      n_tiles = (V + 255) / 256;
+      GemmPairParams p = {};
+      p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale;
+      int rc = gemm_pair(c->tmaps, err, c->hf, std::max(c->Rmax, 128), c->Wlm, V, R, V, d, EPI_LMHEAD, 256, p, st, pdl);
+      if (rc) return rc;
+    } else if (tc) {
       n_tiles = c->n_tiles;
       GemmTcParams p = {};
       p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale;
@@ -1169,6 +1263,18 @@ extern "C" int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t
   if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
   g_op_tmaps.m.clear();   // caller buffers come and go; never reuse a stale map
   return gemm_tc(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, (cudaStream_t)stream);
+}
+
+extern "C" int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epi, int32_t bn, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!A || !W || !out || M <= 0 || N <= 0 || K <= 0 || epi < 0 || epi > 3) { set_err(&g_init_error, "dlm_op_gemm_pair_bf16: bad arguments"); return DLM_E_ARG; }
+  GemmPairParams p = {};
+  p.ldc = N;
+  p.up_row0 = N;
+  if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
+  g_op_tmaps.m.clear();
+  return gemm_pair(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, (cudaStream_t)stream);
 }
 
 extern "C" int dlm_op_gemm_skinny_bf16(const void* X, const void* W, void* out, int32_t T, int32_t N, int32_t K, int32_t epi, int32_t splits, void* stream) {

@@ -1,0 +1,378 @@
+// Persistent CTA-pair tcgen05 GEMM for M > 128 tokens (refresh steps, large cached batches):
+//   D[M, N] = A[M, K] . W[N, K]^T, bf16 in, fp32 accumulation in tensor memory.  Rows a3, a6, a8, a9, a11 of DESIGN.md.
+//
+// A cluster of two CTAs (one TPC) owns a 256 x BN output tile: tcgen05.mma.cta_group::2 with M = 256, N = BN.
+// Each CTA stages its own 128 rows of A and its own BN/2 rows of W per 64-wide K block, so every operand byte is
+// fetched once per CTA pair (half the L2 -> SM traffic of two independent 128 x BN tiles).  The accumulator is
+// double buffered in TMEM (2 x 256 columns): the epilogue warps drain tile i while the MMAs of tile i+1 run.
+//   warp 0      TMA producer (one lane): `stages`-deep ring, completion of BOTH CTAs' boxes counted on the leader's
+//               full[stage] barrier (cp.async.bulk.tensor ... cta_group::2)
+//   warp 1      TMEM allocation (both CTAs); in the leader one lane issues 4 x UMMA (256 x BN x 16) per K block,
+//               tcgen05.commit multicast to both CTAs frees the stage / publishes the accumulator
+//   warps 2..5  epilogue: tcgen05.ld (lane = row, 32 columns at a time) + the fused epilogue (fp32 | bf16 |
+//               residual add | SwiGLU | LM-head split-vocab statistics), then a remote arrive on the leader's
+//               tmem_empty barrier
+// Tiles are walked persistently (grid = one pair per TPC) in panels of `panel` m-tiles so that a wave shares its A
+// panel and a few W tiles through L2.
+// SwiGLU: the leader CTA stages gate rows, its peer the matching up rows, so accumulator columns [0, BN/2) are
+// the gate and [BN/2, BN) the up projection of the same BN/2 features.
+#pragma once
+#include "attn_flash.cuh"
+#include "common.cuh"
+#include "gemm_tc.cuh"
+#include "kernels_basic.cuh"
+#include "ptx_sm100.cuh"
+
+namespace dlm {
+
+struct GemmPairParams {
+  int M, N, K;        // N = output features (SwiGLU: F; a tile covers bn/2 of them)
+  int bn;             // MMA N of the pair tile: multiple of 32 (SwiGLU: 64) in [64, 256]
+  int stages;
+  int up_row0;        // SwiGLU: first row of the up projection inside W (= F)
+  int m_tiles, n_tiles_n, panel;
+  float* out_f32;     // EPI_F32 / EPI_RESID
+  bf16* out_bf16;     // EPI_BF16 / EPI_SWIGLU
+  long long ldc;
+  RowPartial* part;   // EPI_LMHEAD: [M, n_tiles]
+  int n_tiles;        // row pitch of `part`
+  int mask_id;
+  float scale;
+  unsigned long long w_policy, a_policy;
+};
+
+constexpr int kPairThreads = 192;
+constexpr int kPairAccCols = 256;       // TMEM columns per accumulator stage
+
+__host__ __device__ inline int gemm_pair_stage_bytes(int bn) { return kATileBytes + bn * 64; }   // A 128x64 + W (bn/2)x64
+__host__ inline int gemm_pair_smem_bytes(int bn, int stages) { return stages * gemm_pair_stage_bytes(bn) + 1024 + 512; }
+
+namespace ptx {
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cluster_id_x() { uint32_t r; asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t n_clusters_x() { uint32_t r; asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cta address -> shared::cluster address of the same offset in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// 2-D tile load into this CTA's shared memory; the bytes are counted on an mbarrier that may live in the peer CTA.
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst_smem, const void* tmap, int c0, int c1, uint32_t bar_cluster,
+                                                 uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%3, %4}], [%2], %5;"
+      ::"r"(dst_smem), "l"(tmap), "r"(bar_cluster), "r"(c0), "r"(c1), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t dst_smem, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tmem_relinquish_pair() {
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void umma_bf16_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// Low word of the SWIZZLE_128B K-major descriptor (see umma_desc_sw128); the high word is the constant kDescHiSw128.
+constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (2u << 29);
+__device__ __forceinline__ uint32_t umma_desc_lo(uint32_t smem_addr) { return ((smem_addr & 0x3FFFFu) >> 4) | (1u << 16); }
+__device__ __forceinline__ void umma_bf16_pair_lo(uint32_t tmem_d, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "mov.b64 da, {%1, %5};\n\t"
+      "mov.b64 db, {%2, %5};\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %3, p;\n\t}"
+      ::"r"(tmem_d), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(accumulate), "r"(kDescHiSw128)
+      : "memory");
+}
+// arrive (once) on the barrier at this shared-memory offset in BOTH CTAs of the pair when the MMAs issued so far are done
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"((uint16_t)3)
+               : "memory");
+}
+}  // namespace ptx
+
+struct PairTile { int m_blk, n_blk; };
+__device__ __forceinline__ PairTile pair_tile(int t, int m_tiles, int n_tiles, int panel) {
+  const int pw = panel * n_tiles;
+  const int pid = t / pw, rem = t - pid * pw;
+  const int m_base = pid * panel;
+  const int ph = min(panel, m_tiles - m_base);
+  PairTile r;
+  r.n_blk = rem / ph;
+  r.m_blk = m_base + rem - r.n_blk * ph;
+  return r;
+}
+
+template <int EPI>
+__global__ void __launch_bounds__(kPairThreads, 1)
+gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const GemmPairParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const int BN = p.bn;
+  const int stages = p.stages;
+  const uint32_t stage_bytes = gemm_pair_stage_bytes(BN);
+  const uint32_t bar_base = base + stages * stage_bytes;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };                    // used in the leader
+  auto empty_bar = [&](int s) { return bar_base + 8u * (stages + s); };        // per CTA (multicast commit)
+  const uint32_t tmem_full_bar = bar_base + 16u * stages;                      // [2], per CTA (multicast commit)
+  const uint32_t tmem_empty_bar = tmem_full_bar + 16u;                         // [2], used in the leader
+  const uint32_t tmem_ptr_addr = tmem_empty_bar + 16u;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = ptx::cluster_ctarank();
+  const bool leader = rank == 0;
+  const int cluster = (int)ptx::cluster_id_x(), n_clusters = (int)ptx::n_clusters_x();
+  const int num_kb = (p.K + kBK - 1) / kBK;
+  const int total_tiles = p.m_tiles * p.n_tiles_n;
+
+  ptx::pdl_launch_dependents();
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&mapA);
+    ptx::prefetch_tmap(&mapB);
+    for (int s = 0; s < stages; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int a = 0; a < 2; ++a) { ptx::mbar_init(tmem_full_bar + 8u * a, 1); ptx::mbar_init(tmem_empty_bar + 8u * a, 8); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 1) {
+    ptx::tmem_alloc_pair(tmem_ptr_addr, 512);
+    ptx::tmem_relinquish_pair();
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::cluster_sync();          // the peer's barriers exist before anything is signalled across the pair
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr));
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // ---------------- TMA producer (both CTAs, one lane) ----------------
+      const uint32_t half_rows = (uint32_t)BN / 2;
+      const uint32_t tx_pair = 2u * (kATileBytes + half_rows * 128u);
+      auto w_row_of = [&](const PairTile& tl) {
+        if (EPI == EPI_SWIGLU) return tl.n_blk * (int)half_rows + (leader ? 0 : p.up_row0);
+        return tl.n_blk * BN + (int)rank * (int)half_rows;
+      };
+      // Ring fill of the first tile: weights do not depend on the upstream kernel, so their boxes are issued
+      // before the programmatic-dependency wait; A follows once the producer of A has finished.
+      int pre = 0;
+      if (cluster < total_tiles) {
+        const PairTile tl = pair_tile(cluster, p.m_tiles, p.n_tiles_n, p.panel);
+        const int m0 = tl.m_blk * 256 + (int)rank * 128, w_row = w_row_of(tl);
+        pre = min(stages, num_kb);
+        for (int kb = 0; kb < pre; ++kb) {
+          if (leader) ptx::mbar_expect_tx(full_bar(kb), tx_pair);
+          ptx::tma_load_2d_pair(base + kb * stage_bytes + kATileBytes, &mapB, kb * kBK, w_row, ptx::mapa(full_bar(kb), 0), p.w_policy);
+        }
+        ptx::pdl_wait();
+        for (int kb = 0; kb < pre; ++kb)
+          ptx::tma_load_2d_pair(base + kb * stage_bytes, &mapA, kb * kBK, m0, ptx::mapa(full_bar(kb), 0), p.a_policy);
+      } else {
+        ptx::pdl_wait();
+      }
+      int it = 0;
+      for (int t = cluster; t < total_tiles; t += n_clusters) {
+        const PairTile tl = pair_tile(t, p.m_tiles, p.n_tiles_n, p.panel);
+        const int m0 = tl.m_blk * 256 + (int)rank * 128, w_row = w_row_of(tl);
+        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+          if (it < pre) continue;                       // issued by the ring fill above
+          const int s = it % stages;
+          const uint32_t ph = (uint32_t)(it / stages) & 1u;
+          ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+          const uint32_t fb = ptx::mapa(full_bar(s), 0);
+          if (leader) ptx::mbar_expect_tx(full_bar(s), tx_pair);
+          const uint32_t sa = base + s * stage_bytes;
+          ptx::tma_load_2d_pair(sa + kATileBytes, &mapB, kb * kBK, w_row, fb, p.w_policy);
+          ptx::tma_load_2d_pair(sa, &mapA, kb * kBK, m0, fb, p.a_policy);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (leader) {
+      // ---------------- MMA issuer (leader CTA; the whole warp walks the loop, one elected lane issues) ----------------
+      const uint32_t idesc = ptx::umma_idesc_bf16(256, BN);
+      int it = 0, i = 0;
+      for (int t = cluster; t < total_tiles; t += n_clusters, ++i) {
+        const uint32_t as = (uint32_t)i & 1u, aph = ((uint32_t)i >> 1) & 1u;
+        ptx::mbar_wait(tmem_empty_bar + 8u * as, aph ^ 1u);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + as * kPairAccCols;
+        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+          const int s = it % stages;
+          const uint32_t ph = (uint32_t)(it / stages) & 1u;
+          ptx::mbar_wait(full_bar(s), ph);
+          ptx::tc_fence_after();
+          if (ptx::elect_one()) {
+            const uint32_t sa = base + s * stage_bytes;
+            const uint32_t a_lo = ptx::umma_desc_lo(sa), b_lo = ptx::umma_desc_lo(sa + kATileBytes);
+#pragma unroll
+            for (int k = 0; k < kBK / 16; ++k)        // +32 bytes along K inside the 128-byte swizzle row = +2 in the encoded address
+              ptx::umma_bf16_pair_lo(d_tmem, a_lo + 2 * k, b_lo + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+            ptx::umma_commit_pair(empty_bar(s));          // both CTAs' producers may refill the stage
+            if (kb + 1 == num_kb) ptx::umma_commit_pair(tmem_full_bar + 8u * as);   // accumulator complete in both CTAs' TMEM
+          }
+          __syncwarp();
+        }
+      }
+    }
+  } else {
+    // ---------------- epilogue (warps 2..5 of both CTAs; TMEM lane quarter = warp % 4) ----------------
+    const int quarter = warp & 3;
+    const uint32_t te_leader = ptx::mapa(tmem_empty_bar, 0);
+    int i = 0;
+    for (int t = cluster; t < total_tiles; t += n_clusters, ++i) {
+      const PairTile tl = pair_tile(t, p.m_tiles, p.n_tiles_n, p.panel);
+      const uint32_t as = (uint32_t)i & 1u, aph = ((uint32_t)i >> 1) & 1u;
+      const int row = tl.m_blk * 256 + (int)rank * 128 + quarter * 32 + lane;
+      const bool row_ok = row < p.M;
+      ptx::mbar_wait(tmem_full_bar + 8u * as, aph);
+      ptx::tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + as * kPairAccCols;
+      uint32_t r[32];
+      if (EPI == EPI_F32 || EPI == EPI_RESID || EPI == EPI_BF16) {
+        const int n0 = tl.n_blk * BN;
+        for (int c = 0; c < BN / 32; ++c) {
+          __syncwarp();
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+          const int col0 = n0 + c * 32;
+          if (!row_ok || col0 >= p.N) {
+            // nothing to store (the warp stays converged for the next tcgen05.ld)
+          } else if (EPI == EPI_BF16) {
+            bf16* o = p.out_bf16 + (long long)row * p.ldc + col0;
+            if (col0 + 32 <= p.N) {
+#pragma unroll
+              for (int j = 0; j < 32; j += 8) {
+                uint4 v;
+                v.x = pack_bf16(__uint_as_float(r[j]), __uint_as_float(r[j + 1]));
+                v.y = pack_bf16(__uint_as_float(r[j + 2]), __uint_as_float(r[j + 3]));
+                v.z = pack_bf16(__uint_as_float(r[j + 4]), __uint_as_float(r[j + 5]));
+                v.w = pack_bf16(__uint_as_float(r[j + 6]), __uint_as_float(r[j + 7]));
+                *reinterpret_cast<uint4*>(o + j) = v;
+              }
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) if (col0 + j < p.N) o[j] = __float2bfloat16_rn(__uint_as_float(r[j]));
+            }
+          } else {
+            float* o = p.out_f32 + (long long)row * p.ldc + col0;
+            if (col0 + 32 <= p.N) {
+              float4 x[8];
+              if (EPI == EPI_RESID) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) x[j] = *reinterpret_cast<const float4*>(o + 4 * j);
+              }
+#pragma unroll
+              for (int j = 0; j < 8; ++j) {
+                float4 v = make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]), __uint_as_float(r[4 * j + 2]),
+                                       __uint_as_float(r[4 * j + 3]));
+                if (EPI == EPI_RESID) { v.x += x[j].x; v.y += x[j].y; v.z += x[j].z; v.w += x[j].w; }
+                *reinterpret_cast<float4*>(o + 4 * j) = v;
+              }
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) {
+                if (col0 + j < p.N) {
+                  float v = __uint_as_float(r[j]);
+                  o[j] = (EPI == EPI_RESID) ? o[j] + v : v;
+                }
+              }
+            }
+          }
+        }
+      } else if (EPI == EPI_SWIGLU) {
+        const int half = BN / 2;
+        const int f0 = tl.n_blk * half;
+        uint32_t u[32];
+        for (int c = 0; c < half / 32; ++c) {
+          __syncwarp();
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_32x32(taddr + half + c * 32, u);
+          ptx::tmem_ld_wait();
+          const int fc = f0 + c * 32;
+          bf16* o = p.out_bf16 + (long long)row * p.ldc + fc;
+          if (!row_ok || fc >= p.N) {
+          } else if (fc + 32 <= p.N) {
+#pragma unroll
+            for (int j = 0; j < 32; j += 8) {
+              uint32_t w[4];
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                float a0 = silu_f(__uint_as_float(r[j + 2 * q])) * __uint_as_float(u[j + 2 * q]);
+                float a1 = silu_f(__uint_as_float(r[j + 2 * q + 1])) * __uint_as_float(u[j + 2 * q + 1]);
+                w[q] = pack_bf16(a0, a1);
+              }
+              *reinterpret_cast<uint4*>(o + j) = make_uint4(w[0], w[1], w[2], w[3]);
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j)
+              if (fc + j < p.N) o[j] = __float2bfloat16_rn(silu_f(__uint_as_float(r[j])) * __uint_as_float(u[j]));
+          }
+        }
+      } else if (EPI == EPI_LMHEAD) {
+        // a11: split-vocab online (max, sum exp(z - max), argmax); z = scale * acc; mask_id and columns >= V excluded.
+        const int n0 = tl.n_blk * BN;
+        float m = -CUDART_INF_F, ssum = 0.f;
+        int idx = 0x7fffffff;
+        for (int c = 0; c < BN / 32; ++c) {
+          __syncwarp();
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+          const int col0 = n0 + c * 32;
+          float cm = -CUDART_INF_F;
+          int ci = 0x7fffffff;
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const int col = col0 + j;
+            float z = __uint_as_float(r[j]) * p.scale;
+            if (col >= p.N || col == p.mask_id) z = -CUDART_INF_F;
+            r[j] = __float_as_uint(z);
+            if (z > cm) { cm = z; ci = col; }        // strict > keeps the lowest column on ties
+          }
+          if (cm != -CUDART_INF_F) {
+            if (cm > m) { ssum *= __expf(m - cm); m = cm; idx = ci; }
+            float cs = 0.f;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) cs += __expf(__uint_as_float(r[j]) - m);
+            ssum += cs;
+          }
+        }
+        if (row_ok) {
+          RowPartial o;
+          o.m = m; o.s = ssum; o.idx = idx; o.pad = 0;
+          *reinterpret_cast<int4*>(p.part + (long long)row * p.n_tiles + tl.n_blk) = *reinterpret_cast<int4*>(&o);
+        }
+      }
+      // this warp's quarter of the accumulator stage has been read: let the leader's MMA issuer reuse it
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive_cluster(te_leader + 8u * as);
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::cluster_sync();          // no CTA of the pair frees TMEM / leaves while its peer may still signal it
+  if (warp == 1) ptx::tmem_dealloc_pair(tmem_base, 512);
+}
+
+}  // namespace dlm

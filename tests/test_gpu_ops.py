@@ -65,6 +65,47 @@ def test_gemm_tc_swiglu(M, F, K, bn):
     assert np.all(np.abs(_f64(got) - want) <= np.abs(want) * 2 ** -8 + 1e-4)
 
 
+PAIR_SHAPES = [  # (M, N, K): one and several 256-row tiles, ragged tails in every dimension, > 1 tile per pair
+    (129, 256, 128), (300, 200, 512), (512, 768, 256), (257, 96, 4096), (1000, 1056, 200), (2240, 512, 320), (130, 4608, 64)]
+
+
+@pytest.mark.parametrize("M,N,K", PAIR_SHAPES)
+@pytest.mark.parametrize("bn", [0, 64, 96, 160, 256])
+def test_gemm_pair_store_and_residual(M, N, K, bn):
+    """Persistent CTA-pair tcgen05 GEMM (refresh-step a3/a6/a9) vs fp64 matmul."""
+    import paper_2606_29094_b200 as pkg
+    rng = np.random.default_rng(M * 7 + N * 3 + K + bn)
+    A, a = _mk(rng, M, K)
+    W, w = _mk(rng, N, K, 0.05)
+    want = a @ w.T
+    tol = 2e-5 * np.sqrt(K) * np.abs(a).max() * np.abs(w).max() + 1e-6
+    got = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_F32, bn)
+    torch.cuda.synchronize()
+    assert np.abs(_f64(got) - want).max() <= tol
+    x0 = rng.standard_normal((M, N)).astype(np.float32)
+    x = torch.from_numpy(x0).cuda()
+    pkg.op_gemm_pair_bf16(A, W, pkg.EPI_RESID, bn, out=x)
+    torch.cuda.synchronize()
+    assert np.abs(_f64(x) - (x0.astype(np.float64) + want)).max() <= tol + 1e-6
+    gb = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_BF16, bn)
+    torch.cuda.synchronize()
+    assert np.all(np.abs(_f64(gb) - want) <= np.abs(want) * 2 ** -8 + tol)
+
+
+@pytest.mark.parametrize("M,F,K", [(200, 128, 128), (270, 688, 256), (600, 352, 512), (129, 64, 64), (512, 1536, 1024)])
+@pytest.mark.parametrize("bn", [0, 64, 128, 192, 256])
+def test_gemm_pair_swiglu(M, F, K, bn):
+    import paper_2606_29094_b200 as pkg
+    rng = np.random.default_rng(M + F + K + bn)
+    A, a = _mk(rng, M, K)
+    W, w = _mk(rng, 2 * F, K, 0.1 if K < 1024 else 0.03)
+    want = omodel.silu(a @ w[:F].T) * (a @ w[F:].T)
+    got = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_SWIGLU, bn)
+    torch.cuda.synchronize()
+    assert got.shape == (M, F)
+    assert np.all(np.abs(_f64(got) - want) <= np.abs(want) * 2 ** -8 + 2e-4)
+
+
 SKINNY_SHAPES = [  # (T, N, K): tails in every dimension, one and several K blocks per split
     (32, 256, 128), (1, 128, 64), (32, 4096, 4096), (17, 384, 688), (64, 200, 512), (100, 1056, 200), (128, 768, 256), (33, 96, 4096)]
 
