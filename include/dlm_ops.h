@@ -30,9 +30,11 @@ DLM_API int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t M,
 /* Same contraction and epilogues on the persistent CTA-pair kernel the engine uses for M > 128 tokens (refresh
  * steps, large cached batches): clusters of two CTAs, tcgen05.mma.cta_group::2 on 256 x bn tiles, accumulator
  * double-buffered in tensor memory.  bn = 0 picks the tile width; otherwise a multiple of 32 in [64, 256]
- * (multiple of 64 for SwiGLU). */
+ * (multiple of 64 for SwiGLU).  splits (DLM_EPI_F32 only): 1 = no split-K; n > 1 = n K ranges, each writing an fp32
+ * slice, summed in slice order; 0 = the split the engine would choose.  Returns the number of K splits used
+ * (>= 1) or a DLM_E_* code; with splits != 1 the call synchronises the stream. */
 DLM_API int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epilogue,
-                          int32_t bn, void* stream);
+                          int32_t bn, int32_t splits, void* stream);
 
 /* Weight-streaming split-K tcgen05 GEMM for T <= 128 tokens (the cached step's a3/a6/a8/a9): swap-AB (weights on
  * the MMA's M side, tokens on N), every K split writes an fp32 slice and the slices are summed in a fixed order.
@@ -60,8 +62,8 @@ DLM_API int dlm_op_lmhead_unmask_bf16(const void* hidden, const void* W_lm, int3
                               void* stream);
 
 /* Non-causal block attention over a contiguous (unpaged) K/V, bf16 (a5): q [Tq, H, d_h], k/v [S, H_kv, d_h]
- * -> out [Tq, H, d_h]; softmax_j(q.k_j/sqrt(d_h)) v_j over all j.  flash = 1: tensor-core
- * online-softmax kernel; 0: plain kernel. */
+ * -> out [Tq, H, d_h]; softmax_j(q.k_j/sqrt(d_h)) v_j over all j.  flash = 0: plain kernel; 1: mma.sync
+ * online-softmax kernel; 2: tcgen05/TMEM kernel with the K/V split the engine would pick; 2 + s: the same with s K/V splits. */
 DLM_API int dlm_op_attention_bf16(const void* q, const void* k, const void* v, void* out, int32_t Tq, int32_t S,
                           int32_t H, int32_t H_kv, int32_t d_h, int32_t flash, void* stream);
 

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libdlm.so")
 
 DLM_OK, DLM_E_ARG, DLM_E_CAPACITY, DLM_E_STATE, DLM_E_CUDA = 0, -1, -2, -3, -4
 DLM_DRY_RUN = 1
-OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM, OPT_PAIR_GEMM = 1, 2, 3, 4, 5, 6, 7, 8
+OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM, OPT_PAIR_GEMM, OPT_TC_ATTENTION = 1, 2, 3, 4, 5, 6, 7, 8, 9
 KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
                 "combine_unmask")
 KIND_REFRESH, KIND_CACHED = 0, 1
@@ -103,7 +103,7 @@ def lib() -> C.CDLL:
         L.dlm_last_error.argtypes = [vp]
         L.dlm_last_error.restype = C.c_char_p
         L.dlm_op_gemm_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
-        L.dlm_op_gemm_pair_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
+        L.dlm_op_gemm_pair_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
         L.dlm_op_gemm_plain_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp]
         L.dlm_op_gemm_skinny_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
         L.dlm_op_lmhead_scratch_bytes.argtypes = [i32, i32]
@@ -316,15 +316,16 @@ def op_gemm_bf16(A, W, epilogue: int = EPI_F32, bn: int = 0, out=None):
     return out
 
 
-def op_gemm_pair_bf16(A, W, epilogue: int = EPI_F32, bn: int = 0, out=None):
-    """Persistent CTA-pair tcgen05 GEMM (the engine's M > 128 path)."""
+def op_gemm_pair_bf16(A, W, epilogue: int = EPI_F32, bn: int = 0, out=None, splits: int = 1, return_splits: bool = False):
+    """Persistent CTA-pair tcgen05 GEMM (the engine's M > 128 path); splits: see include/dlm_ops.h."""
     import torch
     M, K = A.shape
     N = W.shape[0] // 2 if epilogue == EPI_SWIGLU else W.shape[0]
     if out is None:
         out = torch.empty(M, N, device=A.device, dtype=torch.float32 if epilogue in (EPI_F32, EPI_RESID) else torch.bfloat16)
-    _op_check(lib().dlm_op_gemm_pair_bf16(A.data_ptr(), W.data_ptr(), out.data_ptr(), M, N, K, epilogue, bn, _stream_ptr()))
-    return out
+    rc = lib().dlm_op_gemm_pair_bf16(A.data_ptr(), W.data_ptr(), out.data_ptr(), M, N, K, epilogue, bn, splits, _stream_ptr())
+    _op_check(rc)
+    return (out, rc) if return_splits else out
 
 
 def op_gemm_skinny_bf16(X, W, epilogue: int = EPI_F32, splits: int = 0):
@@ -376,11 +377,12 @@ def op_lmhead_unmask_bf16(hidden, W_lm, n: int, B: int, scale: float, mask_id: i
     return ncomm, pos, tok, conf
 
 
-def op_attention_bf16(q, k, v, flash: bool = True):
+def op_attention_bf16(q, k, v, flash=True):
+    """flash: False/0 plain, True/1 mma.sync kernel, 2 tcgen05 kernel (auto K/V split), 2 + s tcgen05 with s splits."""
     import torch
     Tq, H, dh = q.shape
     S, Hkv, _ = k.shape
     out = torch.empty_like(q)
     _op_check(lib().dlm_op_attention_bf16(q.data_ptr(), k.data_ptr(), v.data_ptr(), out.data_ptr(), Tq, S, H, Hkv, dh,
-                                          1 if flash else 0, _stream_ptr()))
+                                          int(flash), _stream_ptr()))
     return out

@@ -263,14 +263,10 @@ static int attn_flash_launch(bf16* out, const bf16* q, const bf16* kv_store, con
   p.out = out; p.q = q; p.kv_store = kv_store; p.page_table = page_table; p.b = bd; p.g = g; p.layer = layer; p.n_heads = n_heads;
   p.splits = splits; p.scale_log2 = scale * 1.4426950408889634f; p.ws_o = nullptr; p.ws_ml = nullptr;
   const long long TH = (long long)bd.T * n_heads;
+  // the split-KV workspace is allocated once by the caller (captured CUDA graphs keep its address): fit the split to it
+  while (splits > 1 && (size_t)splits * TH * (kFaDh + 2) * 4 > *ws_bytes) --splits;
+  p.splits = splits;
   if (splits > 1) {
-    const size_t need = (size_t)splits * TH * (kFaDh + 2) * 4;
-    if (*ws_bytes < need) {
-      if (*ws) cudaFree(*ws);
-      *ws = nullptr; *ws_bytes = 0;
-      if (cudaMalloc(ws, need) != cudaSuccess) { *err = "attn_flash: workspace allocation failed"; return -2; }
-      *ws_bytes = need;
-    }
     p.ws_o = *ws;
     p.ws_ml = *ws + (size_t)splits * TH * kFaDh;
   }

@@ -17,6 +17,7 @@
 #include "../../include/dlm.h"
 #include "../../include/dlm_ops.h"
 #include "attn_flash.cuh"
+#include "attn_tc.cuh"
 #include "common.cuh"
 #include "gemm_skinny.cuh"
 #include "gemm_pair.cuh"
@@ -173,26 +174,34 @@ static int gemm_tc(TmapCache& tc, std::string* err, const void* A, long long a_r
 // ------------------------------------------------------------------------------------------------
 // CTA-pair persistent tcgen05 GEMM launcher (M > 128)
 // ------------------------------------------------------------------------------------------------
-// Tile width.  Measured on B200: with both operands in shared memory one 256 x bn x 16 UMMA takes ~128 cycles for
-// every bn <= 256 (the A-operand read paces it), so a tile costs the same whatever its width: take the widest tile
-// among those with the fewest waves over one pair per TPC.
-static int pick_bn_pair(int M, int N, int epi) {
-  if (epi == EPI_LMHEAD) return 256;
+// Tile width and K split.  Measured on B200: with both operands in shared memory one 256 x bn x 16 UMMA takes
+// ~128 cycles for every bn <= 256 (the A-operand read paces it), so a work unit costs its K blocks whatever its
+// width.  Cost of a launch ~ waves x (K blocks per unit + fixed per-unit cost); ties go to fewer splits, then to the
+// wider tile (fewer operand bytes per flop).  Split-K (fp32 slices, summed by the consumer in a fixed order) is what
+// fills the 74 CTA pairs when M x N alone gives fewer than ~74 tiles (O / down projections at 512 tokens).
+static void plan_pair(int M, int N, int K, int epi, int max_splits, int* bn_out, int* splits_out) {
   const int m_tiles = (M + 255) / 256;
   const int pairs = std::max(1, g_num_sms / 2);
+  const int num_kb = (K + kBK - 1) / kBK;
   static const int cand_std[] = {256, 224, 192, 160, 128, 96, 64};
   static const int cand_glu[] = {256, 192, 128, 64};
-  const int* cand = epi == EPI_SWIGLU ? cand_glu : cand_std;
-  const int nc = epi == EPI_SWIGLU ? 4 : 7;
-  long long best_waves = -1;
-  int best = cand[0];
-  for (int i = 0; i < nc; ++i) {
-    const int per = epi == EPI_SWIGLU ? cand[i] / 2 : cand[i];
-    const long long tiles = (long long)m_tiles * ((N + per - 1) / per);
-    const long long waves = (tiles + pairs - 1) / pairs;
-    if (best_waves < 0 || waves < best_waves) { best_waves = waves; best = cand[i]; }
+  static const int cand_lm[] = {256};
+  const int* cand = epi == EPI_SWIGLU ? cand_glu : (epi == EPI_LMHEAD ? cand_lm : cand_std);
+  const int nc = epi == EPI_SWIGLU ? 4 : (epi == EPI_LMHEAD ? 1 : 7);
+  const int unit_fixed = 8;                           // epilogue tail + ramp, in K-block units
+  long long best = -1;
+  *bn_out = cand[0]; *splits_out = 1;
+  for (int sp = 1; sp <= std::max(1, max_splits); ++sp) {
+    const int kb_per = (num_kb + sp - 1) / sp;
+    if (sp > 1 && ((sp - 1) * kb_per >= num_kb || kb_per < 8)) continue;
+    for (int i = 0; i < nc; ++i) {
+      const int per = epi == EPI_SWIGLU ? cand[i] / 2 : cand[i];
+      const long long units = (long long)m_tiles * ((N + per - 1) / per) * sp;
+      const long long waves = (units + pairs - 1) / pairs;
+      const long long cost = waves * (kb_per + unit_fixed);
+      if (best < 0 || cost < best) { best = cost; *bn_out = cand[i]; *splits_out = sp; }
+    }
   }
-  return best;
 }
 
 template <int EPI>
@@ -203,7 +212,7 @@ static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* 
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  const int pairs = std::max(1, std::min(g_num_sms / 2, p.m_tiles * p.n_tiles_n));
+  const int pairs = std::max(1, std::min(g_num_sms / 2, p.m_tiles * p.n_tiles_n * p.splits));
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(2 * pairs); cfg.blockDim = dim3(kPairThreads);
   cfg.dynamicSmemBytes = (size_t)gemm_pair_smem_bytes(p.bn, p.stages); cfg.stream = st;
@@ -217,16 +226,27 @@ static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* 
   return cudaLaunchKernelEx(&cfg, gemm_pair_kernel<EPI>, *ma, *mb, p);
 }
 
-// A: bf16 [a_rows_cap, K] buffer (M valid rows); W: bf16 [w_rows, K].
+// A: bf16 [a_rows_cap, K] buffer (M valid rows); W: bf16 [w_rows, K].  max_splits > 1 (EPI_F32 only) allows split-K:
+// p.out_f32 then receives *splits_out slices [split][M][ldc] which the consumer sums.
 static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a_rows_cap, const void* W, long long w_rows,
-                     int M, int N, int K, int epi, int bn, GemmPairParams p, cudaStream_t st, bool pdl = false) {
+                     int M, int N, int K, int epi, int bn, GemmPairParams p, cudaStream_t st, bool pdl = false,
+                     int max_splits = 1, int* splits_out = nullptr) {
+  if (splits_out) *splits_out = M > 0 ? 1 : 0;
   if (M <= 0) return DLM_OK;
   if (K % 8) { set_err(err, "gemm_pair: K=%d must be a multiple of 8", K); return DLM_E_ARG; }
   if (epi != EPI_LMHEAD && p.ldc % 8) { set_err(err, "gemm_pair: output row pitch %lld must be a multiple of 8 elements", p.ldc); return DLM_E_ARG; }
-  if (bn <= 0) bn = pick_bn_pair(M, N, epi);
+  if (epi != EPI_F32) max_splits = 1;
+  int splits = 1;
+  if (bn <= 0) plan_pair(M, N, K, epi, max_splits, &bn, &splits);
+  else if (max_splits < 0) splits = -max_splits;                 // test hook: forced split count
   if (bn % 32 || bn < 64 || bn > 256 || (epi == EPI_SWIGLU && bn % 64)) { set_err(err, "gemm_pair: bad bn=%d", bn); return DLM_E_ARG; }
   p.M = M; p.N = N; p.K = K; p.bn = bn;
   const int num_kb = (K + kBK - 1) / kBK;
+  splits = std::max(1, std::min(splits, num_kb));
+  p.kb_per_split = (num_kb + splits - 1) / splits;
+  p.splits = (num_kb + p.kb_per_split - 1) / p.kb_per_split;
+  p.split_stride = (long long)M * p.ldc;
+  if (splits_out) *splits_out = p.splits;
   p.stages = std::max(2, std::min(std::min(num_kb, 12), (224 * 1024) / gemm_pair_stage_bytes(bn)));
   const int per = epi == EPI_SWIGLU ? bn / 2 : bn;
   p.m_tiles = (M + 255) / 256;
@@ -249,6 +269,60 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
   }
   if (e != cudaSuccess) { set_err(err, "gemm_pair launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
   return DLM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// tcgen05 attention launcher.  *done = false when the shape is not supported or too small to fill the GPU with
+// 128-row tiles (the caller then takes the mma.sync kernel).
+// ------------------------------------------------------------------------------------------------
+static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* kv_store, int n_layers_total, const int* page_table,
+                          const BatchDesc& bd, const KvGeom& g, int layer, int n_heads, float scale, float** ws, size_t* ws_bytes,
+                          cudaStream_t st, bool pdl, std::string* err, bool* done, int force = 0) {
+  *done = false;
+  if (g.head_dim != 128 || g.page_tokens != 64 || bd.T <= 0) return 0;
+  const int r = n_heads / g.n_kv_heads;
+  const int q_tiles = (bd.max_q_len * r + kTaTile - 1) / kTaTile;
+  const long long items = (long long)bd.n * g.n_kv_heads * q_tiles;
+  const int kv_tiles = (bd.max_kv_len + kTaTile - 1) / kTaTile;
+  if (!force && items * kv_tiles < 4LL * g_num_sms) return 0;       // too little work for one-CTA-per-SM tiles of 128 x 128
+  const long long rows = (long long)n_layers_total * g.n_pages * 2 * g.n_kv_heads * g.page_tokens;
+  if (rows >= (1LL << 31)) return 0;
+  int splits = 1;
+  {
+    long long best = -1;
+    for (int s = 1; s <= std::min(8, kv_tiles); ++s) {
+      const long long waves = (items * s + g_num_sms - 1) / g_num_sms;
+      const long long cost = waves * ((kv_tiles + s - 1) / s + 1);
+      if (best < 0 || cost < best) { best = cost; splits = s; }
+    }
+    if (force > 1) splits = std::min(force - 1, kv_tiles);
+  }
+  const CUtensorMap* mkv = tc.get(kv_store, rows, 128, 64);
+  if (!mkv) { set_err(err, "cuTensorMapEncodeTiled failed (attention K/V store %p, %lld rows)", (const void*)kv_store, rows); return DLM_E_CUDA; }
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTaSmem);
+    if (e != cudaSuccess) { set_err(err, "attn_tc: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+    configured = true;
+  }
+  TaParams p;
+  p.out = out; p.q = q; p.page_table = page_table; p.b = bd; p.g = g; p.layer = layer; p.n_heads = n_heads;
+  p.splits = splits; p.q_tiles_max = q_tiles; p.n_items = (int)(items * splits);
+  p.scale_log2 = scale * 1.4426950408889634f; p.ws_o = nullptr; p.ws_ml = nullptr;
+  p.kv_policy = q_tiles == 1 ? DLM_L2_EVICT_FIRST : DLM_L2_EVICT_NORMAL;
+  const long long TH = (long long)bd.T * n_heads;
+  while (splits > 1 && (size_t)splits * TH * (128 + 2) * 4 > *ws_bytes) --splits;     // fixed workspace (see attn_flash_launch)
+  p.splits = splits; p.n_items = (int)(items * splits);
+  if (splits > 1) {
+    p.ws_o = *ws;
+    p.ws_ml = *ws + (size_t)splits * TH * 128;
+  }
+  cudaError_t e = launch_k(attn_tc_kernel, dim3((unsigned)std::min<long long>(g_num_sms, p.n_items)), dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
+  if (splits > 1 && e == cudaSuccess)
+    e = launch_k(attn_combine_kernel, dim3((unsigned)TH), dim3(kFaDh), 0, st, pdl, out, (const float*)p.ws_o, (const float*)p.ws_ml, TH, splits);
+  if (e != cudaSuccess) { set_err(err, "attn_tc launch: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+  *done = true;
+  return 0;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -344,8 +418,15 @@ static int attn_op_contiguous(const void* q, const void* k, const void* v, void*
   const float scale = 1.f / sqrtf((float)dh);
   int rc = DLM_OK;
   bool done = false;
-  float* ws = nullptr; size_t wsb = 0;
-  if (flash) {
+  float* ws = nullptr;
+  size_t wsb = (size_t)32 * Tq * H * (128 + 2) * 4;
+  if (flash && cudaMalloc(&ws, wsb) != cudaSuccess) { cudaFree(store); cudaFree(meta); set_err(err, "dlm_op_attention_bf16: allocation failed"); return DLM_E_CAPACITY; }
+  if (flash >= 2) {
+    static TmapCache op_maps;
+    op_maps.m.clear();
+    rc = attn_tc_launch(op_maps, (bf16*)out, (const bf16*)q, store, 1, meta, bd, g, 0, H, scale, &ws, &wsb, st, false, err, &done, flash - 1);
+    if (!rc && !done) { set_err(err, "dlm_op_attention_bf16: tcgen05 kernel does not support d_h=%d", dh); rc = DLM_E_ARG; }
+  } else if (flash) {
     rc = attn_flash_launch((bf16*)out, (const bf16*)q, store, meta, bd, g, 0, H, scale, &ws, &wsb, g_num_sms, st, false, err, &done);
     if (!rc && !done) { set_err(err, "dlm_op_attention_bf16: flash kernel does not support d_h=%d", dh); rc = DLM_E_ARG; }
   } else {
@@ -446,10 +527,11 @@ struct dlm_ctx {
   char* out_dev = nullptr; char* out_host = nullptr; size_t out_bytes = 0;
   // attention split-KV scratch
   float* attn_ws = nullptr; size_t attn_ws_bytes = 0;
-  float* part_x = nullptr;     // [kSkMaxSplits][<=128][d] split-K slices of the O / down projections
+  float* part_x = nullptr;     // [splits][T][d] split-K slices of the O / down projections (part_rows rows in all)
+  long long part_rows = 0, qkv_rows = 0;
   // options
-  int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1;
-  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4); }
+  int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1, opt_tcattn = 1;
+  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4) | (opt_tcattn << 5); }
   std::map<GraphKey, GraphEntry> graphs;
   // debug dump
   std::map<std::pair<int, int>, void*> dump;   // (layer, which) -> device copy [T, width]
@@ -595,8 +677,11 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   c->Rmax = a.max_requests * a.max_block;
   c->n_tiles = c->bf16_model ? (int)((V + 127) / 128) : 1;
   ALLOC(c->x, (size_t)c->Tmax * d * 4);
-  ALLOC(c->qkv, (size_t)std::max<long long>(c->Tmax, (long long)kSkMaxSplits * kSkMaxTokens) * NQKV * 4);
-  if (c->bf16_model) ALLOC(c->part_x, (size_t)kSkMaxSplits * kSkMaxTokens * d * 4);
+  // fp32 slice capacity (rows): split-K slices of the skinny path (<= 16 x 128 tokens) and of the pair path (<= 4 x M)
+  c->qkv_rows = std::max<long long>(std::max<long long>(c->Tmax, (long long)kSkMaxSplits * kSkMaxTokens), std::min<long long>(3LL * c->Tmax, 4096));
+  c->part_rows = std::max<long long>((long long)kSkMaxSplits * kSkMaxTokens, std::min<long long>(4LL * c->Tmax, 4096));
+  ALLOC(c->qkv, (size_t)c->qkv_rows * NQKV * 4);
+  if (c->bf16_model) ALLOC(c->part_x, (size_t)c->part_rows * d * 4);
   ALLOC(c->u, (size_t)c->Tmax * d * es);
   ALLOC(c->q, (size_t)c->Tmax * HQ * es);
   ALLOC(c->attn, (size_t)c->Tmax * HQ * es);
@@ -604,6 +689,10 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   ALLOC(c->hf, (size_t)std::max(c->Rmax, 128) * d * es);
   ALLOC(c->part, (size_t)c->Rmax * std::max(c->n_tiles, 1) * sizeof(RowPartial));
   ALLOC(c->row_src, (size_t)c->Rmax * 4);
+  if (c->bf16_model) {      // split-KV partials of the attention kernels: fixed size, so captured graphs stay valid
+    c->attn_ws_bytes = (size_t)8 * std::min(c->Tmax, 1024) * a.n_heads * (128 + 2) * 4;
+    ALLOC(c->attn_ws, c->attn_ws_bytes);
+  }
   c->desc_cap_ints = (size_t)10 * a.max_requests + c->Tmax + 64;      // 9 n + T used
   ALLOC(c->desc_dev, c->desc_cap_ints * 4);
   if (cudaMallocHost(&c->desc_host, c->desc_cap_ints * 4) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
@@ -629,7 +718,6 @@ extern "C" void dlm_destroy(dlm_ctx* c) {
   for (auto& g : c->graphs) if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
   if (c->tmp) cudaFree(c->tmp);
   if (c->logits) cudaFree(c->logits);
-  if (c->attn_ws) cudaFree(c->attn_ws);
   c->dfree_all();
   if (c->desc_host) cudaFreeHost(c->desc_host);
   if (c->out_host) cudaFreeHost(c->out_host);
@@ -666,6 +754,7 @@ extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
     case DLM_OPT_PDL: c->opt_pdl = value != 0; return DLM_OK;
     case DLM_OPT_SKINNY_GEMM: c->opt_skinny = value != 0; return DLM_OK;
     case DLM_OPT_PAIR_GEMM: c->opt_pair = value != 0; return DLM_OK;
+    case DLM_OPT_TC_ATTENTION: c->opt_tcattn = value != 0; return DLM_OK;
   }
   set_err(&c->err, "unknown option %d", key);
   return DLM_E_ARG;
@@ -832,16 +921,37 @@ static void dump_stage(dlm_ctx* c, int layer, int which, const void* src, size_t
 }
 
 // Large-M projection of the bf16 path: the CTA-pair persistent kernel above 128 tokens, the single-CTA kernel below.
+// slice_rows_cap > 0 (EPI_F32 into a buffer of that many rows): split-K allowed, *n_slices tells the consumer how
+// many [M, ldc] slices to sum.
 static int gemm_big(dlm_ctx* c, const void* A, long long a_rows_cap, const void* W, long long w_rows, int M, int N, int K, int epi,
-                    float* out_f32, bf16* out_bf16, long long ldc, int up_row0, bool pdl) {
+                    float* out_f32, bf16* out_bf16, long long ldc, int up_row0, bool pdl, long long slice_rows_cap = 0, int* n_slices = nullptr) {
+  if (n_slices) *n_slices = 1;
   if (M > 128 && c->opt_pair) {
     GemmPairParams p = {};
     p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0;
-    return gemm_pair(c->tmaps, &c->err, A, a_rows_cap, W, w_rows, M, N, K, epi, 0, p, c->st, pdl);
+    const int max_splits = (n_slices && slice_rows_cap > 0) ? (int)std::min<long long>(4, slice_rows_cap / M) : 1;
+    return gemm_pair(c->tmaps, &c->err, A, a_rows_cap, W, w_rows, M, N, K, epi, 0, p, c->st, pdl, max_splits, n_slices);
   }
   GemmTcParams p = {};
   p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0;
   return gemm_tc(c->tmaps, &c->err, A, a_rows_cap, W, w_rows, M, N, K, epi, 0, p, c->st, pdl);
+}
+
+// O / down projection of the large-M path: residual add fused in the epilogue, or -- when split-K pays -- fp32 slices
+// in part_x that the next RMSNorm folds into the residual stream (*pend = slices pending).
+static int gemm_big_resid(dlm_ctx* c, const void* A, const void* W, int M, int N, int K, bool pdl, int* pend) {
+  *pend = 0;
+  if (M > 128 && c->opt_pair && c->part_x && c->part_rows >= 2LL * M) {
+    int bn = 0, sp = 1;
+    plan_pair(M, N, K, EPI_F32, (int)std::min<long long>(4, c->part_rows / M), &bn, &sp);
+    if (sp > 1) {
+      int ns = 1;
+      int rc = gemm_big(c, A, c->Tmax, W, N, M, N, K, EPI_F32, c->part_x, nullptr, N, 0, pdl, c->part_rows, &ns);
+      *pend = ns;
+      return rc;
+    }
+  }
+  return gemm_big(c, A, c->Tmax, W, N, M, N, K, EPI_RESID, c->x, nullptr, N, 0, pdl);
 }
 
 template <typename TE>
@@ -890,7 +1000,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, SK_PARTIAL, 0, p, &nq, st, pdl);
         if (rc) return rc;
       } else if (tc) {
-        int rc = gemm_big(c, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, c->qkv, nullptr, NQKV, 0, pdl);
+        int rc = gemm_big(c, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, c->qkv, nullptr, NQKV, 0, pdl, c->qkv_rows, &nq);
         if (rc) return rc;
       } else {
         gemm_plain<TE, TE>(c->qkv, (const TE*)c->u, (const TE*)w.wqkv, T, NQKV, d, st, pdl);
@@ -904,7 +1014,13 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     }
     dump_stage(c, l, DLM_T_Q, c->q, (size_t)HQ * sizeof(TE), T);
     bool flash_done = false;
-    if (tc && c->opt_flash) {
+    if (tc && c->opt_flash && c->opt_tcattn) {
+      KScope ks(c, DLM_K_ATTENTION);
+      int rc = attn_tc_launch(c->tmaps, (bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, a.n_layers, c->page_table, bd, c->kg, l,
+                              a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, st, pdl, err, &flash_done, 0);
+      if (rc) return rc;
+    }
+    if (tc && c->opt_flash && !flash_done) {
       KScope ks(c, DLM_K_ATTENTION);
       int rc = attn_flash_launch((bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, c->page_table, bd, c->kg, l,
                                  a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, pdl, err, &flash_done);
@@ -924,7 +1040,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         int rc = gemm_skinny(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, SK_PARTIAL, 0, p, &pend, st, pdl);
         if (rc) return rc;
       } else if (tc) {
-        int rc = gemm_big(c, c->attn, c->Tmax, w.wo, d, T, d, HQ, EPI_RESID, c->x, nullptr, d, 0, pdl);
+        int rc = gemm_big_resid(c, c->attn, w.wo, T, d, HQ, pdl, &pend);
         if (rc) return rc;
       } else {
         gemm_plain<TE, TE>(c->tmp, (const TE*)c->attn, (const TE*)w.wo, T, d, HQ, st, pdl);
@@ -963,7 +1079,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         int rc = gemm_skinny(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, SK_PARTIAL, 0, p, &pend, st, pdl);
         if (rc) return rc;
       } else if (tc) {
-        int rc = gemm_big(c, c->act, c->Tmax, w.wd, d, T, d, F, EPI_RESID, c->x, nullptr, d, 0, pdl);
+        int rc = gemm_big_resid(c, c->act, w.wd, T, d, F, pdl, &pend);
         if (rc) return rc;
       } else {
         gemm_plain<TE, TE>(c->tmp, (const TE*)c->act, (const TE*)w.wd, T, d, F, st, pdl);
@@ -1265,16 +1381,40 @@ extern "C" int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t
   return gemm_tc(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, (cudaStream_t)stream);
 }
 
-extern "C" int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epi, int32_t bn, void* stream) {
+extern "C" int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epi, int32_t bn,
+                                     int32_t splits, void* stream) {
   int rc = op_check_device();
   if (rc) return rc;
-  if (!A || !W || !out || M <= 0 || N <= 0 || K <= 0 || epi < 0 || epi > 3) { set_err(&g_init_error, "dlm_op_gemm_pair_bf16: bad arguments"); return DLM_E_ARG; }
+  if (!A || !W || !out || M <= 0 || N <= 0 || K <= 0 || epi < 0 || epi > 3 || splits < 0 || splits > 8 || (splits > 1 && epi != EPI_F32)) {
+    set_err(&g_init_error, "dlm_op_gemm_pair_bf16: bad arguments"); return DLM_E_ARG;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
   GemmPairParams p = {};
   p.ldc = N;
   p.up_row0 = N;
-  if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
   g_op_tmaps.m.clear();
-  return gemm_pair(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, (cudaStream_t)stream);
+  if (epi != EPI_F32 || splits == 1) {
+    if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
+    rc = gemm_pair(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, st);
+    return rc < 0 ? rc : 1;
+  }
+  // split-K: slices in a scratch buffer, summed in slice order into `out`
+  const long long n = (long long)M * N;
+  const int cap = splits ? splits : 4;
+  float* part = nullptr;
+  if (cudaMalloc(&part, (size_t)cap * n * 4) != cudaSuccess) { set_err(&g_init_error, "dlm_op_gemm_pair_bf16: allocation failed"); return DLM_E_CAPACITY; }
+  p.out_f32 = part;
+  int ns = 0;
+  if (splits == 0) rc = gemm_pair(g_op_tmaps, &g_init_error, A, M, W, N, M, N, K, epi, 0, p, st, false, cap, &ns);
+  else rc = gemm_pair(g_op_tmaps, &g_init_error, A, M, W, N, M, N, K, epi, bn > 0 ? bn : 256, p, st, false, -splits, &ns);
+  if (!rc) {
+    cudaMemsetAsync(out, 0, (size_t)n * 4, st);
+    launch_k(add_partials_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, st, false, (float*)out, (const float*)part, ns, n, n);
+  }
+  cudaError_t e = cudaStreamSynchronize(st);
+  cudaFree(part);
+  if (!rc && e != cudaSuccess) { set_err(&g_init_error, "dlm_op_gemm_pair_bf16: %s", cudaGetErrorString(e)); rc = DLM_E_CUDA; }
+  return rc < 0 ? rc : ns;
 }
 
 extern "C" int dlm_op_gemm_skinny_bf16(const void* X, const void* W, void* out, int32_t T, int32_t N, int32_t K, int32_t epi, int32_t splits, void* stream) {

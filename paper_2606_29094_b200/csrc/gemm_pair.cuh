@@ -31,6 +31,8 @@ struct GemmPairParams {
   int stages;
   int up_row0;        // SwiGLU: first row of the up projection inside W (= F)
   int m_tiles, n_tiles_n, panel;
+  int splits, kb_per_split;      // split-K (EPI_F32 only): unit = (tile, K range); split s writes slice out_f32 + s * split_stride
+  long long split_stride;
   float* out_f32;     // EPI_F32 / EPI_RESID
   bf16* out_bf16;     // EPI_BF16 / EPI_SWIGLU
   long long ldc;
@@ -143,6 +145,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
   const int cluster = (int)ptx::cluster_id_x(), n_clusters = (int)ptx::n_clusters_x();
   const int num_kb = (p.K + kBK - 1) / kBK;
   const int total_tiles = p.m_tiles * p.n_tiles_n;
+  const int total_units = total_tiles * p.splits;      // unit u: tile u % total_tiles, K split u / total_tiles
 
   ptx::pdl_launch_dependents();
   if (warp == 0 && lane == 0) {
@@ -175,25 +178,28 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
       // Ring fill of the first tile: weights do not depend on the upstream kernel, so their boxes are issued
       // before the programmatic-dependency wait; A follows once the producer of A has finished.
       int pre = 0;
-      if (cluster < total_tiles) {
-        const PairTile tl = pair_tile(cluster, p.m_tiles, p.n_tiles_n, p.panel);
+      if (cluster < total_units) {
+        const PairTile tl = pair_tile(cluster % total_tiles, p.m_tiles, p.n_tiles_n, p.panel);
         const int m0 = tl.m_blk * 256 + (int)rank * 128, w_row = w_row_of(tl);
-        pre = min(stages, num_kb);
+        const int kb0 = (cluster / total_tiles) * p.kb_per_split;
+        pre = min(stages, min(p.kb_per_split, num_kb - kb0));
         for (int kb = 0; kb < pre; ++kb) {
           if (leader) ptx::mbar_expect_tx(full_bar(kb), tx_pair);
-          ptx::tma_load_2d_pair(base + kb * stage_bytes + kATileBytes, &mapB, kb * kBK, w_row, ptx::mapa(full_bar(kb), 0), p.w_policy);
+          ptx::tma_load_2d_pair(base + kb * stage_bytes + kATileBytes, &mapB, (kb0 + kb) * kBK, w_row, ptx::mapa(full_bar(kb), 0), p.w_policy);
         }
         ptx::pdl_wait();
         for (int kb = 0; kb < pre; ++kb)
-          ptx::tma_load_2d_pair(base + kb * stage_bytes, &mapA, kb * kBK, m0, ptx::mapa(full_bar(kb), 0), p.a_policy);
+          ptx::tma_load_2d_pair(base + kb * stage_bytes, &mapA, (kb0 + kb) * kBK, m0, ptx::mapa(full_bar(kb), 0), p.a_policy);
       } else {
         ptx::pdl_wait();
       }
       int it = 0;
-      for (int t = cluster; t < total_tiles; t += n_clusters) {
-        const PairTile tl = pair_tile(t, p.m_tiles, p.n_tiles_n, p.panel);
+      for (int u = cluster; u < total_units; u += n_clusters) {
+        const PairTile tl = pair_tile(u % total_tiles, p.m_tiles, p.n_tiles_n, p.panel);
         const int m0 = tl.m_blk * 256 + (int)rank * 128, w_row = w_row_of(tl);
-        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+        const int kb0 = (u / total_tiles) * p.kb_per_split;
+        const int nkb = min(p.kb_per_split, num_kb - kb0);
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
           if (it < pre) continue;                       // issued by the ring fill above
           const int s = it % stages;
           const uint32_t ph = (uint32_t)(it / stages) & 1u;
@@ -201,8 +207,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
           const uint32_t fb = ptx::mapa(full_bar(s), 0);
           if (leader) ptx::mbar_expect_tx(full_bar(s), tx_pair);
           const uint32_t sa = base + s * stage_bytes;
-          ptx::tma_load_2d_pair(sa + kATileBytes, &mapB, kb * kBK, w_row, fb, p.w_policy);
-          ptx::tma_load_2d_pair(sa, &mapA, kb * kBK, m0, fb, p.a_policy);
+          ptx::tma_load_2d_pair(sa + kATileBytes, &mapB, (kb0 + kb) * kBK, w_row, fb, p.w_policy);
+          ptx::tma_load_2d_pair(sa, &mapA, (kb0 + kb) * kBK, m0, fb, p.a_policy);
         }
       }
     }
@@ -211,12 +217,13 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
       // ---------------- MMA issuer (leader CTA; the whole warp walks the loop, one elected lane issues) ----------------
       const uint32_t idesc = ptx::umma_idesc_bf16(256, BN);
       int it = 0, i = 0;
-      for (int t = cluster; t < total_tiles; t += n_clusters, ++i) {
+      for (int u = cluster; u < total_units; u += n_clusters, ++i) {
         const uint32_t as = (uint32_t)i & 1u, aph = ((uint32_t)i >> 1) & 1u;
         ptx::mbar_wait(tmem_empty_bar + 8u * as, aph ^ 1u);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kPairAccCols;
-        for (int kb = 0; kb < num_kb; ++kb, ++it) {
+        const int nkb = min(p.kb_per_split, num_kb - (u / total_tiles) * p.kb_per_split);
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
           const int s = it % stages;
           const uint32_t ph = (uint32_t)(it / stages) & 1u;
           ptx::mbar_wait(full_bar(s), ph);
@@ -228,7 +235,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
             for (int k = 0; k < kBK / 16; ++k)        // +32 bytes along K inside the 128-byte swizzle row = +2 in the encoded address
               ptx::umma_bf16_pair_lo(d_tmem, a_lo + 2 * k, b_lo + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
             ptx::umma_commit_pair(empty_bar(s));          // both CTAs' producers may refill the stage
-            if (kb + 1 == num_kb) ptx::umma_commit_pair(tmem_full_bar + 8u * as);   // accumulator complete in both CTAs' TMEM
+            if (kb + 1 == nkb) ptx::umma_commit_pair(tmem_full_bar + 8u * as);   // accumulator complete in both CTAs' TMEM
           }
           __syncwarp();
         }
@@ -239,8 +246,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     const int quarter = warp & 3;
     const uint32_t te_leader = ptx::mapa(tmem_empty_bar, 0);
     int i = 0;
-    for (int t = cluster; t < total_tiles; t += n_clusters, ++i) {
-      const PairTile tl = pair_tile(t, p.m_tiles, p.n_tiles_n, p.panel);
+    for (int u = cluster; u < total_units; u += n_clusters, ++i) {
+      const PairTile tl = pair_tile(u % total_tiles, p.m_tiles, p.n_tiles_n, p.panel);
       const uint32_t as = (uint32_t)i & 1u, aph = ((uint32_t)i >> 1) & 1u;
       const int row = tl.m_blk * 256 + (int)rank * 128 + quarter * 32 + lane;
       const bool row_ok = row < p.M;
@@ -274,7 +281,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
               for (int j = 0; j < 32; ++j) if (col0 + j < p.N) o[j] = __float2bfloat16_rn(__uint_as_float(r[j]));
             }
           } else {
-            float* o = p.out_f32 + (long long)row * p.ldc + col0;
+            float* o = p.out_f32 + (long long)(u / total_tiles) * p.split_stride + (long long)row * p.ldc + col0;
             if (col0 + 32 <= p.N) {
               float4 x[8];
               if (EPI == EPI_RESID) {

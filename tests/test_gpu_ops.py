@@ -92,6 +92,22 @@ def test_gemm_pair_store_and_residual(M, N, K, bn):
     assert np.all(np.abs(_f64(gb) - want) <= np.abs(want) * 2 ** -8 + tol)
 
 
+@pytest.mark.parametrize("M,N,K", [(512, 512, 4096), (300, 200, 1024), (257, 96, 4096), (1000, 1056, 640)])
+@pytest.mark.parametrize("splits", [0, 2, 3, 4])
+def test_gemm_pair_split_k(M, N, K, splits):
+    """Split-K units of the CTA-pair kernel (O / down projections of a 512-token step): slices summed in order."""
+    import paper_2606_29094_b200 as pkg
+    rng = np.random.default_rng(M + N + K + splits)
+    A, a = _mk(rng, M, K)
+    W, w = _mk(rng, N, K, 0.05)
+    want = a @ w.T
+    tol = 2e-5 * np.sqrt(K) * np.abs(a).max() * np.abs(w).max() + 1e-6
+    got, ns = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_F32, 0 if splits == 0 else 256, splits=splits, return_splits=True)
+    torch.cuda.synchronize()
+    assert 1 <= ns <= 4 and (splits == 0 or ns <= splits)
+    assert np.abs(_f64(got) - want).max() <= tol
+
+
 @pytest.mark.parametrize("M,F,K", [(200, 128, 128), (270, 688, 256), (600, 352, 512), (129, 64, 64), (512, 1536, 1024)])
 @pytest.mark.parametrize("bn", [0, 64, 128, 192, 256])
 def test_gemm_pair_swiglu(M, F, K, bn):
@@ -229,6 +245,42 @@ def test_attention(Tq, S, H, Hkv, flash):
     assert np.isfinite(got).all()
     err = np.abs(got - want).max()
     assert err < (6e-3 if flash else 3e-3), err      # P rounded to bf16 for the PV MMA + bf16 output
+
+
+@pytest.mark.parametrize("Tq,S,H,Hkv", [(32, 512, 4, 4), (64, 200, 8, 2), (5, 64, 2, 1), (100, 1000, 7, 1), (512, 512, 2, 2),
+                                        (32, 4608, 2, 2), (300, 300, 4, 2), (64, 129, 1, 1)])
+@pytest.mark.parametrize("mode", [2, 3, 5])
+def test_attention_tcgen05(Tq, S, H, Hkv, mode):
+    """tcgen05/TMEM attention (128-row query tiles, 128-token K/V tiles, lazy rescale, optional K/V split) vs
+    oracle.attention (fp64): ragged tails in rows and K/V, GQA stacking, several tiles per item."""
+    import paper_2606_29094_b200 as pkg
+    rng = np.random.default_rng(Tq + S + H + mode)
+    dh = 128
+    q = _bf16((rng.standard_normal((Tq, H, dh)) * 1.5).astype(np.float32)).cuda()
+    k = _bf16(rng.standard_normal((S, Hkv, dh)).astype(np.float32)).cuda()
+    v = _bf16(rng.standard_normal((S, Hkv, dh)).astype(np.float32)).cuda()
+    want = omodel.attention(_f64(q), _f64(k), _f64(v))
+    got = _f64(pkg.op_attention_bf16(q, k, v, mode))
+    assert np.isfinite(got).all()
+    err = np.abs(got - want).max()
+    assert err < 8e-3, err      # P rounded to bf16 for the PV MMA + bf16 output
+
+
+def test_attention_tcgen05_growing_scores():
+    """Scores that keep growing along K/V force the lazy-rescale path (running max raised by > 2^8 several times)."""
+    import paper_2606_29094_b200 as pkg
+    rng = np.random.default_rng(77)
+    Tq, S, H, dh = 40, 1024, 2, 128
+    qn = rng.standard_normal((Tq, H, dh)).astype(np.float32)
+    kn = rng.standard_normal((S, H, dh)).astype(np.float32) * 0.3
+    kn += (np.arange(S, dtype=np.float32)[:, None, None] / S) * 1.2 * np.sign(qn[0:1, :, :])   # drift along q[0]
+    q, k = _bf16(qn).cuda(), _bf16(kn).cuda()
+    v = _bf16(rng.standard_normal((S, H, dh)).astype(np.float32)).cuda()
+    want = omodel.attention(_f64(q), _f64(k), _f64(v))
+    for mode in (2, 3):
+        got = _f64(pkg.op_attention_bf16(q, k, v, mode))
+        assert np.isfinite(got).all()
+        assert np.abs(got - want).max() < 8e-3
 
 
 def test_attention_plain_small_head():
