@@ -147,6 +147,7 @@ DLM_API int  dlm_profile_step_costs(dlm_ctx*, dlm_cost_row* rows, int32_t cap, i
 #define DLM_OPT_PDL            6   /* 1 (default): programmatic dependent launch between the kernels of a step           */
 #define DLM_OPT_SKINNY_GEMM    7   /* 1 (default): weight-streaming split-K GEMM for steps of <= 128 tokens; 0: tile GEMM */
 #define DLM_OPT_TC_ATTENTION   9   /* 1 (default): tcgen05/TMEM attention kernel when a step has enough (request, head) work; 0: mma.sync kernel */
+#define DLM_OPT_FUSE_ROPE     10   /* 1 (default): above 128 tokens RoPE + K/V page write run in the QKV GEMM's epilogue; 0: separate kernel */
 #define DLM_OPT_PAIR_GEMM      8   /* 1 (default): persistent CTA-pair (cta_group::2) GEMM above 128 tokens; 0: single-CTA tile GEMM */
 DLM_API int  dlm_set_option(dlm_ctx*, int32_t key, int32_t value);
 

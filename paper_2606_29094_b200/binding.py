@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libdlm.so")
 
 DLM_OK, DLM_E_ARG, DLM_E_CAPACITY, DLM_E_STATE, DLM_E_CUDA = 0, -1, -2, -3, -4
 DLM_DRY_RUN = 1
-OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM, OPT_PAIR_GEMM, OPT_TC_ATTENTION = 1, 2, 3, 4, 5, 6, 7, 8, 9
+OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM, OPT_PAIR_GEMM, OPT_TC_ATTENTION, OPT_FUSE_ROPE = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
                 "combine_unmask")
 KIND_REFRESH, KIND_CACHED = 0, 1

@@ -297,44 +297,65 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tc_kernel(const __grid_con
         const uint32_t s_addr = tmem_base + lane_addr + b * 128;
         ptx::mbar_wait(s_full(b), (uint32_t)(sc >> 1) & 1u);
         ptx::tc_fence_after();
+        // P_j = exp2(S_j * scale - m) in bf16, held in registers.  This is the MUFU-bound part (16 ex2 per clock per SM) and
+        // it overlaps the PV product of the previous tile, which still owns the shared-memory P buffer.  After the
+        // first tile the previous reference max is used speculatively (one pass over the scores, loads of the next 32
+        // columns in flight while the current ones are exponentiated); only a row whose scores outgrow it by more than
+        // 2^kTaRescaleThreshold takes a second pass with the new max and rescales O.
         float m_new = m_used;
         bool need = false;
-        if (warp_live) {
-          float mx = -CUDART_INF_F;
-#pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            ptx::tmem_ld_32x32(s_addr + c * 32, rg);
-            ptx::tmem_ld_wait();
-            if (c * 32 + 32 <= n_valid) {
-#pragma unroll
-              for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(rg[i]));
-            } else {
-#pragma unroll
-              for (int i = 0; i < 32; ++i) if (c * 32 + i < n_valid) mx = fmaxf(mx, __uint_as_float(rg[i]));
-            }
-          }
-          mx *= p.scale_log2;
-          if (j == 0) m_new = mx;
-          else if (mx > m_used + kTaRescaleThreshold) { m_new = mx; need = true; }
-        }
-        // P_j = exp2(S_j * scale - m) in bf16, held in registers: this is the MUFU-bound part and it overlaps the PV
-        // product of the previous tile, which still owns the shared-memory P buffer
         uint32_t pk[64];
         float rs = 0.f;
         if (warp_live) {
+          uint32_t ra[32], rb[32];
+          const bool full = n_valid == kTaTile;       // warp-uniform
+          if (j == 0) {
+            float mx = -CUDART_INF_F;
+            ptx::tmem_ld_32x32(s_addr, ra);
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            ptx::tmem_ld_32x32(s_addr + c * 32, rg);
-            ptx::tmem_ld_wait();
+            for (int c = 0; c < 4; ++c) {
+              ptx::tmem_ld_wait();
+              if (c < 3) ptx::tmem_ld_32x32(s_addr + (c + 1) * 32, (c & 1) ? ra : rb);
+              const uint32_t(&cur)[32] = (c & 1) ? rb : ra;
 #pragma unroll
-            for (int i = 0; i < 32; i += 2) {
-              float p0 = ptx::ex2(fmaf(__uint_as_float(rg[i]), p.scale_log2, -m_new));
-              float p1 = ptx::ex2(fmaf(__uint_as_float(rg[i + 1]), p.scale_log2, -m_new));
-              if (c * 32 + i >= n_valid) p0 = 0.f;
-              if (c * 32 + i + 1 >= n_valid) p1 = 0.f;
-              rs += p0 + p1;
-              pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
+              for (int i = 0; i < 32; ++i) if (full || c * 32 + i < n_valid) mx = fmaxf(mx, __uint_as_float(cur[i]));
             }
+            m_new = mx * p.scale_log2;
+          }
+          for (int pass = 0; pass < 2; ++pass) {
+            float mx = -CUDART_INF_F;
+            rs = 0.f;
+            ptx::tmem_ld_32x32(s_addr, ra);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              ptx::tmem_ld_wait();
+              if (c < 3) ptx::tmem_ld_32x32(s_addr + (c + 1) * 32, (c & 1) ? ra : rb);
+              const uint32_t(&cur)[32] = (c & 1) ? rb : ra;
+              if (full) {
+#pragma unroll
+                for (int i = 0; i < 32; i += 2) {
+                  const float s0 = __uint_as_float(cur[i]), s1 = __uint_as_float(cur[i + 1]);
+                  mx = fmaxf(mx, fmaxf(s0, s1));
+                  const float p0 = ptx::ex2(fmaf(s0, p.scale_log2, -m_new)), p1 = ptx::ex2(fmaf(s1, p.scale_log2, -m_new));
+                  rs += p0 + p1;
+                  pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
+                }
+              } else {
+#pragma unroll
+                for (int i = 0; i < 32; i += 2) {
+                  const bool v0 = c * 32 + i < n_valid, v1 = c * 32 + i + 1 < n_valid;
+                  const float s0 = v0 ? __uint_as_float(cur[i]) : -CUDART_INF_F, s1 = v1 ? __uint_as_float(cur[i + 1]) : -CUDART_INF_F;
+                  mx = fmaxf(mx, fmaxf(s0, s1));
+                  const float p0 = v0 ? ptx::ex2(fmaf(s0, p.scale_log2, -m_new)) : 0.f, p1 = v1 ? ptx::ex2(fmaf(s1, p.scale_log2, -m_new)) : 0.f;
+                  rs += p0 + p1;
+                  pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
+                }
+              }
+            }
+            mx *= p.scale_log2;
+            const bool grow = j > 0 && pass == 0 && mx > m_new + kTaRescaleThreshold;
+            if (grow) { m_new = mx; need = true; }
+            if (!__any_sync(0xffffffffu, grow)) break;       // warp-uniform: the second pass is rare
           }
         }
         ptx::tc_fence_before();

@@ -234,9 +234,10 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
   if (splits_out) *splits_out = M > 0 ? 1 : 0;
   if (M <= 0) return DLM_OK;
   if (K % 8) { set_err(err, "gemm_pair: K=%d must be a multiple of 8", K); return DLM_E_ARG; }
-  if (epi != EPI_LMHEAD && p.ldc % 8) { set_err(err, "gemm_pair: output row pitch %lld must be a multiple of 8 elements", p.ldc); return DLM_E_ARG; }
+  if (epi != EPI_LMHEAD && epi != EPI_ROPE && p.ldc % 8) { set_err(err, "gemm_pair: output row pitch %lld must be a multiple of 8 elements", p.ldc); return DLM_E_ARG; }
   if (epi != EPI_F32) max_splits = 1;
   int splits = 1;
+  if (epi == EPI_ROPE) bn = 256;                                 // two 128-wide heads per tile
   if (bn <= 0) plan_pair(M, N, K, epi, max_splits, &bn, &splits);
   else if (max_splits < 0) splits = -max_splits;                 // test hook: forced split count
   if (bn % 32 || bn < 64 || bn > 256 || (epi == EPI_SWIGLU && bn % 64)) { set_err(err, "gemm_pair: bad bn=%d", bn); return DLM_E_ARG; }
@@ -265,6 +266,7 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
     case EPI_RESID: e = launch_gemm_pair_t<EPI_RESID>(ma, mb, p, st, pdl); break;
     case EPI_SWIGLU: e = launch_gemm_pair_t<EPI_SWIGLU>(ma, mb, p, st, pdl); break;
     case EPI_LMHEAD: e = launch_gemm_pair_t<EPI_LMHEAD>(ma, mb, p, st, pdl); break;
+    case EPI_ROPE: e = launch_gemm_pair_t<EPI_ROPE>(ma, mb, p, st, pdl); break;
     default: set_err(err, "gemm_pair: bad epilogue %d", epi); return DLM_E_ARG;
   }
   if (e != cudaSuccess) { set_err(err, "gemm_pair launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
@@ -530,8 +532,8 @@ struct dlm_ctx {
   float* part_x = nullptr;     // [splits][T][d] split-K slices of the O / down projections (part_rows rows in all)
   long long part_rows = 0, qkv_rows = 0;
   // options
-  int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1, opt_tcattn = 1;
-  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4) | (opt_tcattn << 5); }
+  int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1, opt_tcattn = 1, opt_fuse_rope = 1;
+  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4) | (opt_tcattn << 5) | (opt_fuse_rope << 6); }
   std::map<GraphKey, GraphEntry> graphs;
   // debug dump
   std::map<std::pair<int, int>, void*> dump;   // (layer, which) -> device copy [T, width]
@@ -755,6 +757,7 @@ extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
     case DLM_OPT_SKINNY_GEMM: c->opt_skinny = value != 0; return DLM_OK;
     case DLM_OPT_PAIR_GEMM: c->opt_pair = value != 0; return DLM_OK;
     case DLM_OPT_TC_ATTENTION: c->opt_tcattn = value != 0; return DLM_OK;
+    case DLM_OPT_FUSE_ROPE: c->opt_fuse_rope = value != 0; return DLM_OK;
   }
   set_err(&c->err, "unknown option %d", key);
   return DLM_E_ARG;
@@ -961,6 +964,8 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   const int T = bd.T, d = a.d_model, F = a.d_ffn, V = a.vocab, HQ = a.n_heads * a.head_dim, NQKV = nqkv(a);
   const bool tc = c->bf16_model && !c->opt_simple;
   const bool skinny = tc && c->opt_skinny && T <= kSkMaxTokens;      // weight-streaming regime (cached steps of small batches)
+  // a3 + a4 in one kernel above 128 tokens: the QKV epilogue rotates, rounds and writes Q and the K/V pages itself
+  const bool fuse_rope = tc && !skinny && T > 128 && c->opt_pair && c->opt_fuse_rope && a.head_dim == 128 && NQKV % 256 == 0;
   const bool pdl = c->opt_pdl && !c->kprof.on;                        // event pairs between kernels would serialise anyway
   const float scale = 1.f / sqrtf((float)a.head_dim);
   std::string* err = &c->err;
@@ -999,6 +1004,12 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         p.out_f32 = c->qkv; p.ldc = NQKV;
         int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, SK_PARTIAL, 0, p, &nq, st, pdl);
         if (rc) return rc;
+      } else if (fuse_rope) {
+        GemmPairParams p = {};
+        p.rope.q = (bf16*)c->q; p.rope.kv_store = (bf16*)c->kv_store; p.rope.rope_cos = c->rope_cos; p.rope.rope_sin = c->rope_sin;
+        p.rope.page_table = c->page_table; p.rope.b = bd; p.rope.g = c->kg; p.rope.layer = l; p.rope.n_heads = a.n_heads;
+        int rc = gemm_pair(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_ROPE, 256, p, st, pdl);
+        if (rc) return rc;
       } else if (tc) {
         int rc = gemm_big(c, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, c->qkv, nullptr, NQKV, 0, pdl, c->qkv_rows, &nq);
         if (rc) return rc;
@@ -1006,7 +1017,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         gemm_plain<TE, TE>(c->qkv, (const TE*)c->u, (const TE*)w.wqkv, T, NQKV, d, st, pdl);
       }
     }
-    {
+    if (!fuse_rope) {
       KScope ks(c, DLM_K_ROPE_KV);
       const int hpb = std::max(1, 256 / (a.head_dim / 2));       // heads per block
       launch_k(rope_kv_write_kernel<TE>, dim3(T, (a.n_heads + 2 * a.n_kv_heads + hpb - 1) / hpb), dim3(hpb * (a.head_dim / 2)), 0, st, pdl, (TE*)c->q, (TE*)c->kv_store, (const float*)c->qkv, (const float*)c->rope_cos,

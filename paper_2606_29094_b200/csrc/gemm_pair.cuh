@@ -25,6 +25,20 @@
 
 namespace dlm {
 
+// EPI_ROPE (a3 + a4 fused): the QKV projection's epilogue rotates Q and K (half-split pairs, table lookup by absolute
+// position), rounds to bf16 and writes Q to [T, H, 128] and K / V straight into the request's pages.
+constexpr int EPI_ROPE = 5;
+struct RopeEpi {
+  bf16* q;
+  bf16* kv_store;
+  const float* rope_cos;   // [max_seq, 64]
+  const float* rope_sin;
+  const int* page_table;
+  BatchDesc b;
+  KvGeom g;
+  int layer, n_heads;
+};
+
 struct GemmPairParams {
   int M, N, K;        // N = output features (SwiGLU: F; a tile covers bn/2 of them)
   int bn;             // MMA N of the pair tile: multiple of 32 (SwiGLU: 64) in [64, 256]
@@ -41,6 +55,7 @@ struct GemmPairParams {
   int mask_id;
   float scale;
   unsigned long long w_policy, a_policy;
+  RopeEpi rope;       // EPI_ROPE
 };
 
 constexpr int kPairThreads = 192;
@@ -334,6 +349,63 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
 #pragma unroll
             for (int j = 0; j < 32; ++j)
               if (fc + j < p.N) o[j] = __float2bfloat16_rn(silu_f(__uint_as_float(r[j])) * __uint_as_float(u[j]));
+          }
+        }
+      } else if (EPI == EPI_ROPE) {
+        // tile = 256 columns = two heads of 128; thread = token row; pairs (i, i + 64) live in chunks (a, a + 2)
+        const RopeEpi& e = p.rope;
+        int pos = 0, page = 0, slot_in_page = 0;
+        if (row_ok) {
+          const int bi = e.b.tok_bi[row];
+          pos = e.b.q_pos0[bi] + (row - e.b.q_off[bi]);
+          page = e.page_table[(long long)e.b.slot[bi] * e.g.max_pages_per_req + pos / e.g.page_tokens];
+          slot_in_page = pos % e.g.page_tokens;
+        }
+        const float4* cs4 = reinterpret_cast<const float4*>(e.rope_cos + (long long)pos * 64);
+        const float4* sn4 = reinterpret_cast<const float4*>(e.rope_sin + (long long)pos * 64);
+        uint32_t u[32];
+#pragma unroll 1
+        for (int hh = 0; hh < 2; ++hh) {
+          const int hg = tl.n_blk * 2 + hh;                     // global head index: Q heads, then K heads, then V heads
+          const bool head_ok = hg < e.n_heads + 2 * e.g.n_kv_heads;
+          const bool rotate = hg < e.n_heads + e.g.n_kv_heads;
+          bf16* dst = nullptr;
+          if (row_ok && head_ok) {
+            if (hg < e.n_heads) dst = e.q + ((long long)row * e.n_heads + hg) * 128;
+            else if (rotate) dst = e.kv_store + e.g.offset(e.layer, page, 0, hg - e.n_heads, slot_in_page);
+            else dst = e.kv_store + e.g.offset(e.layer, page, 1, hg - e.n_heads - e.g.n_kv_heads, slot_in_page);
+          }
+#pragma unroll 1
+          for (int a = 0; a < 2; ++a) {
+            __syncwarp();
+            ptx::tmem_ld_32x32(taddr + hh * 128 + a * 32, r);
+            ptx::tmem_ld_32x32(taddr + hh * 128 + a * 32 + 64, u);
+            ptx::tmem_ld_wait();
+            if (dst) {
+              if (rotate) {
+#pragma unroll
+                for (int j = 0; j < 32; j += 4) {
+                  const float4 c = cs4[a * 8 + (j >> 2)], s = sn4[a * 8 + (j >> 2)];
+                  const float cc[4] = {c.x, c.y, c.z, c.w}, ss[4] = {s.x, s.y, s.z, s.w};
+#pragma unroll
+                  for (int q = 0; q < 4; ++q) {
+                    const float lo = __uint_as_float(r[j + q]), hi = __uint_as_float(u[j + q]);
+                    r[j + q] = __float_as_uint(lo * cc[q] - hi * ss[q]);
+                    u[j + q] = __float_as_uint(hi * cc[q] + lo * ss[q]);
+                  }
+                }
+              }
+#pragma unroll
+              for (int j = 0; j < 32; j += 8) {
+                uint4 v, w;
+                v.x = pack_bf16(__uint_as_float(r[j]), __uint_as_float(r[j + 1])); v.y = pack_bf16(__uint_as_float(r[j + 2]), __uint_as_float(r[j + 3]));
+                v.z = pack_bf16(__uint_as_float(r[j + 4]), __uint_as_float(r[j + 5])); v.w = pack_bf16(__uint_as_float(r[j + 6]), __uint_as_float(r[j + 7]));
+                w.x = pack_bf16(__uint_as_float(u[j]), __uint_as_float(u[j + 1])); w.y = pack_bf16(__uint_as_float(u[j + 2]), __uint_as_float(u[j + 3]));
+                w.z = pack_bf16(__uint_as_float(u[j + 4]), __uint_as_float(u[j + 5])); w.w = pack_bf16(__uint_as_float(u[j + 6]), __uint_as_float(u[j + 7]));
+                *reinterpret_cast<uint4*>(dst + a * 32 + j) = v;
+                *reinterpret_cast<uint4*>(dst + a * 32 + 64 + j) = w;
+              }
+            }
           }
         }
       } else if (EPI == EPI_LMHEAD) {
