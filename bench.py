@@ -144,8 +144,8 @@ class Runner:
     """Drives a batch of requests through libdlm the way the paper's scheduler would: every
     request gets the step kind that is due; refresh and cached requests of one iteration go in two calls."""
 
-    def __init__(self, pkg, arch, seed, specs):
-        self.pkg, self.arch, self.specs = pkg, arch, specs
+    def __init__(self, pkg, arch, seed, specs, mixed_launch=True):
+        self.pkg, self.arch, self.specs, self.mixed_launch = pkg, arch, specs, mixed_launch
         max_seq = max(len(s.prompt) + s.gen_len for s in specs)
         max_seq = (max_seq + 63) // 64 * 64
         self.max_block = max(s.block_len for s in specs)
@@ -181,20 +181,25 @@ class Runner:
             (cached if st["cache_valid"] else refresh).append(i)
         usec, commits = 0.0, 0
         q_lens, kv_lens, rows = [], [], 0
-        for kind, idx in (("refresh", refresh), ("cached", cached)):
+        if refresh and cached and self.mixed_launch:
+            calls = (("mixed", refresh + cached),)          # one ragged launch, weights streamed once (dlm_mixed_step)
+        else:
+            calls = (("refresh", refresh), ("cached", cached))
+        for kind, idx in calls:
             if not idx:
                 continue
             rids = [self.ids[i] for i in idx]
-            g = eng.refresh_step(rids) if kind == "refresh" else eng.cached_step(rids)
+            is_ref = set(refresh)
+            g = eng.refresh_step(rids) if kind == "refresh" else (eng.cached_step(rids) if kind == "cached" else eng.mixed_step(rids))
             usec += g.usec
             commits += g.total
-            self.h2d += 4 * (10 * len(rids) + sum((len(self.specs[i].prompt) + self.specs[i].gen_len) if kind == "refresh"
+            self.h2d += 4 * (10 * len(rids) + sum((len(self.specs[i].prompt) + self.specs[i].gen_len) if (kind == "refresh" or (kind == "mixed" and i in is_ref))
                                                    else self.specs[i].block_len for i in idx))
             self.d2h += 4 * (len(self.specs) + 6 * len(self.specs) * self.max_block)
             for i in idx:
                 s = self.specs[i]
                 S = len(s.prompt) + s.gen_len
-                q_lens.append(S if kind == "refresh" else s.block_len)
+                q_lens.append(S if (kind == "refresh" or (kind == "mixed" and i in is_ref)) else s.block_len)
                 kv_lens.append(S)
                 rows += s.block_len
         return usec, commits, len(refresh), len(cached), step_work(self.arch, q_lens, kv_lens, rows)
@@ -300,6 +305,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-pass", action="store_true")
+    ap.add_argument("--two-call", action="store_true", help="mixed iterations as dlm_refresh_step + dlm_cached_step instead of one dlm_mixed_step")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -319,7 +325,7 @@ def main():
     peaks = load_peaks()
     K, W = max(1, args.steps), max(3, args.warmup)
 
-    run = Runner(pkg, arch, seed, specs)
+    run = Runner(pkg, arch, seed, specs, mixed_launch=not args.two_call)
     for _ in range(W):
         run.step()
     torch.cuda.synchronize()

@@ -133,6 +133,13 @@ DLM_API int  dlm_refresh_step(dlm_ctx*, const dlm_batch*, dlm_result*);
  * change at every step).  DLM_E_STATE if a request's cache is not valid (new request, block just completed). */
 DLM_API int  dlm_cached_step(dlm_ctx*, const dlm_batch*, const float* per_request_threshold, dlm_result*);
 
+/* Mixed step (P:616-618 batches are sized by their total token count, whatever the kinds):
+ * ONE ragged launch in which every request of the batch takes the step kind that is due -- a recompute step if
+ * its cache is not valid (new request, block just completed), a cache step otherwise.  Results per request are
+ * those of dlm_refresh_step / dlm_cached_step on that request alone (requests are independent, G17); the weights
+ * are streamed once for the whole batch instead of once per kind.  Thresholds as in dlm_cached_step. */
+DLM_API int  dlm_mixed_step(dlm_ctx*, const dlm_batch*, const float* per_request_threshold, dlm_result*);
+
 /* One-time latency profiling: times synthetic refresh and cached steps over a grid of (requests,
  * tokens, K/V length) with CUDA events and fills rows[0..*n_rows).  Uses scratch requests; needs free slots. */
 DLM_API int  dlm_profile_step_costs(dlm_ctx*, dlm_cost_row* rows, int32_t cap, int32_t* n_rows);

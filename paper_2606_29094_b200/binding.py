@@ -21,7 +21,7 @@ DLM_DRY_RUN = 1
 OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM, OPT_PAIR_GEMM, OPT_TC_ATTENTION, OPT_FUSE_ROPE = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
                 "combine_unmask")
-KIND_REFRESH, KIND_CACHED = 0, 1
+KIND_REFRESH, KIND_CACHED, KIND_MIXED = 0, 1, 2
 T_X_IN, T_NORM1, T_Q, T_K, T_V, T_ATTN, T_X_MID, T_NORM2, T_ACT, T_X_OUT, T_FINAL_NORM, T_KCACHE, T_VCACHE = range(13)
 EPI_F32, EPI_BF16, EPI_RESID, EPI_SWIGLU = 0, 1, 2, 3
 
@@ -91,6 +91,7 @@ def lib() -> C.CDLL:
         L.dlm_request_info.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
         L.dlm_refresh_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(_Result)]
         L.dlm_cached_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(f32), C.POINTER(_Result)]
+        L.dlm_mixed_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(f32), C.POINTER(_Result)]
         L.dlm_profile_step_costs.argtypes = [vp, C.POINTER(_CostRow), i32, C.POINTER(i32)]
         L.dlm_set_option.argtypes = [vp, i32, i32]
         L.dlm_kernel_times.argtypes = [vp, C.POINTER(_KernelTime), i32, C.POINTER(i32), i32]
@@ -249,6 +250,8 @@ class Engine:
         L = lib()
         if kind == KIND_REFRESH:
             rc = L.dlm_refresh_step(self._h, C.byref(b), C.byref(res))
+        elif kind == KIND_MIXED:
+            rc = L.dlm_mixed_step(self._h, C.byref(b), None, C.byref(res))
         else:
             rc = L.dlm_cached_step(self._h, C.byref(b), None, C.byref(res))
         self._check(rc)
@@ -262,6 +265,10 @@ class Engine:
 
     def cached_step(self, reqs, thresholds=None, dry_run=False) -> StepResult:
         return self._step(KIND_CACHED, reqs, thresholds, dry_run)
+
+    def mixed_step(self, reqs, thresholds=None, dry_run=False) -> StepResult:
+        """One ragged launch: every request takes the step kind that is due (refresh if its cache is invalid)."""
+        return self._step(KIND_MIXED, reqs, thresholds, dry_run)
 
     # -- misc --
     def set_option(self, key: int, value: int):

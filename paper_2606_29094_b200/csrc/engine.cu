@@ -465,6 +465,7 @@ struct HostBatch {
   int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0;
   std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, tok_bi;
   std::vector<float> tau;
+  std::vector<char> refresh;     // per request: whole sequence recomputed this step
 };
 
 // Per-kernel-class device timing (DLM_OPT_KERNEL_TIMING): an event pair around every launch, resolved after the
@@ -858,7 +859,8 @@ extern "C" int dlm_request_info(dlm_ctx* c, int32_t r, int32_t* cur_block, int32
 // ------------------------------------------------------------------------------------------------
 // One step
 // ------------------------------------------------------------------------------------------------
-static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override, bool refresh, HostBatch& hb) {
+// kind: 0 = cached step, 1 = refresh step, 2 = mixed (each request takes the kind that is due, P:616-618 token-count batching)
+static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override, int kind, HostBatch& hb) {
   const dlm_arch& a = c->a;
   if (!b || b->n <= 0 || !b->req) { set_err(&c->err, "step: empty batch"); return DLM_E_ARG; }
   if (b->n > a.max_requests) { set_err(&c->err, "step: batch of %d exceeds max_requests", b->n); return DLM_E_CAPACITY; }
@@ -872,6 +874,7 @@ static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override
     if (seen[r]) { set_err(&c->err, "step: request %d appears twice in the batch", r); return DLM_E_ARG; }
     seen[r] = 1;
     const bool done = q->cur_block >= q->G / q->B;
+    const bool refresh = kind == 1 || (kind == 2 && !done && !q->cache_valid);
     if (!refresh && !done && !q->cache_valid) {
       set_err(&c->err, "dlm_cached_step: request %d has no valid K/V cache (a refresh step is due)", r);
       return DLM_E_STATE;
@@ -883,7 +886,7 @@ static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override
     float tau = thr_override ? thr_override[i] : (b->threshold ? b->threshold[i] : q->tau);
     hb.slot.push_back(r); hb.q_off.push_back(hb.T); hb.q_len.push_back(qlen); hb.q_pos0.push_back(qpos0);
     hb.kv_len.push_back(q->S); hb.blk_lo.push_back(blk_lo); hb.blk_len.push_back(done ? 0 : q->B);
-    hb.row_off.push_back(hb.R); hb.tau.push_back(tau);
+    hb.row_off.push_back(hb.R); hb.tau.push_back(tau); hb.refresh.push_back(refresh ? 1 : 0);
     for (int t = 0; t < qlen; ++t) hb.tok_bi.push_back(i);
     hb.T += qlen; hb.R += done ? 0 : q->B;
     hb.max_q = std::max(hb.max_q, qlen); hb.max_kv = std::max(hb.max_kv, q->S);
@@ -1160,11 +1163,11 @@ static int enqueue_step(dlm_ctx* c, const HostBatch& hb, bool dry, size_t desc_i
   return DLM_OK;
 }
 
-static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, dlm_result* res, bool refresh) {
+static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, dlm_result* res, int kind) {
   if (!c) return DLM_E_ARG;
   if (!res || !res->n_committed || !res->pos || !res->tok || !res->conf) { set_err(&c->err, "step: result buffers missing"); return DLM_E_ARG; }
   HostBatch hb;
-  int rc = build_batch(c, b, thr_override, refresh, hb);
+  int rc = build_batch(c, b, thr_override, kind, hb);
   if (rc) return rc;
   const dlm_arch& a = c->a;
   const bool dry = (b->flags & DLM_DRY_RUN) != 0;
@@ -1174,7 +1177,7 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   const bool use_graph = c->opt_graph && !c->kprof.on && !c->opt_dump;
   bool launched = false;
   if (use_graph) {
-    GraphKey key = std::make_tuple(refresh ? 1 : 0, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask());
+    GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask());
     GraphEntry& g = c->graphs[key];
     if (g.seen == 1) {                         // second sighting of this batch shape: capture it
       const long long l0 = g_launches;
@@ -1233,7 +1236,7 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
       if (res->row_conf) res->row_conf[i * a.max_block + j] = v ? rconf[i * a.max_block + j] : 0.f;
       if (res->row_tok) res->row_tok[i * a.max_block + j] = v ? rtok[i * a.max_block + j] : -1;
     }
-    if (refresh && hb.blk_len[i]) q.cache_valid = true;      // K/V of all positions now match the pre-step tokens
+    if (hb.refresh[i] && hb.blk_len[i]) q.cache_valid = true;      // K/V of all positions now match the pre-step tokens
     if (!dry && hb.blk_len[i]) {
       q.n_masked -= k; q.n_masked_block -= k;
       if (q.n_masked_block == 0) {                            // P:109 block complete -> recompute before the next block
@@ -1246,12 +1249,13 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   }
   res->total = total;
   c->last_batch = hb;
-  c->last_refresh = refresh;
+  c->last_refresh = kind == 1;
   return DLM_OK;
 }
 
-extern "C" int dlm_refresh_step(dlm_ctx* c, const dlm_batch* b, dlm_result* r) { return run_step(c, b, nullptr, r, true); }
-extern "C" int dlm_cached_step(dlm_ctx* c, const dlm_batch* b, const float* thr, dlm_result* r) { return run_step(c, b, thr, r, false); }
+extern "C" int dlm_refresh_step(dlm_ctx* c, const dlm_batch* b, dlm_result* r) { return run_step(c, b, nullptr, r, 1); }
+extern "C" int dlm_cached_step(dlm_ctx* c, const dlm_batch* b, const float* thr, dlm_result* r) { return run_step(c, b, thr, r, 0); }
+extern "C" int dlm_mixed_step(dlm_ctx* c, const dlm_batch* b, const float* thr, dlm_result* r) { return run_step(c, b, thr, r, 2); }
 
 // ------------------------------------------------------------------------------------------------
 // Debug tensors

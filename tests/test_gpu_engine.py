@@ -169,6 +169,41 @@ def test_batch_independence_ragged():
     eng.close()
 
 
+@pytest.mark.parametrize("bf16_model", [False, True])
+def test_mixed_step_equals_per_kind_calls(bf16_model):
+    """dlm_mixed_step (one ragged launch, every request takes the kind that is due) gives each request what
+    dlm_refresh_step / dlm_cached_step give it alone (requests are independent, G17)."""
+    pkg = _pkg()
+    a = ARCH_C1.replace(weight_dtype=1) if bf16_model else ARCH_C1
+    rng = np.random.default_rng(5)
+    specs = [(random_tokens(rng, P, a.vocab, a.mask_id), G, B, tau) for P, G, B, tau in
+             [(64, 64, 32, 0.9), (17, 32, 16, 0.05), (100, 24, 8, 0.5), (40, 64, 32, 1.5), (200, 32, 32, 0.3)]]
+    eng = pkg.Engine(a, WEIGHT_SEED["C1"], max_requests=5, max_seq=256, max_block=32, max_batch_tokens=640)
+    ids = [eng.add_request(*s) for s in specs]
+    eng.refresh_step([ids[1], ids[3]], dry_run=True)           # requests 1 and 3 now hold a valid cache, 0 / 2 / 4 do not
+    assert [eng.info(i)["cache_valid"] for i in ids] == [False, True, False, True, False]
+    want = [eng.cached_step([i], dry_run=True) if eng.info(i)["cache_valid"] else None for i in ids]
+    want = [w if w is not None else eng.refresh_step([i], dry_run=True) for w, i in zip(want, ids)]
+    # the dry-run refreshes above validated every cache: invalidate 0 / 2 / 4 again by rewriting their tokens
+    for k in (0, 2, 4):
+        eng.set_tokens(ids[k], eng.tokens(ids[k]), keep_cache=False)
+    assert [eng.info(i)["cache_valid"] for i in ids] == [False, True, False, True, False]
+    got = eng.mixed_step(ids, dry_run=True)
+    assert all(eng.info(i)["cache_valid"] for i in ids)         # the refreshed requests now hold a cache
+    for j in range(len(ids)):
+        w = want[j]
+        if bf16_model:      # GEMM tiling differs with the batch's token count: fp32 summation order, not values
+            assert np.allclose(got.lse[j], w.lse[0], rtol=2e-3, atol=2e-3)
+        else:
+            assert got.commits[j] == w.commits[0]
+            assert np.allclose(got.lse[j], w.lse[0], rtol=1e-5, atol=1e-5) and np.array_equal(got.row_tok[j], w.row_tok[0])
+    # cached-only and refresh-only batches through the same entry point, then a real (committing) mixed step
+    eng.mixed_step(ids, dry_run=True)
+    r = eng.mixed_step(ids)
+    assert r.total >= len(ids)
+    eng.close()
+
+
 # ------------------------------------------------------------------------------------------------------------------
 ARCH_C1_BF16 = ARCH_C1.replace(weight_dtype=1)
 
