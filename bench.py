@@ -435,7 +435,14 @@ def kernel_pass(run, pkg, arch, peaks, n_steps=24):
     else:
         ach = flops / (g_launch / n_cached) / per_launch_s * 1e-12
         rf = {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"]}
-    rf.update({"traffic": None, "kernel": "gemm_tc_kernel (QKV, O, gate/up+SwiGLU, down, LM-head epilogues) inside cached steps",
+    # dram__bytes_read + dram__bytes_write per launch, from the committed ncu --set full capture of this workload
+    # (profiles/r01_ncu_kernels.md: 15.38 GB over the 129 GEMM launches of a C2 cached step); other workloads: not captured
+    traffic = 119.2e6 if (T == 32 and arch.n_layers == 32 and arch.d_model == 4096) else None
+    big = T > 128
+    rf.update({"traffic": traffic, "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_kernels.md)",
+               "algorithmic_bytes_per_launch": w_bytes / (g_launch / n_cached),
+               "kernel": ("gemm_pair_kernel (CTA-pair tcgen05 GEMM: QKV+RoPE, O, gate/up+SwiGLU, down, LM head)" if big else
+                          "gemm_skinny_kernel (QKV, O, gate/up+SwiGLU, down) + gemm_tc_kernel<LM head>: the weight-streaming GEMMs") + " inside cached steps",
                "launches_per_step": g_launch / n_cached, "avg_launch_us": per_launch_s * 1e6, "share_of_step": g_us / tot,
                "algorithmic": f"weights streamed once per step ({w_bytes * 1e-9:.2f} GB bf16) / GEMM launches; tokens per step T={T}",
                "peak_source": peaks["source"], "steps_sampled": n_cached})

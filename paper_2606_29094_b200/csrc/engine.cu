@@ -286,7 +286,7 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   const int q_tiles = (bd.max_q_len * r + kTaTile - 1) / kTaTile;
   const long long items = (long long)bd.n * g.n_kv_heads * q_tiles;
   const int kv_tiles = (bd.max_kv_len + kTaTile - 1) / kTaTile;
-  if (!force && items * kv_tiles < 4LL * g_num_sms) return 0;       // too little work for one-CTA-per-SM tiles of 128 x 128
+  if (!force && items < 64) return 0;       // too few (request, head, query tile) items to fill the SMs with one CTA each
   const long long rows = (long long)n_layers_total * g.n_pages * 2 * g.n_kv_heads * g.page_tokens;
   if (rows >= (1LL << 31)) return 0;
   int splits = 1;
