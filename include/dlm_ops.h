@@ -63,7 +63,8 @@ DLM_API int dlm_op_lmhead_unmask_bf16(const void* hidden, const void* W_lm, int3
 
 /* Non-causal block attention over a contiguous (unpaged) K/V, bf16 (a5): q [Tq, H, d_h], k/v [S, H_kv, d_h]
  * -> out [Tq, H, d_h]; softmax_j(q.k_j/sqrt(d_h)) v_j over all j.  flash = 0: plain kernel; 1: mma.sync
- * online-softmax kernel; 2: tcgen05/TMEM kernel with the K/V split the engine would pick; 2 + s: the same with s K/V splits. */
+ * online-softmax kernel; 2: tcgen05/TMEM kernel with the K/V split the engine would pick (the transposed-score variant when Tq * H / H_kv <= 64); 2 + s: the same
+ * with s K/V splits; 102 / 102 + s: the row-major tcgen05 kernel even when the transposed one fits. */
 DLM_API int dlm_op_attention_bf16(const void* q, const void* k, const void* v, void* out, int32_t Tq, int32_t S,
                           int32_t H, int32_t H_kv, int32_t d_h, int32_t flash, void* stream);
 

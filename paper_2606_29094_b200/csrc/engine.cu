@@ -18,6 +18,7 @@
 #include "../../include/dlm_ops.h"
 #include "attn_flash.cuh"
 #include "attn_tc.cuh"
+#include "attn_tct.cuh"
 #include "common.cuh"
 #include "gemm_skinny.cuh"
 #include "gemm_pair.cuh"
@@ -286,6 +287,8 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   const int q_tiles = (bd.max_q_len * r + kTaTile - 1) / kTaTile;
   const long long items = (long long)bd.n * g.n_kv_heads * q_tiles;
   const int kv_tiles = (bd.max_kv_len + kTaTile - 1) / kTaTile;
+  const bool no_transposed = force >= 100;      // test hook: 100 + f = attn_tc_kernel even when the transposed kernel fits
+  if (no_transposed) force -= 100;
   if (!force && items < 64) return 0;       // too few (request, head, query tile) items to fill the SMs with one CTA each
   const long long rows = (long long)n_layers_total * g.n_pages * 2 * g.n_kv_heads * g.page_tokens;
   if (rows >= (1LL << 31)) return 0;
@@ -294,16 +297,21 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
     long long best = -1;
     for (int s = 1; s <= std::min(8, kv_tiles); ++s) {
       const long long waves = (items * s + g_num_sms - 1) / g_num_sms;
-      const long long cost = waves * ((kv_tiles + s - 1) / s + 1);
+      const long long cost = waves * ((kv_tiles + s - 1) / s + 3);      // + per-item ramp, epilogue and combine share (measured: ~3 tiles)
       if (best < 0 || cost < best) { best = cost; splits = s; }
     }
     if (force > 1) splits = std::min(force - 1, kv_tiles);
   }
+  // stacked rows <= 64 (cached steps of MHA models): the transposed-score kernel shares the exponentials over all four
+  // sub-partitions; force: 0 engine choice, 1 = forced with the split the engine would pick, 1 + s = forced with s splits
+  const bool fits_t = bd.max_q_len * r <= kTtNQ;
+  const bool transposed = fits_t && !no_transposed;
   const CUtensorMap* mkv = tc.get(kv_store, rows, 128, 64);
   if (!mkv) { set_err(err, "cuTensorMapEncodeTiled failed (attention K/V store %p, %lld rows)", (const void*)kv_store, rows); return DLM_E_CUDA; }
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTaSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(attn_tct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTtSmem);
     if (e != cudaSuccess) { set_err(err, "attn_tc: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
     configured = true;
   }
@@ -319,7 +327,9 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
     p.ws_o = *ws;
     p.ws_ml = *ws + (size_t)splits * TH * 128;
   }
-  cudaError_t e = launch_k(attn_tc_kernel, dim3((unsigned)std::min<long long>(g_num_sms, p.n_items)), dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
+  const dim3 grid((unsigned)std::min<long long>(g_num_sms, p.n_items));
+  cudaError_t e = transposed ? launch_k(attn_tct_kernel, grid, dim3(kTaThreads), (size_t)kTtSmem, st, pdl, *mkv, p)
+                             : launch_k(attn_tc_kernel, grid, dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
   if (splits > 1 && e == cudaSuccess)
     e = launch_k(attn_combine_kernel, dim3((unsigned)TH), dim3(kFaDh), 0, st, pdl, out, (const float*)p.ws_o, (const float*)p.ws_ml, TH, splits);
   if (e != cudaSuccess) { set_err(err, "attn_tc launch: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
@@ -426,7 +436,7 @@ static int attn_op_contiguous(const void* q, const void* k, const void* v, void*
   if (flash >= 2) {
     static TmapCache op_maps;
     op_maps.m.clear();
-    rc = attn_tc_launch(op_maps, (bf16*)out, (const bf16*)q, store, 1, meta, bd, g, 0, H, scale, &ws, &wsb, st, false, err, &done, flash - 1);
+    rc = attn_tc_launch(op_maps, (bf16*)out, (const bf16*)q, store, 1, meta, bd, g, 0, H, scale, &ws, &wsb, st, false, err, &done, flash >= 102 ? 100 + (flash - 101) : flash - 1);
     if (!rc && !done) { set_err(err, "dlm_op_attention_bf16: tcgen05 kernel does not support d_h=%d", dh); rc = DLM_E_ARG; }
   } else if (flash) {
     rc = attn_flash_launch((bf16*)out, (const bf16*)q, store, meta, bd, g, 0, H, scale, &ws, &wsb, g_num_sms, st, false, err, &done);

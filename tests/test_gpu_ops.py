@@ -248,11 +248,12 @@ def test_attention(Tq, S, H, Hkv, flash):
 
 
 @pytest.mark.parametrize("Tq,S,H,Hkv", [(32, 512, 4, 4), (64, 200, 8, 2), (5, 64, 2, 1), (100, 1000, 7, 1), (512, 512, 2, 2),
-                                        (32, 4608, 2, 2), (300, 300, 4, 2), (64, 129, 1, 1)])
-@pytest.mark.parametrize("mode", [2, 3, 5])
+                                        (32, 4608, 2, 2), (300, 300, 4, 2), (64, 129, 1, 1), (9, 700, 14, 2), (33, 1000, 3, 3)])
+@pytest.mark.parametrize("mode", [2, 3, 5, 102, 104])
 def test_attention_tcgen05(Tq, S, H, Hkv, mode):
-    """tcgen05/TMEM attention (128-row query tiles, 128-token K/V tiles, lazy rescale, optional K/V split) vs
-    oracle.attention (fp64): ragged tails in rows and K/V, GQA stacking, several tiles per item."""
+    """tcgen05/TMEM attention vs oracle.attention (fp64): ragged tails in rows and K/V, GQA stacking, several tiles per
+    item, optional K/V split.  Modes 2.. take the transposed-score kernel when Tq * H / H_kv <= 64 and the row-major
+    kernel (128-row query tiles, lazy rescale) otherwise; modes 102.. force the row-major kernel."""
     import paper_2606_29094_b200 as pkg
     rng = np.random.default_rng(Tq + S + H + mode)
     dh = 128
@@ -273,11 +274,11 @@ def test_attention_tcgen05_growing_scores():
     Tq, S, H, dh = 40, 1024, 2, 128
     qn = rng.standard_normal((Tq, H, dh)).astype(np.float32)
     kn = rng.standard_normal((S, H, dh)).astype(np.float32) * 0.3
-    kn += (np.arange(S, dtype=np.float32)[:, None, None] / S) * 1.2 * np.sign(qn[0:1, :, :])   # drift along q[0]
+    kn += (np.arange(S, dtype=np.float32)[:, None, None] / S) * 2.5 * np.sign(qn[0:1, :, :])   # drift along q[0]
     q, k = _bf16(qn).cuda(), _bf16(kn).cuda()
     v = _bf16(rng.standard_normal((S, H, dh)).astype(np.float32)).cuda()
     want = omodel.attention(_f64(q), _f64(k), _f64(v))
-    for mode in (2, 3):
+    for mode in (2, 3, 102, 103):        # transposed-score kernel (exact-maxima pass) and row-major kernel (lazy rescale)
         got = _f64(pkg.op_attention_bf16(q, k, v, mode))
         assert np.isfinite(got).all()
         assert np.abs(got - want).max() < 8e-3
