@@ -295,6 +295,22 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+def reduce_over_ranks(dist, device, dev_us, wall, commits, launches):
+    """Replicas-only scaling: every rank runs its own replica of the workload with no data-path
+    collective; the job's time is the MAX over ranks (device and wall clock), its commits and launches the SUM."""
+    import torch
+    t = torch.tensor([dev_us, wall], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([commits, launches], device=device, dtype=torch.float64)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), int(c[0]), int(c[1])
+
+
+def job_value(world, steps, dev_us):
+    """Whole-job steps/s of `world` replicas that each ran `steps` steps, timed as the slowest rank."""
+    return world * steps / (dev_us * 1e-6)
+
+
 # ---------------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -349,14 +365,9 @@ def main():
         wall = time.perf_counter() - t0
     launches = run.eng.launch_count() - launches0
     if dist:
-        t = torch.tensor([dev_us, wall], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_us, wall = float(t[0]), float(t[1])
-        c = torch.tensor([commits, launches], device="cuda", dtype=torch.float64)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        commits, launches = int(c[0]), int(c[1])
+        dev_us, wall, commits, launches = reduce_over_ranks(dist, "cuda", dev_us, wall, commits, launches)
     n_req = len(specs)
-    value = world * K / (dev_us * 1e-6)
+    value = job_value(world, K, dev_us)
     out = {"metric": "denoise_steps_per_s", "value": value, "unit": "steps/s", "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": dev_us / K * 1e-3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
            "data": "synthetic",
