@@ -295,6 +295,73 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+def run_lmhead_micro(args):
+    """BASELINE.json configs[4]: isolated micro-benchmark of the fused LM-head + softmax-max + argmax + unmask path on
+    unit-RMS random hidden states [2048, 3584] (64 requests x 32 block rows) against the Qwen-shape vocabulary matrix
+    [152064, 3584]: rows a11-a13 only, logits never written.  One JSON line (not the headline metric)."""
+    import torch
+    import paper_2606_29094_b200 as pkg
+    from synth_inputs import unit_rms_hidden
+    peaks = load_peaks()
+    a = ARCH_QWEN7B
+    n, B = 64, 32
+    R, K, V = n * B, a.d_model, a.vocab
+    hidden = torch.from_numpy(unit_rms_hidden(2005, R, K)).to(torch.bfloat16).cuda()
+    g = torch.Generator(device="cuda").manual_seed(WEIGHT_SEED["C5"])
+    W = (torch.randn(V, K, device="cuda", generator=g) * a.init_std).to(torch.bfloat16)
+    tau = torch.full((n,), 0.9, device="cuda")
+    tokens0 = torch.full((n, B), a.mask_id, dtype=torch.int32, device="cuda")
+    scratch = torch.empty(pkg.lib().dlm_op_lmhead_scratch_bytes(R, V), device="cuda", dtype=torch.uint8)
+    outs = (torch.empty(n, device="cuda", dtype=torch.int32), torch.empty(R, device="cuda", dtype=torch.int32),
+            torch.empty(R, device="cuda", dtype=torch.int32), torch.empty(R, device="cuda", dtype=torch.float32))
+    K_steps, Wm = max(1, args.steps), max(3, args.warmup)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K_steps)]
+    committed = 0
+    with ClockSampler(0) as clk:
+        for i in range(Wm + K_steps):
+            tio = tokens0.clone()
+            if i >= Wm:
+                ev[2 * (i - Wm)].record()
+            pkg.op_lmhead_unmask_bf16(hidden, W, n, B, a.logit_scale, a.mask_id, tau, tio, scratch=scratch, outs=outs)
+            if i >= Wm:
+                ev[2 * (i - Wm) + 1].record()
+        torch.cuda.synchronize()
+        committed = int(outs[0].sum().item())
+    ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(K_steps)]
+    t = float(np.mean(ms)) * 1e-3
+    flops = 2.0 * R * K * V
+    ach = flops / t * 1e-12
+    out = {"metric": "lmhead_unmask_micro_tflops", "value": ach, "unit": "TFLOP/s", "n_gpus": 1, "steps": K_steps, "warmup": Wm, "ms_per_step": t * 1e3,
+           "higher_is_better": True, "dtype": "bf16", "data": "synthetic",
+           "config": {"workload": "C5 micro: fused LM head + split-vocab (max, sum-exp, argmax) + combine + threshold unmask, hidden [2048, 3584] x W [152064, 3584], 64 requests x 32 rows, tau 0.9",
+                      "l2": "the vocabulary matrix (1.09 GB) is larger than L2", "timing": "CUDA events around the C-ABI op (includes its 1 KB descriptor copy)"},
+           "roofline": {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops"], "traffic": None,
+                        "kernel": "gemm_pair_kernel<LM head> + combine_unmask_kernel", "peak_source": peaks["source"] + " (burst: kernel timed alone)"},
+           "logits_bytes_avoided": R * V * 4 * 2, "logits_time_avoided_ms_at_hbm_peak": R * V * 4 * 2 / (peaks["hbm_gbs"] * 1e9) * 1e3,
+           "committed_rows": committed, "clocks": clk.summary()}
+    print(json.dumps(out), flush=True)
+
+
+def run_cost_table(args):
+    """a15: dlm_profile_step_costs on the workload's architecture -- the per-step cost table the paper's scheduler
+    consumes (LP[tp][tokens]), split by step kind, with the K/V length added; plus the per-token
+    costs alpha (refresh) and beta (cached) of P:349."""
+    import torch
+    import paper_2606_29094_b200 as pkg
+    arch, seed, specs, desc = get_workload(args.workload)
+    eng = pkg.Engine(arch, seed, max_requests=64, max_seq=4608, max_block=32, max_batch_tokens=32768)
+    rows = eng.profile_step_costs(cap=256)
+    eng.close()
+    table = [{"kind": r["kind"], "n": r["n_requests"], "tokens": r["n_tokens"], "kv": r["kv_tokens"], "usec": round(r["usec"], 1)} for r in rows]
+    ref = [r for r in table if r["kind"] == "refresh"]
+    cac = [r for r in table if r["kind"] == "cached"]
+    out = {"metric": "step_cost_table", "unit": "usec", "data": "synthetic", "config": {"workload": f"{args.workload} architecture: {desc}"},
+           "rows": table,
+           "alpha_usec_per_token_refresh": round(float(np.median([r["usec"] / r["tokens"] for r in ref])), 3) if ref else None,
+           "beta_usec_per_token_cached": round(float(np.median([r["usec"] / r["tokens"] for r in cac])), 3) if cac else None}
+    print(json.dumps(out), flush=True)
+
+
 def reduce_over_ranks(dist, device, dev_us, wall, commits, launches):
     """Replicas-only scaling: every rank runs its own replica of the workload with no data-path
     collective; the job's time is the MAX over ranks (device and wall clock), its commits and launches the SUM."""
@@ -321,10 +388,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-pass", action="store_true")
+    ap.add_argument("--micro", default=None, choices=["lmhead"], help="isolated micro-benchmark instead of the step benchmark")
+    ap.add_argument("--cost-table", action="store_true", help="print dlm_profile_step_costs for the workload's architecture")
     ap.add_argument("--two-call", action="store_true", help="mixed iterations as dlm_refresh_step + dlm_cached_step instead of one dlm_mixed_step")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.micro == "lmhead":
+        return run_lmhead_micro(args)
+    if args.cost_table:
+        return run_cost_table(args)
 
     import torch
     rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))

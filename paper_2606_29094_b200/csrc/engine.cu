@@ -1488,7 +1488,7 @@ extern "C" int64_t dlm_op_lmhead_scratch_bytes(int32_t R, int32_t V) {
 static int op_head(const void* hidden, const void* Wlm, int n, int B, int V, int K, float scale, int mask_id, const float* tau,
                    int* tokens_io, StepOut so, void* scratch, cudaStream_t st, int dry) {
   const int R = n * B;
-  const int n_tiles = (V + 127) / 128;
+  int n_tiles = (V + 127) / 128;
   RowPartial* part = (RowPartial*)scratch;
   int* meta = (int*)((char*)scratch + (size_t)R * n_tiles * sizeof(RowPartial));
   // meta: slot[n], blk_lo[n], blk_len[n], row_off[n]  (+ tau passed separately)
@@ -1496,10 +1496,18 @@ static int op_head(const void* hidden, const void* Wlm, int n, int B, int V, int
   for (int i = 0; i < n; ++i) { h[i] = i; h[n + i] = 0; h[2 * n + i] = B; h[3 * n + i] = i * B; }
   cudaMemcpyAsync(meta, h.data(), h.size() * 4, cudaMemcpyHostToDevice, st);
   cudaStreamSynchronize(st);   // h is a stack-lifetime staging buffer
-  GemmTcParams p = {};
-  p.part = part; p.n_tiles = n_tiles; p.mask_id = mask_id; p.scale = scale;
   g_op_tmaps.m.clear();
-  int rc = gemm_tc(g_op_tmaps, &g_init_error, hidden, R, Wlm, V, R, V, K, EPI_LMHEAD, 128, p, st);
+  int rc;
+  if (R > 128) {                 // as in the engine: the CTA-pair kernel with 256-wide vocabulary tiles above 128 rows
+    n_tiles = (V + 255) / 256;
+    GemmPairParams p = {};
+    p.part = part; p.n_tiles = n_tiles; p.mask_id = mask_id; p.scale = scale;
+    rc = gemm_pair(g_op_tmaps, &g_init_error, hidden, R, Wlm, V, R, V, K, EPI_LMHEAD, 256, p, st);
+  } else {
+    GemmTcParams p = {};
+    p.part = part; p.n_tiles = n_tiles; p.mask_id = mask_id; p.scale = scale;
+    rc = gemm_tc(g_op_tmaps, &g_init_error, hidden, R, Wlm, V, R, V, K, EPI_LMHEAD, 128, p, st);
+  }
   if (rc) return rc;
   BatchDesc bd = {};
   bd.n = n; bd.R = R; bd.slot = meta; bd.blk_lo = meta + n; bd.blk_len = meta + 2 * n; bd.row_off = meta + 3 * n; bd.tau = tau;
