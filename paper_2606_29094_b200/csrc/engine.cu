@@ -579,6 +579,17 @@ struct KScope {
 
 static int norm_threads(int d) { return std::min(1024, ((d / 4) + 31) / 32 * 32); }
 
+// a2 / a7 / a10: latency kernel (one block per row) for small steps, warp-per-row throughput kernel from 1024 rows on.
+// Same arithmetic per row up to the order of the sum of squares.
+template <typename TE>
+static void launch_rmsnorm(dlm_ctx* c, TE* u, float* x, const int* row_src, int rows, int d, float eps, const float* part, int n_part,
+                           long long part_stride, bool pdl) {
+  if (rows >= 1024)
+    launch_k(rmsnorm_rows_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride);
+  else
+    launch_k(rmsnorm_kernel<TE>, dim3(rows), dim3(norm_threads(d)), 0, c->st, pdl, u, x, row_src, d, eps, part, n_part, part_stride);
+}
+
 static int nqkv(const dlm_arch& a) { return (a.n_heads + 2 * a.n_kv_heads) * a.head_dim; }
 
 // ------------------------------------------------------------------------------------------------
@@ -1005,7 +1016,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     dump_stage(c, l, DLM_T_X_IN, c->x, (size_t)d * 4, T);
     {
       KScope ks(c, DLM_K_RMSNORM);
-      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(norm_threads(d)), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      launch_rmsnorm<TE>(c, (TE*)c->u, c->x, (const int*)nullptr, T, d, a.rms_eps, (const float*)c->part_x, pend, pstride, pdl);
       pend = 0;
     }
     dump_stage(c, l, DLM_T_NORM1, c->u, (size_t)d * sizeof(TE), T);
@@ -1075,7 +1086,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     dump_stage(c, l, DLM_T_X_MID, c->x, (size_t)d * 4, T);
     {
       KScope ks(c, DLM_K_RMSNORM);
-      launch_k(rmsnorm_kernel<TE>, dim3(T), dim3(norm_threads(d)), 0, st, pdl, (TE*)c->u, c->x, (const int*)nullptr, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      launch_rmsnorm<TE>(c, (TE*)c->u, c->x, (const int*)nullptr, T, d, a.rms_eps, (const float*)c->part_x, pend, pstride, pdl);
       pend = 0;
     }
     dump_stage(c, l, DLM_T_NORM2, c->u, (size_t)d * sizeof(TE), T);
@@ -1126,7 +1137,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     {
       KScope ks(c, DLM_K_RMSNORM);
       launch_k(build_row_src_kernel, dim3(bd.n), dim3(64), 0, st, pdl, c->row_src, bd);
-      launch_k(rmsnorm_kernel<TE>, dim3(R), dim3(norm_threads(d)), 0, st, pdl, (TE*)c->hf, c->x, (const int*)c->row_src, d, a.rms_eps, (const float*)c->part_x, pend, pstride);
+      launch_rmsnorm<TE>(c, (TE*)c->hf, c->x, (const int*)c->row_src, R, d, a.rms_eps, (const float*)c->part_x, pend, pstride, pdl);
       pend = 0;
     }
     dump_stage(c, 0, DLM_T_FINAL_NORM, c->hf, (size_t)d * sizeof(TE), R);

@@ -141,6 +141,53 @@ __global__ void __launch_bounds__(1024) rmsnorm_kernel(TA* __restrict__ u, float
   }
 }
 
+// Throughput variant for large token counts (T >= 1024): one WARP per row, no block barrier, two passes (sum of
+// squares while folding the split-K slices into x; then re-read x -- an L2 hit -- scale and round).  At 512..36 864 rows the
+// one-block-per-row kernel above is latency-bound (~0.7 TB/s at 2048 rows); this one keeps up to 64 rows per SM in flight.
+template <typename TA>
+__global__ void __launch_bounds__(512) rmsnorm_rows_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
+                                                           int n_rows, int d, float eps, const float* __restrict__ part, int n_part,
+                                                           long long part_stride) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (r >= n_rows) return;
+  const int lane = threadIdx.x & 31;
+  const long long sr = row_src ? row_src[r] : r;
+  float4* xr = reinterpret_cast<float4*>(x + sr * d);
+  const int nvec = d >> 2;
+  const long long ps4 = part_stride >> 2;
+  float ss = 0.f;
+#pragma unroll 4
+  for (int i = lane; i < nvec; i += 32) {
+    float4 a = xr[i];
+    if (n_part > 0) {
+      const float4* pr = reinterpret_cast<const float4*>(part + sr * d) + i;
+      for (int s = 0; s < n_part; ++s) {
+        const float4 q = __ldcg(pr + s * ps4);
+        a.x += q.x; a.y += q.y; a.z += q.z; a.w += q.w;
+      }
+      xr[i] = a;
+    }
+    ss += a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w;
+  }
+  ss = warp_sum(ss);
+  const float rs = rsqrtf(ss / (float)d + eps);
+  TA* ur = u + (long long)r * d;
+#pragma unroll 4
+  for (int i = lane; i < nvec; i += 32) {
+    const float4 a = xr[i];
+    if (sizeof(TA) == 2) {
+      __nv_bfloat162 lo = __floats2bfloat162_rn(a.x * rs, a.y * rs), hi = __floats2bfloat162_rn(a.z * rs, a.w * rs);
+      uint2 w;
+      w.x = *reinterpret_cast<uint32_t*>(&lo); w.y = *reinterpret_cast<uint32_t*>(&hi);
+      *reinterpret_cast<uint2*>(reinterpret_cast<bf16*>(ur) + 4 * i) = w;
+    } else {
+      *reinterpret_cast<float4*>(reinterpret_cast<float*>(ur) + 4 * i) = make_float4(a.x * rs, a.y * rs, a.z * rs, a.w * rs);
+    }
+  }
+}
+
 // x[row] += sum of split-K partials (debug-dump mode only: makes x complete right after the projection)
 __global__ void add_partials_kernel(float* __restrict__ x, const float* __restrict__ part, int n_part, long long part_stride, long long n) {
   pdl_launch_dependents();
