@@ -61,6 +61,9 @@ class Request:
         assert len(self.tokens) == self.S
         self.cache = None            # per layer (K, V) float64, valid from a refresh until the block completes
         self.cache_valid = False
+        # Step Predictor inputs ("confidence statistics ... tracked by the Scheduler", App. A; reading G22):
+        self.conf_state = np.zeros(self.G, dtype=np.float64)   # per output position: last confidence seen while masked
+        self.steps_done = 0                                    # completed (non-dry) denoising steps
 
     def masked(self) -> np.ndarray:
         return self.tokens == self.arch.mask_id
@@ -100,6 +103,10 @@ def unmask(tokens: np.ndarray, lo: int, hi: int, tok: np.ndarray, conf: np.ndarr
 def _finish(req: Request, b: int, hidden: np.ndarray, tau: float, dry_run: bool, kind: str, wts) -> StepResult:
     lo, hi = req.block_range(b)
     tok, conf, lse, margin = model.head(req.arch, wts, hidden)
+    if not dry_run:
+        was_masked = req.tokens[lo:hi] == req.arch.mask_id   # G22: live while masked, frozen at commit
+        req.conf_state[lo - req.P:hi - req.P][was_masked] = conf[was_masked]
+        req.steps_done += 1
     commits = unmask(req.tokens, lo, hi, tok, conf, tau, req.arch.mask_id, dry_run)
     if not dry_run and not (req.tokens[lo:hi] == req.arch.mask_id).any():
         req.cache_valid = False          # P:109 recompute "after the current block is fully unmasked"
@@ -135,6 +142,43 @@ def cached_step(req: Request, wts, tau: Optional[float] = None, dry_run: bool = 
             req.cache[l][0][lo:hi] = k
             req.cache[l][1][lo:hi] = v
     return _finish(req, b, hidden, tau, dry_run, "cached", wts)
+
+
+FEATURE_NAMES = ("confidence_threshold", "output_length", "full_progress", "full_unmask_progress", "block_progress",
+                 "block_unmask_progress", "output_min_confidence", "output_q25_confidence", "output_median_confidence",
+                 "output_avg_confidence", "output_q75_confidence")
+
+
+def quantile_linear(sorted_vals: np.ndarray, q: float) -> float:
+    """q-quantile of ascending values by linear interpolation between order statistics: h = (n - 1) q,
+    v = s[floor h] + (h - floor h) (s[floor h + 1] - s[floor h])."""
+    n = len(sorted_vals)
+    h = (n - 1) * q
+    lo = int(np.floor(h))
+    hi = min(lo + 1, n - 1)
+    return float(sorted_vals[lo] + (h - lo) * (sorted_vals[hi] - sorted_vals[lo]))
+
+
+def predictor_features(req: Request, tau: Optional[float] = None) -> np.ndarray:
+    """The Step Predictor's 11 scalar features of a request in its current state (App. A), in the
+    paper's order (FEATURE_NAMES).  Reading G22: an output token's confidence is the softmax confidence the
+    model last gave its position while it was still masked (so it is frozen when the token is committed), 0
+    for positions no step has evaluated yet; quartiles by linear interpolation; a finished request reports
+    block_progress = block_unmask_progress = 1."""
+    tau = req.threshold if tau is None else float(tau)
+    G, B = req.G, req.B
+    n_blocks = G // B
+    b = req.current_block()
+    masked = req.masked()[req.P:]
+    if b is None:
+        block_progress, block_unmask = 1.0, 1.0
+    else:
+        block_progress = b / n_blocks
+        block_unmask = float((~masked[b * B:(b + 1) * B]).sum()) / B
+    s = np.sort(req.conf_state)
+    return np.array([tau, G, req.steps_done / G, float((~masked).sum()) / G, block_progress, block_unmask,
+                     s[0], quantile_linear(s, 0.25), quantile_linear(s, 0.5), float(req.conf_state.sum() / G), quantile_linear(s, 0.75)],
+                    dtype=np.float64)
 
 
 def next_step(req: Request, wts, tau: Optional[float] = None, use_cache: bool = True) -> Optional[StepResult]:

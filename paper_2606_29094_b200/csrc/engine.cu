@@ -703,7 +703,7 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   ALLOC(c->x, (size_t)c->Tmax * d * 4);
   // fp32 slice capacity (rows): split-K slices of the skinny path (<= 16 x 128 tokens) and of the pair path (<= 4 x M)
   c->qkv_rows = std::max<long long>(std::max<long long>(c->Tmax, (long long)kSkMaxSplits * kSkMaxTokens), std::min<long long>(3LL * c->Tmax, 4096));
-  c->part_rows = std::max<long long>((long long)kSkMaxSplits * kSkMaxTokens, std::min<long long>(4LL * c->Tmax, 4096));
+  c->part_rows = std::max<long long>((long long)kSkMaxSplits * kSkMaxTokens, std::min<long long>(4LL * c->Tmax, 8192));
   ALLOC(c->qkv, (size_t)c->qkv_rows * NQKV * 4);
   if (c->bf16_model) ALLOC(c->part_x, (size_t)c->part_rows * d * 4);
   ALLOC(c->u, (size_t)c->Tmax * d * es);

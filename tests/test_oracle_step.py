@@ -149,3 +149,53 @@ def test_brute_force_twin_trajectories(tau, use_cache):
     toks, bh = brute.run(arch, wts, prompt, 8, 4, tau, use_cache)
     assert [[(c.pos, c.tok) for c in h.commits] for h in hist] == bh
     assert r.tokens.tolist() == toks
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Step Predictor features (App. A; reading G22)
+# ------------------------------------------------------------------------------------------------------------------
+def test_quantile_linear_matches_library_and_hand_cases():
+    """Special cases with a textbook answer + the library routine on random data (numpy's default is the same
+    linear interpolation between order statistics)."""
+    assert step.quantile_linear(np.array([0.0, 1.0]), 0.25) == 0.25
+    assert step.quantile_linear(np.array([1.0, 2.0, 3.0, 4.0, 5.0]), 0.5) == 3.0
+    assert step.quantile_linear(np.array([1.0, 2.0, 3.0, 4.0]), 0.75) == 3.25      # h = 2.25
+    assert step.quantile_linear(np.array([7.0]), 0.25) == 7.0
+    rng = np.random.default_rng(3)
+    for n in (2, 5, 32, 256, 257):
+        v = np.sort(rng.random(n))
+        for q in (0.25, 0.5, 0.75):
+            assert abs(step.quantile_linear(v, q) - np.quantile(v, q)) < 1e-15
+
+
+def test_predictor_features_invariants_and_closed_forms(tiny_arch):
+    """Fresh request: progress 0, confidences 0.  tau > 1: one commit per step, so after k steps
+    full_progress = full_unmask_progress = k / G and block_unmask_progress = (k mod B) / B.  Committed
+    positions keep their confidence (frozen), min <= q25 <= median <= q75, avg within [min, max]."""
+    arch, wts = tiny_arch, W.Weights(tiny_arch, 47)
+    prompt = random_tokens(np.random.default_rng(9), 10, arch.vocab, arch.mask_id)
+    req = step.Request(arch, prompt, 16, 8, 1.5)
+    f0 = step.predictor_features(req)
+    assert list(f0[:2]) == [1.5, 16] and not f0[2:].any()
+    frozen = {}
+    for k in range(1, 17):
+        r = step.next_step(req, wts)
+        assert len(r.commits) == 1
+        f = step.predictor_features(req, tau=0.7)
+        assert f[0] == 0.7 and f[1] == 16
+        assert f[2] == k / 16 and f[3] == k / 16
+        if k < 16:
+            assert f[4] == (k // 8) / 2 and f[5] == (k % 8) / 8
+        else:
+            assert f[4] == 1.0 and f[5] == 1.0
+        assert f[6] <= f[7] <= f[8] <= f[10] <= req.conf_state.max() and f[6] <= f[9] <= req.conf_state.max()
+        c = r.commits[0]
+        frozen[c.pos] = c.conf
+        for pos, v in frozen.items():                 # frozen at commit, never touched again
+            assert req.conf_state[pos - req.P] == v
+        if k <= 8:                                    # the second block has not been evaluated yet
+            assert not req.conf_state[8:].any()
+    # a dry-run step leaves the predictor state alone
+    req2 = step.Request(arch, prompt, 16, 8, 0.5)
+    step.refresh_step(req2, wts, dry_run=True)
+    assert req2.steps_done == 0 and not req2.conf_state.any()
