@@ -92,7 +92,14 @@ typedef struct {
   float*   lse;                  /* [n*max_block] out, may be NULL: log-sum-exp of each block row       */
   float*   row_conf;             /* [n*max_block] out, may be NULL: confidence of each block row        */
   int32_t* row_tok;              /* [n*max_block] out, may be NULL: predicted token of each block row   */
+  float*   features;             /* [n*DLM_N_FEATURES] out, may be NULL: the Step Predictor's features of each request after
+                                    this step ("confidence statistics", App. A), in the paper's order:
+                                    confidence_threshold, output_length, full_progress, full_unmask_progress, block_progress,
+                                    block_unmask_progress, output_{min, q25, median, avg, q75}_confidence.  An output token's
+                                    confidence is the one its position last had while masked (frozen at commit, 0 before any
+                                    step evaluated it); quartiles by linear interpolation; computed on the device.            */
 } dlm_result;
+#define DLM_N_FEATURES 11
 
 #define DLM_KIND_REFRESH 0
 #define DLM_KIND_CACHED  1

@@ -3,7 +3,7 @@
 The product is libdlm.so (CUDA for sm_100a behind the C ABI of include/dlm.h); this package is its thin
 ctypes binding.  Nothing here falls back to a CPU implementation.
 """
-from .binding import (DLM_DRY_RUN, EPI_BF16, EPI_F32, EPI_RESID, EPI_SWIGLU, KIND_CACHED, KIND_MIXED, KIND_REFRESH, LIB_PATH,  # noqa: F401
+from .binding import (DLM_DRY_RUN, EPI_BF16, EPI_F32, EPI_RESID, EPI_SWIGLU, FEATURE_NAMES, KIND_CACHED, KIND_MIXED, KIND_REFRESH, LIB_PATH,  # noqa: F401
                       OPT_CUDA_GRAPH, OPT_DEBUG_DUMP, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SIMPLE_KERNELS, OPT_SKINNY_GEMM, OPT_PAIR_GEMM, OPT_TC_ATTENTION, OPT_FUSE_ROPE, DlmError, Engine,
                       StepResult, exported_symbols, lib, op_attention_bf16, op_gemm_bf16, op_gemm_pair_bf16, op_gemm_plain_bf16, op_gemm_skinny_bf16,
                       op_lmhead_bf16, op_lmhead_unmask_bf16)

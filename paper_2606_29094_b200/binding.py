@@ -22,6 +22,9 @@ OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KER
 KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
                 "combine_unmask")
 KIND_REFRESH, KIND_CACHED, KIND_MIXED = 0, 1, 2
+N_FEATURES = 11
+FEATURE_NAMES = ("confidence_threshold", "output_length", "full_progress", "full_unmask_progress", "block_progress", "block_unmask_progress",
+                 "output_min_confidence", "output_q25_confidence", "output_median_confidence", "output_avg_confidence", "output_q75_confidence")
 T_X_IN, T_NORM1, T_Q, T_K, T_V, T_ATTN, T_X_MID, T_NORM2, T_ACT, T_X_OUT, T_FINAL_NORM, T_KCACHE, T_VCACHE = range(13)
 EPI_F32, EPI_BF16, EPI_RESID, EPI_SWIGLU = 0, 1, 2, 3
 
@@ -56,7 +59,7 @@ class _Result(C.Structure):
     _fields_ = [("n_committed", C.POINTER(C.c_int32)), ("pos", C.POINTER(C.c_int32)), ("tok", C.POINTER(C.c_int32)),
                 ("conf", C.POINTER(C.c_float)), ("capacity", C.c_int32), ("total", C.c_int32),
                 ("n_masked_left", C.POINTER(C.c_int32)), ("lse", C.POINTER(C.c_float)),
-                ("row_conf", C.POINTER(C.c_float)), ("row_tok", C.POINTER(C.c_int32))]
+                ("row_conf", C.POINTER(C.c_float)), ("row_tok", C.POINTER(C.c_int32)), ("features", C.POINTER(C.c_float))]
 
 
 class _CostRow(C.Structure):
@@ -138,8 +141,9 @@ def _fp(a: np.ndarray):
 class StepResult:
     """Host copy of a dlm_result: per-request commit lists plus the per-row statistics."""
 
-    def __init__(self, n, max_block, n_committed, pos, tok, conf, n_masked_left, lse, row_conf, row_tok, usec):
+    def __init__(self, n, max_block, n_committed, pos, tok, conf, n_masked_left, lse, row_conf, row_tok, usec, features=None):
         self.n_committed = n_committed
+        self.features = features          # [n, 11] Step Predictor features (FEATURE_NAMES) when requested
         self.n_masked_left = n_masked_left
         self.lse, self.row_conf, self.row_tok = lse.reshape(n, max_block), row_conf.reshape(n, max_block), row_tok.reshape(n, max_block)
         self.usec = usec
@@ -196,6 +200,7 @@ class Engine:
         self._left = np.zeros(max_requests, np.int32)
         self._lse, self._rconf = np.zeros(R, np.float32), np.zeros(R, np.float32)
         self._rtok = np.zeros(R, np.int32)
+        self._feat = np.zeros(max_requests * N_FEATURES, np.float32)
 
     # -- lifetime --
     def close(self):
@@ -240,13 +245,13 @@ class Engine:
         return {"cur_block": a.value, "cache_valid": bool(b.value), "n_masked": c.value}
 
     # -- steps --
-    def _step(self, kind: int, reqs: Sequence[int], thresholds, dry_run: bool) -> StepResult:
+    def _step(self, kind: int, reqs: Sequence[int], thresholds, dry_run: bool, features: bool = False) -> StepResult:
         n = len(reqs)
         r = np.ascontiguousarray(reqs, dtype=np.int32)
         thr = None if thresholds is None else np.ascontiguousarray(thresholds, dtype=np.float32)
         b = _Batch(n, _ip(r), _fp(thr) if thr is not None else None, DLM_DRY_RUN if dry_run else 0)
         res = _Result(_ip(self._nc), _ip(self._pos), _ip(self._tok), _fp(self._conf), len(self._pos), 0, _ip(self._left),
-                      _fp(self._lse), _fp(self._rconf), _ip(self._rtok))
+                      _fp(self._lse), _fp(self._rconf), _ip(self._rtok), _fp(self._feat) if features else None)
         L = lib()
         if kind == KIND_REFRESH:
             rc = L.dlm_refresh_step(self._h, C.byref(b), C.byref(res))
@@ -258,17 +263,17 @@ class Engine:
         mb = self.max_block
         return StepResult(n, mb, self._nc[:n].copy(), self._pos, self._tok, self._conf, self._left[:n].copy(),
                           self._lse[:n * mb].copy(), self._rconf[:n * mb].copy(), self._rtok[:n * mb].copy(),
-                          L.dlm_last_step_usec(self._h))
+                          L.dlm_last_step_usec(self._h), self._feat[:n * N_FEATURES].reshape(n, N_FEATURES).copy() if features else None)
 
-    def refresh_step(self, reqs, thresholds=None, dry_run=False) -> StepResult:
-        return self._step(KIND_REFRESH, reqs, thresholds, dry_run)
+    def refresh_step(self, reqs, thresholds=None, dry_run=False, features=False) -> StepResult:
+        return self._step(KIND_REFRESH, reqs, thresholds, dry_run, features)
 
-    def cached_step(self, reqs, thresholds=None, dry_run=False) -> StepResult:
-        return self._step(KIND_CACHED, reqs, thresholds, dry_run)
+    def cached_step(self, reqs, thresholds=None, dry_run=False, features=False) -> StepResult:
+        return self._step(KIND_CACHED, reqs, thresholds, dry_run, features)
 
-    def mixed_step(self, reqs, thresholds=None, dry_run=False) -> StepResult:
+    def mixed_step(self, reqs, thresholds=None, dry_run=False, features=False) -> StepResult:
         """One ragged launch: every request takes the step kind that is due (refresh if its cache is invalid)."""
-        return self._step(KIND_MIXED, reqs, thresholds, dry_run)
+        return self._step(KIND_MIXED, reqs, thresholds, dry_run, features)
 
     # -- misc --
     def set_option(self, key: int, value: int):

@@ -466,6 +466,7 @@ struct Req {
   bool cache_valid = false;
   int n_masked = 0;           // whole request
   int n_masked_block = 0;     // current block
+  int steps_done = 0;         // completed (non-dry) denoising steps (Step Predictor feature full_progress)
   std::vector<int> pages;
 };
 
@@ -473,7 +474,7 @@ struct LayerW { void *wqkv, *wo, *wgu, *wd; };
 
 struct HostBatch {
   int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0;
-  std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, tok_bi;
+  std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, gen_lo, gen_len, tok_bi;
   std::vector<float> tau;
   std::vector<char> refresh;     // per request: whole sequence recomputed this step
 };
@@ -524,6 +525,8 @@ struct dlm_ctx {
   float *rope_cos = nullptr, *rope_sin = nullptr;
   // request state
   int* tokens = nullptr;       // [max_requests, max_seq]
+  float* conf_state = nullptr; // [max_requests, max_seq] per position: confidence last seen while masked (NEXT-1)
+  bool want_feat = false;      // this step's caller asked for the Step Predictor features
   int* page_table = nullptr;   // [max_requests, max_pages_per_req]
   void* kv_store = nullptr;
   KvGeom kg;
@@ -717,10 +720,12 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
     c->attn_ws_bytes = (size_t)8 * std::min(c->Tmax, 1024) * a.n_heads * (128 + 2) * 4;
     ALLOC(c->attn_ws, c->attn_ws_bytes);
   }
-  c->desc_cap_ints = (size_t)10 * a.max_requests + c->Tmax + 64;      // 9 n + T used
+  c->desc_cap_ints = (size_t)12 * a.max_requests + c->Tmax + 64;      // 11 n + T used
   ALLOC(c->desc_dev, c->desc_cap_ints * 4);
   if (cudaMallocHost(&c->desc_host, c->desc_cap_ints * 4) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
-  c->out_bytes = (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6;
+  c->out_bytes = (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6 + (size_t)a.max_requests * 5 * 4;     // + confidence features
+  ALLOC(c->conf_state, (size_t)a.max_requests * a.max_seq * 4);
+  cudaMemsetAsync(c->conf_state, 0, (size_t)a.max_requests * a.max_seq * 4, c->st);
   ALLOC(c->out_dev, c->out_bytes);
   if (cudaMallocHost(&c->out_host, c->out_bytes) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
   cudaEventCreate(&c->ev0);
@@ -831,6 +836,7 @@ extern "C" int dlm_request_add(dlm_ctx* c, const int32_t* prompt, int32_t P, int
   for (int i = 0; i < P; ++i) tok[i] = prompt[i];
   for (int i = P; i < S; ++i) tok[i] = a.mask_id;
   CU_TRY(&c->err, cudaMemcpyAsync(c->tokens + (size_t)slot * a.max_seq, tok.data(), (size_t)S * 4, cudaMemcpyHostToDevice, c->st));
+  CU_TRY(&c->err, cudaMemsetAsync(c->conf_state + (size_t)slot * a.max_seq, 0, (size_t)a.max_seq * 4, c->st));
   CU_TRY(&c->err, cudaMemcpyAsync(c->page_table + (size_t)slot * c->kg.max_pages_per_req, row.data(), row.size() * 4, cudaMemcpyHostToDevice, c->st));
   CU_TRY(&c->err, cudaStreamSynchronize(c->st));
   *out_req = slot;
@@ -907,6 +913,7 @@ static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override
     float tau = thr_override ? thr_override[i] : (b->threshold ? b->threshold[i] : q->tau);
     hb.slot.push_back(r); hb.q_off.push_back(hb.T); hb.q_len.push_back(qlen); hb.q_pos0.push_back(qpos0);
     hb.kv_len.push_back(q->S); hb.blk_lo.push_back(blk_lo); hb.blk_len.push_back(done ? 0 : q->B);
+    hb.gen_lo.push_back(q->P); hb.gen_len.push_back(q->G);
     hb.row_off.push_back(hb.R); hb.tau.push_back(tau); hb.refresh.push_back(refresh ? 1 : 0);
     for (int t = 0; t < qlen; ++t) hb.tok_bi.push_back(i);
     hb.T += qlen; hb.R += done ? 0 : q->B;
@@ -924,8 +931,10 @@ static size_t fill_desc_host(dlm_ctx* c, const HostBatch& hb) {
   const std::vector<int>* v[8] = {&hb.slot, &hb.q_off, &hb.q_len, &hb.q_pos0, &hb.kv_len, &hb.blk_lo, &hb.blk_len, &hb.row_off};
   for (int i = 0; i < 8; ++i) memcpy(h + i * n, v[i]->data(), n * 4);
   memcpy(h + 8 * n, hb.tau.data(), n * 4);
-  memcpy(h + 9 * n, hb.tok_bi.data(), hb.tok_bi.size() * 4);
-  return 9 * n + hb.tok_bi.size();
+  memcpy(h + 9 * n, hb.gen_lo.data(), n * 4);
+  memcpy(h + 10 * n, hb.gen_len.data(), n * 4);
+  memcpy(h + 11 * n, hb.tok_bi.data(), hb.tok_bi.size() * 4);
+  return 11 * n + hb.tok_bi.size();
 }
 static BatchDesc make_desc(dlm_ctx* c, const HostBatch& hb) {
   BatchDesc d;
@@ -933,7 +942,7 @@ static BatchDesc make_desc(dlm_ctx* c, const HostBatch& hb) {
   const int* b = c->desc_dev;
   d.n = hb.n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv;
   d.slot = b; d.q_off = b + n; d.q_len = b + 2 * n; d.q_pos0 = b + 3 * n; d.kv_len = b + 4 * n; d.blk_lo = b + 5 * n;
-  d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.tok_bi = b + 9 * n;
+  d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.tok_bi = b + 11 * n;
   return d;
 }
 
@@ -1163,6 +1172,12 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     KScope ks(c, DLM_K_COMBINE_UNMASK);
     launch_k(combine_unmask_kernel, dim3(bd.n), dim3(1024), 0, st, pdl, so, (const RowPartial*)c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd,
              dry_run ? 1 : 0);
+    if (c->want_feat) {
+      float* feats = (float*)(c->out_dev + (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6);
+      const int* gl = c->desc_dev + 9 * (size_t)bd.n;
+      launch_k(conf_features_kernel, dim3(bd.n), dim3(1024), 0, st, pdl, feats, c->conf_state, (const int*)c->tokens, a.max_seq, a.max_block, a.mask_id, so, bd,
+               gl, gl + bd.n, dry_run ? 1 : 0);
+    }
   }
   CU_TRY(err, cudaGetLastError());
   return DLM_OK;
@@ -1195,10 +1210,11 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   if (res->capacity < hb.R) { set_err(&c->err, "step: result capacity %d < %d block rows", res->capacity, hb.R); return DLM_E_CAPACITY; }
   std::string* err = &c->err;
   const size_t desc_ints = fill_desc_host(c, hb);
+  c->want_feat = res->features != nullptr;
   const bool use_graph = c->opt_graph && !c->kprof.on && !c->opt_dump;
   bool launched = false;
   if (use_graph) {
-    GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask());
+    GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask() | (c->want_feat ? 1 << 16 : 0));
     GraphEntry& g = c->graphs[key];
     if (g.seen == 1) {                         // second sighting of this batch shape: capture it
       const long long l0 = g_launches;
@@ -1239,7 +1255,8 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   const int* n_comm = (const int*)ob; ob += (size_t)a.max_requests * 4;
   const size_t rb = (size_t)c->Rmax * 4;
   const int* pos = (const int*)ob; ob += rb; const int* tok = (const int*)ob; ob += rb; const float* conf = (const float*)ob; ob += rb;
-  const float* rlse = (const float*)ob; ob += rb; const float* rconf = (const float*)ob; ob += rb; const int* rtok = (const int*)ob;
+  const float* rlse = (const float*)ob; ob += rb; const float* rconf = (const float*)ob; ob += rb; const int* rtok = (const int*)ob; ob += rb;
+  const float* feats = (const float*)ob;
   int total = 0;
   for (int i = 0; i < hb.n; ++i) {
     Req& q = c->reqs[hb.slot[i]];
@@ -1260,6 +1277,7 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
     if (hb.refresh[i] && hb.blk_len[i]) q.cache_valid = true;      // K/V of all positions now match the pre-step tokens
     if (!dry && hb.blk_len[i]) {
       q.n_masked -= k; q.n_masked_block -= k;
+      q.steps_done++;
       if (q.n_masked_block == 0) {                            // P:109 block complete -> recompute before the next block
         q.cache_valid = false;
         q.cur_block++;
@@ -1267,6 +1285,14 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
       }
     }
     if (res->n_masked_left) res->n_masked_left[i] = q.n_masked;
+    if (res->features) {          // App. A order; the request's state AFTER this step (a dry run reports, like everything else, without mutating)
+      float* f = res->features + (size_t)i * DLM_N_FEATURES;
+      const int nb = q.G / q.B;
+      const bool fin = q.cur_block >= nb;
+      f[0] = hb.tau[i]; f[1] = (float)q.G; f[2] = (float)q.steps_done / q.G; f[3] = (float)(q.G - q.n_masked) / q.G;
+      f[4] = fin ? 1.f : (float)q.cur_block / nb; f[5] = fin ? 1.f : (float)(q.B - q.n_masked_block) / q.B;
+      for (int j = 0; j < 5; ++j) f[6 + j] = feats[i * 5 + j];
+    }
   }
   res->total = total;
   c->last_batch = hb;

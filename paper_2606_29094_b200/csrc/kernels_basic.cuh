@@ -500,4 +500,75 @@ __global__ void __launch_bounds__(1024) combine_unmask_kernel(StepOut o, const R
   if (l == 0) o.n_committed[bi] = count;
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-1  Step Predictor confidence features ("confidence statistics", App. A; reading G22).
+// conf_state[slot][pos] = the confidence the model last gave position pos while it was masked (frozen at commit, 0
+// before any step evaluated it).  After the unmask: positions of the current block that were masked before the step
+// take this step's row confidence; then min / q25 / median / mean / q75 over the G output positions (bitonic sort in
+// shared memory, quartiles by linear interpolation between order statistics).  One block per request.
+// ------------------------------------------------------------------------------------------------
+constexpr int kFeatMaxGen = 2048;
+__global__ void __launch_bounds__(1024) conf_features_kernel(float* __restrict__ feats, float* __restrict__ conf_state,
+                                                            const int* __restrict__ tokens, int max_seq, int max_block, int mask_id,
+                                                            StepOut o, BatchDesc b, const int* __restrict__ gen_lo,
+                                                            const int* __restrict__ gen_len, int dry_run) {
+  __shared__ float s[kFeatMaxGen];
+  __shared__ float red[33];
+  pdl_launch_dependents();
+  pdl_wait();
+  const int bi = blockIdx.x, tid = threadIdx.x;
+  const int P = gen_lo[bi], G = gen_len[bi], B = b.blk_len[bi], lo = b.blk_lo[bi];
+  float* f = feats + bi * 5;
+  if (G > kFeatMaxGen || G <= 0) {
+    if (tid < 5) f[tid] = __int_as_float(0x7fc00000);
+    return;
+  }
+  int n2 = 1;
+  while (n2 < G) n2 <<= 1;
+  const long long row = (long long)b.slot[bi] * max_seq;
+  const int n_comm = B > 0 ? o.n_committed[bi] : 0;
+  float part = 0.f;
+  for (int j = tid; j < n2; j += blockDim.x) {
+    float v = CUDART_INF_F;
+    if (j < G) {
+      const int pos = P + j;
+      v = conf_state[row + pos];
+      if (pos >= lo && pos < lo + B) {
+        bool was_masked = tokens[row + pos] == mask_id;
+        if (!was_masked && !dry_run)
+          for (int k = 0; k < n_comm; ++k) was_masked |= o.pos[bi * max_block + k] == pos;      // committed by this very step
+        if (was_masked) {
+          v = o.row_conf[bi * max_block + (pos - lo)];
+          if (!dry_run) conf_state[row + pos] = v;
+        }
+      }
+      part += v;
+    }
+    s[j] = v;
+  }
+  const float total = block_sum(part, red);
+  for (int k = 2; k <= n2; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = tid; i < n2; i += blockDim.x) {
+        const int ixj = i ^ j;
+        if (ixj > i) {
+          const float a = s[i], c = s[ixj];
+          const bool up = (i & k) == 0;
+          if ((a > c) == up) { s[i] = c; s[ixj] = a; }
+        }
+      }
+      __syncthreads();
+    }
+  }
+  if (tid == 0) {
+    auto quant = [&](float q) {
+      const float h = (float)(G - 1) * q;
+      const int l = (int)floorf(h);
+      const int u = min(l + 1, G - 1);
+      return s[l] + (h - (float)l) * (s[u] - s[l]);
+    };
+    f[0] = s[0]; f[1] = quant(0.25f); f[2] = quant(0.5f); f[3] = total / (float)G; f[4] = quant(0.75f);
+  }
+}
+
 }  // namespace dlm

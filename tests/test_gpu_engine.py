@@ -204,6 +204,43 @@ def test_mixed_step_equals_per_kind_calls(bf16_model):
     eng.close()
 
 
+@pytest.mark.parametrize("tau", [0.9, 0.05, 1.5])
+def test_step_predictor_features_from_gpu_confidences(tau):
+    """NEXT-1 (App. A, reading G22): the 11 features the device returns after every step equal
+    oracle.predictor_features evaluated on the GPU's own per-row confidences and commits (stage-wise, protocol P-C):
+    progress features exact, confidence features within fp32 rounding.  Free-running to completion, two requests of
+    different block lengths in one batch, with dry-run steps interleaved (they must not move the state)."""
+    pkg = _pkg()
+    a = ARCH_C1
+    rng = np.random.default_rng(31)
+    specs = [(random_tokens(rng, 40, a.vocab, a.mask_id), 64, 32, tau), (random_tokens(rng, 9, a.vocab, a.mask_id), 48, 16, tau)]
+    eng = pkg.Engine(a, WEIGHT_SEED["C1"], max_requests=2, max_seq=128, max_block=32)
+    ids = [eng.add_request(*s) for s in specs]
+    mirror = [ostep.Request(a, s[0], s[1], s[2], s[3]) for s in specs]
+    assert pkg.FEATURE_NAMES == ostep.FEATURE_NAMES
+    steps = 0
+    while any(eng.info(i)["n_masked"] for i in ids) and steps < 200:
+        live = [k for k, i in enumerate(ids) if eng.info(i)["n_masked"]]
+        rids = [ids[k] for k in live]
+        d = eng.mixed_step(rids, dry_run=True, features=True)          # reports, mutates nothing
+        g = eng.mixed_step(rids, features=True)
+        for j, k in enumerate(live):
+            m = mirror[k]
+            lo, hi = m.block_range(m.current_block())
+            was_masked = m.tokens[lo:hi] == a.mask_id
+            m.conf_state[lo - m.P:hi - m.P][was_masked] = g.row_conf[j][:hi - lo][was_masked].astype(np.float64)
+            m.steps_done += 1
+            for pos, tok, _ in g.commits[j]:
+                m.tokens[pos] = tok
+            want = ostep.predictor_features(m, tau)
+            assert np.array_equal(g.features[j][:6], want[:6].astype(np.float32)), (steps, g.features[j], want)
+            assert np.allclose(g.features[j][6:], want[6:], rtol=2e-6, atol=1e-7), (steps, g.features[j], want)
+            assert d.commits[j] == g.commits[j]
+        steps += 1
+    assert all(m.current_block() is None for m in mirror)
+    eng.close()
+
+
 # ------------------------------------------------------------------------------------------------------------------
 ARCH_C1_BF16 = ARCH_C1.replace(weight_dtype=1)
 
