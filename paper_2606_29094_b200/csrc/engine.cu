@@ -590,7 +590,13 @@ static void launch_rmsnorm(dlm_ctx* c, TE* u, float* x, const int* row_src, int 
   if (rows >= 1024)
     launch_k(rmsnorm_rows_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride);
   else
-    launch_k(rmsnorm_kernel<TE>, dim3(rows), dim3(norm_threads(d)), 0, c->st, pdl, u, x, row_src, d, eps, part, n_part, part_stride);
+  {
+    // more rows than two resident 1024-thread blocks per SM can hold: 256-thread blocks (4 float4 per thread) keep every
+    // row of a 512-token step in flight in one wave
+    int threads = norm_threads(d);
+    if (rows > 2 * g_num_sms && d >= 1024 && d <= 4096) threads = 256;
+    launch_k(rmsnorm_kernel<TE>, dim3(rows), dim3(threads), 0, c->st, pdl, u, x, row_src, d, eps, part, n_part, part_stride);
+  }
 }
 
 static int nqkv(const dlm_arch& a) { return (a.n_heads + 2 * a.n_kv_heads) * a.head_dim; }
