@@ -106,6 +106,16 @@ def lib() -> C.CDLL:
         L.dlm_last_step_usec.restype = f32
         L.dlm_last_error.argtypes = [vp]
         L.dlm_last_error.restype = C.c_char_p
+        f64 = C.c_double
+        L.dlm_lp_lookup.argtypes = [C.POINTER(_CostRow), i32, i32, f64, i32]
+        L.dlm_lp_lookup.restype = f64
+        L.dlm_req_load.argtypes = [f64, i32, i32, i32]
+        L.dlm_req_load.restype = f64
+        L.dlm_instance_capacity.argtypes = [C.POINTER(_CostRow), i32, i32, i32, i32, i32, f64]
+        L.dlm_instance_capacity.restype = f64
+        L.dlm_time_left.argtypes = [C.POINTER(_CostRow), i32, f64, i32, i32, i32, i32, i32]
+        L.dlm_time_left.restype = f64
+        L.dlm_pick_threshold.argtypes = [C.POINTER(f32), C.POINTER(f64), i32, f64, C.POINTER(_CostRow), i32, i32, i32, i32, i32, i32]
         L.dlm_op_gemm_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
         L.dlm_op_gemm_pair_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
         L.dlm_op_gemm_plain_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp]
@@ -303,6 +313,50 @@ class Engine:
         self._check(lib().dlm_profile_step_costs(self._h, rows, cap, C.byref(n)))
         return [dict(kind="refresh" if rows[i].kind == KIND_REFRESH else "cached", n_requests=rows[i].n_requests,
                      n_tokens=rows[i].n_tokens, kv_tokens=rows[i].kv_tokens, usec=rows[i].usec) for i in range(n.value)]
+
+
+# ---------------------------------------------------------------------------------------------------------
+# host-side consumers of the cost table (include/dlm_sched.h; rows = [(kind, tokens, kv, usec)] or profile_step_costs dicts)
+# ---------------------------------------------------------------------------------------------------------
+def _cost_rows(rows):
+    arr = (_CostRow * len(rows))()
+    for i, r in enumerate(rows):
+        if isinstance(r, dict):
+            kind, n, tokens, kv, usec = r["kind"], r.get("n_requests", 0), r["n_tokens"], r["kv_tokens"], r["usec"]
+        else:
+            kind, tokens, kv, usec = r
+            n = 0
+        arr[i] = _CostRow(KIND_REFRESH if kind in ("refresh", KIND_REFRESH) else KIND_CACHED, n, int(tokens), int(kv), float(usec))
+    return arr, len(rows)
+
+
+def lp_lookup(rows, kind, tokens, kv):
+    a, n = _cost_rows(rows)
+    return lib().dlm_lp_lookup(a, n, KIND_REFRESH if kind in ("refresh", KIND_REFRESH) else KIND_CACHED, float(tokens), int(kv))
+
+
+def req_load(pred_steps_left, recomp_steps_left, num_tokens, cache_block):
+    return lib().dlm_req_load(float(pred_steps_left), recomp_steps_left, num_tokens, cache_block)
+
+
+def instance_capacity(rows, cache_block, max_seq_per_batch, num_token_per_req, kv, slo_sec):
+    a, n = _cost_rows(rows)
+    return lib().dlm_instance_capacity(a, n, cache_block, max_seq_per_batch, num_token_per_req, kv, float(slo_sec))
+
+
+def time_left(rows, pred_steps_left, recomp_steps_left, cache_block, num_reqs, num_tokens, kv):
+    a, n = _cost_rows(rows)
+    return lib().dlm_time_left(a, n, float(pred_steps_left), recomp_steps_left, cache_block, num_reqs, num_tokens, kv)
+
+
+def pick_threshold(allowed_desc, pred_steps_left, slo_left_sec, rows, recomp_steps_left, cache_block, num_reqs, num_tokens, kv):
+    a, n = _cost_rows(rows)
+    th = (C.c_float * len(allowed_desc))(*allowed_desc)
+    st = (C.c_double * len(pred_steps_left))(*pred_steps_left)
+    rc = lib().dlm_pick_threshold(th, st, len(allowed_desc), float(slo_left_sec), a, n, recomp_steps_left, cache_block, num_reqs, num_tokens, kv)
+    if rc < 0:
+        raise DlmError(rc, "dlm_pick_threshold: bad arguments")
+    return rc
 
 
 # ---------------------------------------------------------------------------------------------------------

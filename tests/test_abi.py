@@ -56,3 +56,25 @@ def test_arch_validation(pkg):
         with pytest.raises(pkg.DlmError) as e:
             pkg.Engine(bad, 1)
         assert e.value.code == pkg.binding.DLM_E_ARG
+
+
+def test_cost_table_consumers_match_the_oracle(pkg):
+    """NEXT-3 host functions of libdlm.so (no device needed) against oracle/sched.py on a toy latency profile and on
+    random queries: Alg. 1 / 4 / 5 with the G18 readings."""
+    import numpy as np
+    from oracle import sched
+    from paper_2606_29094_b200 import binding as B
+    LP = [("cached", 32, 512, 1320.0), ("cached", 64, 512, 1640.0), ("cached", 256, 512, 3560.0), ("cached", 32, 2048, 2640.0),
+          ("cached", 256, 2048, 7120.0), ("refresh", 512, 512, 51200.0), ("refresh", 1024, 512, 102400.0), ("refresh", 2048, 2048, 204800.0)]
+    rng = np.random.default_rng(0)
+    for _ in range(200):
+        kind = "cached" if rng.random() < 0.5 else "refresh"
+        tokens, kv = float(rng.integers(1, 3000)), int(rng.integers(64, 4096))
+        assert abs(B.lp_lookup(LP, kind, tokens, kv) - sched.lp_lookup(LP, kind, tokens, kv)) < 1e-9
+    assert B.req_load(40, 2, 512, 32) == sched.req_load(40, 2, 512, 32) == 2240
+    assert abs(B.instance_capacity(LP, 32, 8, 512, 512, 10.0) - sched.instance_capacity(LP, 32, 8, 512, 512, 10.0)) < 1e-6
+    assert abs(B.time_left(LP, 40, 2, 32, 4, 1024, 512) - sched.time_left(LP, 40, 2, 32, 4, 1024, 512)) < 1e-12
+    allowed, steps = [0.95, 0.9, 0.7, 0.5], [60.0, 40.0, 25.0, 12.0]
+    for slo in (0.0, 0.1, 0.25, 0.3, 0.35, 1.0):
+        assert B.pick_threshold(allowed, steps, slo, LP, 2, 32, 4, 1024, 512) == sched.pick_threshold(allowed, steps, slo, LP, 2, 32, 4, 1024, 512)
+    assert np.isnan(B.lp_lookup([r for r in LP if r[0] == "cached"], "refresh", 10, 512))
