@@ -16,6 +16,9 @@ Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`):
                trajectory == recompute-every-step trajectory; batch independence
   brute.py     scalar-loop twin (no matmul) agreeing with model.py/step.py on tiny shapes
   split-vocab  (max, sum-exp, argmax) merge == direct softmax for any tiling
+  step.py      Step Predictor features (App. A, G22): library quantile on random data, hand cases, tau>1
+               closed forms, frozen-at-commit, dry-run leaves the state alone
+  sched.py     Alg. 1 / 4 / 5 (G18 readings): hand-worked numbers on a toy latency profile
 
 parity unpinned: trained-model behaviour (Figure 2 example, "-38% steps at 0.7")
 needs LLaDA/Dream weights and datasets that are not in this container.
