@@ -46,6 +46,7 @@ struct TaParams {
   float* ws_o;              // [splits, T*H, 128] (splits > 1)
   float* ws_ml;             // [splits, T*H, 2]
   unsigned long long kv_policy;
+  int row_filter;           // mixed steps: 0 all requests, 1 only those with <= 64 stacked rows, 2 only those with more
 };
 
 namespace ptx {
@@ -96,6 +97,7 @@ __device__ __forceinline__ void ta_range(const TaItem& im, const TaParams& p, in
   *t_begin = im.split * per;
   *t_end = min(n_tiles, *t_begin + per);
   if (im.qt * kTaTile >= *n_rows) { *t_begin = 0; *t_end = 0; }
+  if ((p.row_filter == 1 && *n_rows > 64) || (p.row_filter == 2 && *n_rows <= 64)) { *t_begin = 0; *t_end = 0; *n_rows = 0; }   // the other launch's request
 }
 
 __global__ void __launch_bounds__(kTaThreads, 1) attn_tc_kernel(const __grid_constant__ CUtensorMap mapKV, const TaParams p) {

@@ -42,6 +42,7 @@ struct BatchDesc {
   int R;             // rows that need logits (sum blk_len)
   int max_q_len;     // max over requests (attention grid sizing)
   int max_kv_len;
+  int min_q_len;     // min over requests that compute anything (mixed steps: block rows of the cached requests)
   const int* slot;   // [n] request slot (row of tokens / page table)
   const int* q_off;  // [n]
   const int* q_len;  // [n]

@@ -306,6 +306,10 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   // sub-partitions; force: 0 engine choice, 1 = forced with the split the engine would pick, 1 + s = forced with s splits
   const bool fits_t = bd.max_q_len * r <= kTtNQ;
   const bool transposed = fits_t && !no_transposed;
+  // mixed step: the cached requests (<= 64 stacked rows) go to the transposed-score kernel, the refreshing ones to the
+  // row-major kernel; each launch skips the other's requests (row_filter), no K/V split
+  const bool two_kernels = !force && !fits_t && bd.min_q_len > 0 && bd.min_q_len * r <= kTtNQ;
+  if (two_kernels) splits = 1;
   const CUtensorMap* mkv = tc.get(kv_store, rows, 128, 64);
   if (!mkv) { set_err(err, "cuTensorMapEncodeTiled failed (attention K/V store %p, %lld rows)", (const void*)kv_store, rows); return DLM_E_CUDA; }
   static bool configured = false;
@@ -320,12 +324,24 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   p.splits = splits; p.q_tiles_max = q_tiles; p.n_items = (int)(items * splits);
   p.scale_log2 = scale * 1.4426950408889634f; p.ws_o = nullptr; p.ws_ml = nullptr;
   p.kv_policy = q_tiles == 1 ? DLM_L2_EVICT_FIRST : DLM_L2_EVICT_NORMAL;
+  p.row_filter = 0;
   const long long TH = (long long)bd.T * n_heads;
   while (splits > 1 && (size_t)splits * TH * (128 + 2) * 4 > *ws_bytes) --splits;     // fixed workspace (see attn_flash_launch)
   p.splits = splits; p.n_items = (int)(items * splits);
   if (splits > 1) {
     p.ws_o = *ws;
     p.ws_ml = *ws + (size_t)splits * TH * 128;
+  }
+  if (two_kernels) {
+    TaParams pt = p;
+    pt.row_filter = 1; pt.q_tiles_max = 1; pt.n_items = bd.n * g.n_kv_heads; pt.kv_policy = DLM_L2_EVICT_FIRST;
+    p.row_filter = 2;
+    cudaError_t e2 = launch_k(attn_tct_kernel, dim3((unsigned)std::min(g_num_sms, pt.n_items)), dim3(kTaThreads), (size_t)kTtSmem, st, pdl, *mkv, pt);
+    if (e2 == cudaSuccess)
+      e2 = launch_k(attn_tc_kernel, dim3((unsigned)std::min<long long>(g_num_sms, p.n_items)), dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
+    if (e2 != cudaSuccess) { set_err(err, "attn_tc launch: %s", cudaGetErrorString(e2)); return DLM_E_CUDA; }
+    *done = true;
+    return 0;
   }
   const dim3 grid((unsigned)std::min<long long>(g_num_sms, p.n_items));
   cudaError_t e = transposed ? launch_k(attn_tct_kernel, grid, dim3(kTaThreads), (size_t)kTtSmem, st, pdl, *mkv, p)
@@ -424,7 +440,7 @@ static int attn_op_contiguous(const void* q, const void* k, const void* v, void*
   repack_kv_kernel<<<S, 128, 0, st>>>(store, (const bf16*)k, (const bf16*)v, S, g);
   DLM_LAUNCH_CHECK();
   BatchDesc bd = {};
-  bd.n = 1; bd.T = Tq; bd.max_q_len = Tq; bd.max_kv_len = S;
+  bd.n = 1; bd.T = Tq; bd.max_q_len = Tq; bd.max_kv_len = S; bd.min_q_len = Tq;
   int* md = meta + g.n_pages;
   bd.slot = md; bd.q_off = md + 1; bd.q_len = md + 2; bd.q_pos0 = md + 3; bd.kv_len = md + 4; bd.tok_bi = md + 16;
   const float scale = 1.f / sqrtf((float)dh);
@@ -473,7 +489,7 @@ struct Req {
 struct LayerW { void *wqkv, *wo, *wgu, *wd; };
 
 struct HostBatch {
-  int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0;
+  int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0, min_q = 1 << 30;
   std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, gen_lo, gen_len, tok_bi;
   std::vector<float> tau;
   std::vector<char> refresh;     // per request: whole sequence recomputed this step
@@ -924,6 +940,7 @@ static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override
     for (int t = 0; t < qlen; ++t) hb.tok_bi.push_back(i);
     hb.T += qlen; hb.R += done ? 0 : q->B;
     hb.max_q = std::max(hb.max_q, qlen); hb.max_kv = std::max(hb.max_kv, q->S);
+    if (qlen > 0) hb.min_q = std::min(hb.min_q, qlen);
   }
   if (hb.T > c->Tmax) { set_err(&c->err, "step: %d tokens exceed max_batch_tokens=%d", hb.T, c->Tmax); return DLM_E_CAPACITY; }
   return DLM_OK;
@@ -946,7 +963,7 @@ static BatchDesc make_desc(dlm_ctx* c, const HostBatch& hb) {
   BatchDesc d;
   const size_t n = hb.n;
   const int* b = c->desc_dev;
-  d.n = hb.n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv;
+  d.n = hb.n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv; d.min_q_len = std::min(hb.min_q, hb.max_q);
   d.slot = b; d.q_off = b + n; d.q_len = b + 2 * n; d.q_pos0 = b + 3 * n; d.kv_len = b + 4 * n; d.blk_lo = b + 5 * n;
   d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.tok_bi = b + 11 * n;
   return d;
@@ -1220,7 +1237,7 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   const bool use_graph = c->opt_graph && !c->kprof.on && !c->opt_dump;
   bool launched = false;
   if (use_graph) {
-    GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask() | (c->want_feat ? 1 << 16 : 0));
+    GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask() | (c->want_feat ? 1 << 16 : 0) | (std::min(hb.min_q, 255) << 20));
     GraphEntry& g = c->graphs[key];
     if (g.seen == 1) {                         // second sighting of this batch shape: capture it
       const long long l0 = g_launches;

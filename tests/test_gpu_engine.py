@@ -204,6 +204,27 @@ def test_mixed_step_equals_per_kind_calls(bf16_model):
     eng.close()
 
 
+def test_mixed_step_llada_shape_two_attention_kernels():
+    """Mixed step at the LLaDA head shape (d_h 128, 32 heads, 2 layers): the refreshing request goes through the row-major
+    tcgen05 attention kernel, the cached ones through the transposed-score kernel, in the same step; per-request results
+    equal those of the per-kind calls up to GEMM tiling (fp32 summation order)."""
+    pkg = _pkg()
+    a = _reduced(ARCH_LLADA8B, 2)
+    rng = np.random.default_rng(8)
+    specs = [(random_tokens(rng, P, a.vocab, a.mask_id), 64, 32, 0.9) for P in (300, 100, 200, 129)]
+    eng = pkg.Engine(a, WEIGHT_SEED["C2"], max_requests=4, max_seq=384, max_block=32, max_batch_tokens=1280)
+    ids = [eng.add_request(*s) for s in specs]
+    eng.refresh_step(ids[1:], dry_run=True)                       # requests 1..3 hold a cache, request 0 does not
+    want = [eng.refresh_step([ids[0]], dry_run=True)] + [eng.cached_step([i], dry_run=True) for i in ids[1:]]
+    eng.set_tokens(ids[0], eng.tokens(ids[0]), keep_cache=False)
+    assert [eng.info(i)["cache_valid"] for i in ids] == [False, True, True, True]
+    got = eng.mixed_step(ids, dry_run=True)
+    for j in range(4):
+        assert np.allclose(got.lse[j], want[j].lse[0], rtol=3e-3, atol=3e-3), (j, np.abs(got.lse[j] - want[j].lse[0]).max())
+        assert np.abs(got.row_conf[j] - want[j].row_conf[0]).max() < 2e-2
+    eng.close()
+
+
 @pytest.mark.parametrize("tau", [0.9, 0.05, 1.5])
 def test_step_predictor_features_from_gpu_confidences(tau):
     """NEXT-1 (App. A, reading G22): the 11 features the device returns after every step equal
