@@ -393,6 +393,33 @@ def test_stagewise_from_gpu_inputs():
     eng.close()
 
 
+def test_batched_llada_shape_vs_oracle_tcgen05_attention():
+    """Engine-level parity with the oracle on a batch that takes the tcgen05 attention kernels (>= 64 (request, head) items):
+    refresh step (row-major kernel, several query tiles, ragged K/V tails) and cached step (transposed-score kernel, 64- and
+    32-row blocks in one launch), LLaDA head shape at 2 layers, both requests teacher-forced from the same tokens."""
+    pkg = _pkg()
+    a = _reduced(ARCH_LLADA8B, 2)
+    seed = WEIGHT_SEED["C2"]
+    rng = np.random.default_rng(21)
+    specs = [(random_tokens(rng, 200, a.vocab, a.mask_id), 128, 64, 0.9), (random_tokens(rng, 90, a.vocab, a.mask_id), 64, 32, 0.5)]
+    eng = pkg.Engine(a, seed, max_requests=2, max_seq=384, max_block=64, max_batch_tokens=640)
+    ids = [eng.add_request(*s) for s in specs]
+    wts = ow.Weights(a, seed)
+    oreqs = [ostep.Request(a, s[0], s[1], s[2], s[3]) for s in specs]
+    g_r = eng.refresh_step(ids, dry_run=True)
+    g_c = eng.cached_step(ids, dry_run=True)
+    for j, oreq in enumerate(oreqs):
+        o_r = ostep.refresh_step(oreq, wts, dry_run=True)
+        o_c = ostep.cached_step(oreq, wts, dry_run=True)
+        Bk = oreq.B
+        for g, o in ((g_r, o_r), (g_c, o_c)):
+            assert np.abs(g.lse[j][:Bk] - o.lse).max() <= 2e-2 * np.abs(o.lse).max()
+            assert np.abs(g.row_conf[j][:Bk] - o.conf).max() < 5e-2
+            clear = o.margin >= 5e-2
+            assert np.array_equal(g.row_tok[j][:Bk][clear], o.tok[clear])
+    eng.close()
+
+
 def test_c2_full_size_sampled_stages_and_properties():
     """BASELINE.json configs[1] at FULL size (32 layers, d 4096, vocab 126 464; the workload and launch configuration bench.py
     times).  The oracle cannot run 32 fp64 layers in test time, so: (i) properties in the production configuration
