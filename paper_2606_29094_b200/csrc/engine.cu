@@ -92,7 +92,30 @@ static bool make_tmap_bf16(CUtensorMap* m, const void* ptr, long long rows, long
   return r == CUDA_SUCCESS;
 }
 
+// fp32 output [splits][rows][ldc] of which `cols` columns are valid: box 32 columns x 32 rows x 1 slice, 128-byte swizzle
+// (the layout of the epilogue's coalescing stage).  TMA clips rows >= rows and columns >= cols, so ragged tiles need no code.
+static bool make_tmap_f32_out(CUtensorMap* m, const void* ptr, long long rows, long long cols, long long ldc, long long splits, long long split_stride) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)cols, (cuuint64_t)rows, (cuuint64_t)splits};
+  cuuint64_t strides[2] = {(cuuint64_t)ldc * 4, (cuuint64_t)split_stride * 4};
+  cuuint32_t box[3] = {32, 32, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
 struct TmapCache {
+  std::map<std::tuple<const void*, long long, long long, long long, long long>, CUtensorMap> mo;
+  const CUtensorMap* get_f32_out(const void* ptr, long long rows, long long cols, long long ldc, long long splits) {
+    auto key = std::make_tuple(ptr, rows, cols, ldc, splits);
+    auto it = mo.find(key);
+    if (it != mo.end()) return &it->second;
+    CUtensorMap t;
+    if (!make_tmap_f32_out(&t, ptr, rows, cols, ldc, splits, rows * ldc)) return nullptr;
+    return &mo.emplace(key, t).first->second;
+  }
   std::map<std::tuple<const void*, long long, long long, int>, CUtensorMap> m;
   const CUtensorMap* get(const void* ptr, long long rows, long long cols, int box_rows) {
     auto key = std::make_tuple(ptr, rows, cols, box_rows);
@@ -206,7 +229,7 @@ static void plan_pair(int M, int N, int K, int epi, int max_splits, int* bn_out,
 }
 
 template <int EPI>
-static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* mb, const GemmPairParams& p, cudaStream_t st, bool pdl) {
+static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* mb, const CUtensorMap* mc, const GemmPairParams& p, cudaStream_t st, bool pdl) {
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(gemm_pair_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
@@ -224,7 +247,7 @@ static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* 
   at[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = pdl ? 2 : 1;
   g_launches++;
-  return cudaLaunchKernelEx(&cfg, gemm_pair_kernel<EPI>, *ma, *mb, p);
+  return cudaLaunchKernelEx(&cfg, gemm_pair_kernel<EPI>, *ma, *mb, *mc, p);
 }
 
 // A: bf16 [a_rows_cap, K] buffer (M valid rows); W: bf16 [w_rows, K].  max_splits > 1 (EPI_F32 only) allows split-K:
@@ -259,15 +282,21 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
   if (epi == EPI_LMHEAD && p.n_tiles_n != p.n_tiles) { set_err(err, "gemm_pair: lm-head tile count mismatch"); return DLM_E_ARG; }
   const CUtensorMap* ma = tc.get(A, a_rows_cap, K, 128);
   const CUtensorMap* mb = tc.get(W, w_rows, K, bn / 2);
+  // fp32 outputs leave through TMA (store / reduce-add) from the epilogue's shared-memory stage
+  const CUtensorMap* mc = ma;
+  if (epi == EPI_F32 || epi == EPI_RESID) {
+    mc = tc.get_f32_out(p.out_f32, M, N, p.ldc, p.splits);
+    if (!mc) { set_err(err, "cuTensorMapEncodeTiled failed (gemm_pair output %p)", (void*)p.out_f32); return DLM_E_CUDA; }
+  }
   if (!ma || !mb) { set_err(err, "cuTensorMapEncodeTiled failed (gemm_pair A=%p rows=%lld K=%d, W=%p rows=%lld box=%d)", A, a_rows_cap, K, W, w_rows, bn / 2); return DLM_E_CUDA; }
   cudaError_t e;
   switch (epi) {
-    case EPI_F32: e = launch_gemm_pair_t<EPI_F32>(ma, mb, p, st, pdl); break;
-    case EPI_BF16: e = launch_gemm_pair_t<EPI_BF16>(ma, mb, p, st, pdl); break;
-    case EPI_RESID: e = launch_gemm_pair_t<EPI_RESID>(ma, mb, p, st, pdl); break;
-    case EPI_SWIGLU: e = launch_gemm_pair_t<EPI_SWIGLU>(ma, mb, p, st, pdl); break;
-    case EPI_LMHEAD: e = launch_gemm_pair_t<EPI_LMHEAD>(ma, mb, p, st, pdl); break;
-    case EPI_ROPE: e = launch_gemm_pair_t<EPI_ROPE>(ma, mb, p, st, pdl); break;
+    case EPI_F32: e = launch_gemm_pair_t<EPI_F32>(ma, mb, mc, p, st, pdl); break;
+    case EPI_BF16: e = launch_gemm_pair_t<EPI_BF16>(ma, mb, mc, p, st, pdl); break;
+    case EPI_RESID: e = launch_gemm_pair_t<EPI_RESID>(ma, mb, mc, p, st, pdl); break;
+    case EPI_SWIGLU: e = launch_gemm_pair_t<EPI_SWIGLU>(ma, mb, mc, p, st, pdl); break;
+    case EPI_LMHEAD: e = launch_gemm_pair_t<EPI_LMHEAD>(ma, mb, mc, p, st, pdl); break;
+    case EPI_ROPE: e = launch_gemm_pair_t<EPI_ROPE>(ma, mb, mc, p, st, pdl); break;
     default: set_err(err, "gemm_pair: bad epilogue %d", epi); return DLM_E_ARG;
   }
   if (e != cudaSuccess) { set_err(err, "gemm_pair launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
@@ -1462,7 +1491,7 @@ extern "C" int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t
   p.ldc = N;
   p.up_row0 = N;
   if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
-  g_op_tmaps.m.clear();   // caller buffers come and go; never reuse a stale map
+  g_op_tmaps.m.clear(); g_op_tmaps.mo.clear();   // caller buffers come and go; never reuse a stale map
   return gemm_tc(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, (cudaStream_t)stream);
 }
 
@@ -1477,7 +1506,7 @@ extern "C" int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, in
   GemmPairParams p = {};
   p.ldc = N;
   p.up_row0 = N;
-  g_op_tmaps.m.clear();
+  g_op_tmaps.m.clear(); g_op_tmaps.mo.clear();
   if (epi != EPI_F32 || splits == 1) {
     if (epi == EPI_F32 || epi == EPI_RESID) p.out_f32 = (float*)out; else p.out_bf16 = (bf16*)out;
     rc = gemm_pair(g_op_tmaps, &g_init_error, A, M, W, epi == EPI_SWIGLU ? 2LL * N : N, M, N, K, epi, bn, p, st);
@@ -1509,7 +1538,7 @@ extern "C" int dlm_op_gemm_skinny_bf16(const void* X, const void* W, void* out, 
     set_err(&g_init_error, "dlm_op_gemm_skinny_bf16: bad arguments (T must be in [1, %d])", kSkMaxTokens); return DLM_E_ARG;
   }
   cudaStream_t st = (cudaStream_t)stream;
-  g_op_tmaps.m.clear();
+  g_op_tmaps.m.clear(); g_op_tmaps.mo.clear();
   SkinnyParams p = {};
   p.ldc = N; p.up_row0 = N;
   if (epi == EPI_SWIGLU) {
@@ -1556,7 +1585,7 @@ static int op_head(const void* hidden, const void* Wlm, int n, int B, int V, int
   for (int i = 0; i < n; ++i) { h[i] = i; h[n + i] = 0; h[2 * n + i] = B; h[3 * n + i] = i * B; }
   cudaMemcpyAsync(meta, h.data(), h.size() * 4, cudaMemcpyHostToDevice, st);
   cudaStreamSynchronize(st);   // h is a stack-lifetime staging buffer
-  g_op_tmaps.m.clear();
+  g_op_tmaps.m.clear(); g_op_tmaps.mo.clear();
   int rc;
   if (R > 128) {                 // as in the engine: the CTA-pair kernel with 256-wide vocabulary tiles above 128 rows
     n_tiles = (V + 255) / 256;
@@ -1618,5 +1647,3 @@ extern "C" int dlm_op_attention_bf16(const void* q, const void* k, const void* v
   if (rc) return rc;
   return attn_op_contiguous(q, k, v, out, Tq, S, H, Hkv, dh, flash, (cudaStream_t)stream, &g_init_error);
 }
-
-extern "C" __attribute__((visibility("default"))) int dlm_debug_pair(long long* out) { return (int)cudaMemcpyFromSymbol(out, dlm::g_pair_dbg, sizeof(long long) * 80 * 8); }

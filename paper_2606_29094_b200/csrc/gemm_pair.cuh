@@ -63,7 +63,7 @@ constexpr int kPairAccCols = 256;       // TMEM columns per accumulator stage
 
 __host__ __device__ inline int gemm_pair_stage_bytes(int bn) { return kATileBytes + bn * 64; }   // A 128x64 + W (bn/2)x64
 constexpr int kPairEpiStageBytes = 4 * 2 * 4096;      // per epilogue warp: two swizzled 32 x 32 fp32 tiles (coalescing stage)
-__host__ inline int gemm_pair_smem_bytes(int bn, int stages) { return stages * gemm_pair_stage_bytes(bn) + 1024 + 512 + kPairEpiStageBytes; }
+__host__ inline int gemm_pair_smem_bytes(int bn, int stages) { return stages * gemm_pair_stage_bytes(bn) + 1024 + 1024 + kPairEpiStageBytes; }
 
 namespace ptx {
 __device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
@@ -120,6 +120,18 @@ __device__ __forceinline__ void umma_bf16_pair_lo(uint32_t tmem_d, uint32_t a_lo
       ::"r"(tmem_d), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(accumulate), "r"(kDescHiSw128)
       : "memory");
 }
+// Bulk tensor store / reduce-add of one shared-memory box to global memory (async proxy, bulk-group completion).
+__device__ __forceinline__ void tma_store_3d(const void* tmap, uint32_t src_smem, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"(tmap), "r"(src_smem), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_3d(const void* tmap, uint32_t src_smem, int c0, int c1, int c2) {
+  asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"(tmap), "r"(src_smem), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
 // arrive (once) on the barrier at this shared-memory offset in BOTH CTAs of the pair when the MMAs issued so far are done
 __device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
@@ -128,7 +140,6 @@ __device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
 }
 }  // namespace ptx
 
-__device__ long long g_pair_dbg[80 * 8];
 struct PairTile { int m_blk, n_blk; };
 __device__ __forceinline__ PairTile pair_tile(int t, int m_tiles, int n_tiles, int panel) {
   const int pw = panel * n_tiles;
@@ -143,7 +154,8 @@ __device__ __forceinline__ PairTile pair_tile(int t, int m_tiles, int n_tiles, i
 
 template <int EPI>
 __global__ void __launch_bounds__(kPairThreads, 1)
-gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const GemmPairParams p) {
+gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CUtensorMap mapC,
+                 const GemmPairParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const int BN = p.bn;
@@ -155,7 +167,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
   const uint32_t tmem_full_bar = bar_base + 16u * stages;                      // [2], per CTA (multicast commit)
   const uint32_t tmem_empty_bar = tmem_full_bar + 16u;                         // [2], used in the leader
   const uint32_t tmem_ptr_addr = tmem_empty_bar + 16u;
-  const uint32_t epi_stage = bar_base + 512u;                                  // kPairEpiStageBytes, 128-byte aligned
+  const uint32_t epi_stage = bar_base + 1024u;                                 // kPairEpiStageBytes, 1024-byte aligned (TMA 128-byte swizzle)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = ptx::cluster_ctarank();
@@ -165,7 +177,6 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
   const int total_tiles = p.m_tiles * p.n_tiles_n;
   const int total_units = total_tiles * p.splits;      // unit u: tile u % total_tiles, K split u / total_tiles
 
-  const long long t_entry = clock64();
   ptx::pdl_launch_dependents();
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&mapA);
@@ -271,7 +282,6 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
       const int row = tl.m_blk * 256 + (int)rank * 128 + quarter * 32 + lane;
       const bool row_ok = row < p.M;
       ptx::mbar_wait(tmem_full_bar + 8u * as, aph);
-      if (leader && lane == 0) g_pair_dbg[cluster * 8 + (warp - 2)] = clock64() - t_entry;
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + as * kPairAccCols;
       uint32_t r[32];
@@ -295,58 +305,53 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
       };
       const int row_w0 = tl.m_blk * 256 + (int)rank * 128 + quarter * 32;       // first row of this warp's quarter
       const int t_rr = lane >> 3, t_c4 = (lane & 7) * 4;                         // transposed view: row 4 i + t_rr, columns t_c4 .. t_c4 + 3
-      if (EPI == EPI_F32 || EPI == EPI_RESID || EPI == EPI_BF16) {
+      if (EPI == EPI_F32 || EPI == EPI_RESID) {
+        // fp32 outputs leave through TMA: the chunk is staged (swizzled as the output map expects) and one lane issues a bulk
+        // tensor store -- or, for the residual stream, a bulk REDUCE-ADD (x += acc happens in L2: no read of x by the SM, and
+        // exactly one add per element, so the result is deterministic).  TMA clips rows >= M and columns >= N.
         const int n0 = tl.n_blk * BN, nch = BN / 32;
-        // per-lane base of the transposed view, hoisted: (row 4 i + t_rr, column n0 + 32 c + t_c4) = obase + i * 4 ldc + 32 c
-        const long long obase = (long long)(u / total_tiles) * p.split_stride + (long long)(row_w0 + t_rr) * p.ldc + n0 + t_c4;
-        float4 xq[2][8];                                                           // residual rows, one chunk ahead
-        auto ldx = [&](int c, float4 (&dst)[8]) {
-          if (EPI == EPI_RESID && n0 + c * 32 + 32 <= p.N) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const int grow = row_w0 + 4 * i + t_rr;
-              if (grow < p.M) dst[i] = *reinterpret_cast<const float4*>(p.out_f32 + obase + (long long)i * 4 * p.ldc + c * 32);
-            }
+        for (int c = 0; c < nch; ++c) {
+          const int b = c & 1;
+          if (c >= 2) {                                                            // the bulk op that last read this buffer
+            if (lane == 0) ptx::bulk_wait_read<1>();
           }
-        };
-        ldx(0, xq[0]);
-        for (int c0 = 0; c0 < nch; c0 += 2) {
+          __syncwarp();
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+          stg_write(b, r);
+          ptx::fence_proxy_async();
+          __syncwarp();
+          if (lane == 0 && n0 + c * 32 < p.N && row_w0 < p.M) {
+            if (EPI == EPI_RESID) ptx::tma_reduce_add_3d(&mapC, stg + b * 4096, n0 + c * 32, row_w0, 0);
+            else ptx::tma_store_3d(&mapC, stg + b * 4096, n0 + c * 32, row_w0, u / total_tiles);
+          }
+          if (lane == 0) ptx::bulk_commit();
+        }
+        if (lane == 0) ptx::bulk_wait_read<0>();                                   // the stage is reused by the next tile
+        __syncwarp();
+      } else if (EPI == EPI_BF16) {
+        const int n0 = tl.n_blk * BN, nch = BN / 32;
+        const long long obase = (long long)(row_w0 + t_rr) * p.ldc + n0 + t_c4;   // transposed view, hoisted
+        for (int c = 0; c < nch; ++c) {
+          __syncwarp();
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+          stg_write(0, r);
+          __syncwarp();
+          const int col0 = n0 + c * 32;
+          float4 v[8];
 #pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const int c = c0 + k;
-            if (c < nch) {                                                         // warp-uniform
-              __syncwarp();
-              ptx::tmem_ld_32x32(taddr + c * 32, r);
-              if (c + 1 < nch) ldx(c + 1, xq[k ^ 1]);
-              ptx::tmem_ld_wait();
-              stg_write(0, r);
-              __syncwarp();
-              const int col0 = n0 + c * 32;
-              const bool full = col0 + 32 <= p.N;
+          for (int i = 0; i < 8; ++i) v[i] = stg_read(0, i);
 #pragma unroll
-              for (int i = 0; i < 8; ++i) {
-                const int grow = row_w0 + 4 * i + t_rr;
-                float4 v = stg_read(0, i);
-                if (grow >= p.M || col0 + t_c4 >= p.N) continue;
-                if (EPI == EPI_BF16) {
-                  bf16* o = p.out_bf16 + obase + (long long)i * 4 * p.ldc + c * 32;
-                  if (full) {
-                    *reinterpret_cast<uint2*>(o) = make_uint2(pack_bf16(v.x, v.y), pack_bf16(v.z, v.w));
-                  } else {
-                    const float e[4] = {v.x, v.y, v.z, v.w};
-                    for (int q = 0; q < 4; ++q) if (col0 + t_c4 + q < p.N) o[q] = __float2bfloat16_rn(e[q]);
-                  }
-                } else {
-                  float* o = p.out_f32 + obase + (long long)i * 4 * p.ldc + c * 32;
-                  if (full) {
-                    if (EPI == EPI_RESID) { const float4 x = xq[k][i]; v.x += x.x; v.y += x.y; v.z += x.z; v.w += x.w; }
-                    *reinterpret_cast<float4*>(o) = v;
-                  } else {
-                    const float e[4] = {v.x, v.y, v.z, v.w};
-                    for (int q = 0; q < 4; ++q) if (col0 + t_c4 + q < p.N) o[q] = (EPI == EPI_RESID) ? o[q] + e[q] : e[q];
-                  }
-                }
-              }
+          for (int i = 0; i < 8; ++i) {
+            const int grow = row_w0 + 4 * i + t_rr;
+            if (grow >= p.M || col0 + t_c4 >= p.N) continue;
+            bf16* o = p.out_bf16 + obase + (long long)i * 4 * p.ldc + c * 32;
+            if (col0 + t_c4 + 4 <= p.N) {
+              *reinterpret_cast<uint2*>(o) = make_uint2(pack_bf16(v[i].x, v[i].y), pack_bf16(v[i].z, v[i].w));
+            } else {
+              const float e[4] = {v[i].x, v[i].y, v[i].z, v[i].w};
+              for (int q = 0; q < 4; ++q) if (col0 + t_c4 + q < p.N) o[q] = __float2bfloat16_rn(e[q]);
             }
           }
         }
@@ -467,13 +472,13 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
           *reinterpret_cast<int4*>(p.part + (long long)row * p.n_tiles + tl.n_blk) = *reinterpret_cast<int4*>(&o);
         }
       }
-      if (leader && lane == 0) g_pair_dbg[cluster * 8 + 4 + (warp - 2)] = clock64() - t_entry;
       // this warp's quarter of the accumulator stage has been read: let the leader's MMA issuer reuse it
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive_cluster(te_leader + 8u * as);
     }
   }
+  if ((EPI == EPI_F32 || EPI == EPI_RESID) && warp >= 2 && lane == 0) ptx::bulk_wait<0>();   // bulk stores / reductions have landed
   ptx::tc_fence_before();
   __syncthreads();
   ptx::cluster_sync();          // no CTA of the pair frees TMEM / leaves while its peer may still signal it
