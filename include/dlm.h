@@ -128,6 +128,21 @@ DLM_API int  dlm_request_remove(dlm_ctx*, int32_t req);
 DLM_API int  dlm_request_tokens(dlm_ctx*, int32_t req, int32_t* out, int32_t cap);     /* returns S or error    */
 DLM_API int  dlm_request_info(dlm_ctx*, int32_t req, int32_t* cur_block, int32_t* cache_valid, int32_t* n_masked);
 
+/* Migration ("a request may be migrated to another instance only at recompute steps",
+ * P:365 the executor command carries the request's tokens).  dlm_request_export serialises what a request is apart
+ * from its K/V cache -- prompt||generation ids, block length, threshold, completed-step count and the per-position
+ * confidence state of the Step Predictor features -- into a caller-owned HOST blob and returns the blob size in
+ * bytes (nothing is written when cap_bytes is smaller; call with blob = NULL to size it).  Layout, little-endian:
+ * int32 {magic 0x524D4C44 "DLMR", version 1, prompt_len, gen_len, block_len, steps_done, cache_valid_at_export,
+ * reserved}, float threshold, int32 reserved, int32 tokens[S], float conf_state[S].  dlm_request_import registers
+ * the blob as a new request of ctx (which may be another context, on another GPU, of the same arch): the cache is
+ * INVALID, so the next step must be dlm_refresh_step, which recomputes every K/V.  Exported at a block's first step
+ * (cache invalid there anyway) the imported request continues bit-identically; exported mid-block it continues with
+ * a fresh cache instead of the approximate one (legal, G19, but not the same trajectory).  Errors: DLM_E_ARG for a
+ * malformed blob or ids outside the vocabulary, DLM_E_CAPACITY as dlm_request_add; nothing is applied on error. */
+DLM_API int64_t dlm_request_export(dlm_ctx*, int32_t req, void* blob, int64_t cap_bytes);
+DLM_API int  dlm_request_import(dlm_ctx*, const void* blob, int64_t bytes, int32_t* out_req);
+
 /* Recompute step: all S_r positions of every request in the batch pass through the model,
  * every layer's K (post-RoPE) and V are written to the request's pages, then the current block (the
  * lowest-index block holding a MASK) is unmasked with the batch's / stored threshold.  Legal at any time;

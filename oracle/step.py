@@ -65,6 +65,14 @@ class Request:
         self.conf_state = np.zeros(self.G, dtype=np.float64)   # per output position: last confidence seen while masked
         self.steps_done = 0                                    # completed (non-dry) denoising steps
 
+    def migrate(self) -> "Request":
+        """The request as another instance receives it ("migrated ... only at recompute steps"; P:365 the command
+        carries the request's tokens): everything except the K/V cache, which the receiver recomputes."""
+        r = Request(self.arch, self.tokens[:self.P], self.G, self.B, self.threshold, tokens=self.tokens)
+        r.conf_state = self.conf_state.copy()
+        r.steps_done = self.steps_done
+        return r
+
     def masked(self) -> np.ndarray:
         return self.tokens == self.arch.mask_id
 

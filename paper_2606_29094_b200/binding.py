@@ -92,6 +92,9 @@ def lib() -> C.CDLL:
         L.dlm_request_remove.argtypes = [vp, i32]
         L.dlm_request_tokens.argtypes = [vp, i32, C.POINTER(i32), i32]
         L.dlm_request_info.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
+        L.dlm_request_export.argtypes = [vp, i32, vp, i64]
+        L.dlm_request_export.restype = i64
+        L.dlm_request_import.argtypes = [vp, vp, i64, C.POINTER(i32)]
         L.dlm_refresh_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(_Result)]
         L.dlm_cached_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(f32), C.POINTER(_Result)]
         L.dlm_mixed_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(f32), C.POINTER(_Result)]
@@ -253,6 +256,19 @@ class Engine:
         a, b, c = C.c_int32(), C.c_int32(), C.c_int32()
         self._check(lib().dlm_request_info(self._h, req, C.byref(a), C.byref(b), C.byref(c)))
         return {"cur_block": a.value, "cache_valid": bool(b.value), "n_masked": c.value}
+
+    def export_request(self, req: int) -> bytes:
+        """The request without its K/V cache, as the host blob include/dlm.h describes (migration)."""
+        need = self._check(lib().dlm_request_export(self._h, req, None, 0))
+        buf = C.create_string_buffer(need)
+        self._check(lib().dlm_request_export(self._h, req, buf, need))
+        return buf.raw
+
+    def import_request(self, blob: bytes) -> int:
+        out = C.c_int32(-1)
+        buf = C.create_string_buffer(blob, len(blob))
+        self._check(lib().dlm_request_import(self._h, buf, len(blob), C.byref(out)))
+        return out.value
 
     # -- steps --
     def _step(self, kind: int, reqs: Sequence[int], thresholds, dry_run: bool, features: bool = False) -> StepResult:

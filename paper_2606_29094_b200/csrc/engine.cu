@@ -925,6 +925,59 @@ extern "C" int dlm_request_tokens(dlm_ctx* c, int32_t r, int32_t* out, int32_t c
   return q->S;
 }
 
+// ---- migration blob (include/dlm.h): header of 10 words, tokens[S], conf_state[S] ----
+namespace {
+constexpr int32_t kBlobMagic = 0x524D4C44, kBlobVersion = 1, kBlobHeaderWords = 10;
+}
+
+extern "C" int64_t dlm_request_export(dlm_ctx* c, int32_t r, void* blob, int64_t cap) {
+  Req* q = get_req(c, r);
+  if (!q) { if (c) set_err(&c->err, "dlm_request_export: bad request %d", r); return DLM_E_ARG; }
+  const int64_t need = (int64_t)kBlobHeaderWords * 4 + (int64_t)q->S * 8;
+  if (!blob || cap < need) return need;
+  int32_t* h = static_cast<int32_t*>(blob);
+  h[0] = kBlobMagic; h[1] = kBlobVersion; h[2] = q->P; h[3] = q->G; h[4] = q->B; h[5] = q->steps_done;
+  h[6] = q->cache_valid ? 1 : 0; h[7] = 0;
+  memcpy(&h[8], &q->tau, 4); h[9] = 0;
+  CU_TRY(&c->err, cudaMemcpyAsync(h + kBlobHeaderWords, c->tokens + (size_t)r * c->a.max_seq, (size_t)q->S * 4, cudaMemcpyDeviceToHost, c->st));
+  CU_TRY(&c->err, cudaMemcpyAsync(h + kBlobHeaderWords + q->S, c->conf_state + (size_t)r * c->a.max_seq, (size_t)q->S * 4, cudaMemcpyDeviceToHost, c->st));
+  CU_TRY(&c->err, cudaStreamSynchronize(c->st));
+  return need;
+}
+
+extern "C" int dlm_request_import(dlm_ctx* c, const void* blob, int64_t bytes, int32_t* out_req) {
+  if (!c) return DLM_E_ARG;
+  const int32_t* h = static_cast<const int32_t*>(blob);
+  if (!blob || !out_req || bytes < (int64_t)kBlobHeaderWords * 4 || h[0] != kBlobMagic || h[1] != kBlobVersion) {
+    set_err(&c->err, "dlm_request_import: not a version-%d request blob", kBlobVersion);
+    return DLM_E_ARG;
+  }
+  const int P = h[2], G = h[3], B = h[4], steps = h[5];
+  if (P < 0 || G <= 0 || B <= 0 || steps < 0 || bytes != (int64_t)kBlobHeaderWords * 4 + ((int64_t)P + G) * 8) {
+    set_err(&c->err, "dlm_request_import: header (P=%d G=%d B=%d) does not match %lld bytes", P, G, B, (long long)bytes);
+    return DLM_E_ARG;
+  }
+  const int S = P + G;
+  float tau; memcpy(&tau, &h[8], 4);
+  const int32_t* tok = h + kBlobHeaderWords;
+  for (int i = 0; i < S; ++i)
+    if (tok[i] < 0 || tok[i] >= c->a.vocab || (i < P && tok[i] == c->a.mask_id)) { set_err(&c->err, "dlm_request_import: bad id at %d", i); return DLM_E_ARG; }
+  int32_t slot = -1;
+  int rc = dlm_request_add(c, tok, P, G, B, tau, &slot);
+  if (rc != DLM_OK) return rc;
+  rc = dlm_request_set_tokens(c, slot, tok, S, 0);
+  if (rc == DLM_OK) {
+    cudaError_t e = cudaMemcpyAsync(c->conf_state + (size_t)slot * c->a.max_seq, tok + S, (size_t)S * 4, cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) { set_err(&c->err, "dlm_request_import: %s", cudaGetErrorString(e)); rc = DLM_E_CUDA; }
+  }
+  if (rc != DLM_OK) { dlm_request_remove(c, slot); return rc; }
+  c->reqs[slot].steps_done = steps;
+  c->reqs[slot].cache_valid = false;
+  *out_req = slot;
+  return DLM_OK;
+}
+
 extern "C" int dlm_request_info(dlm_ctx* c, int32_t r, int32_t* cur_block, int32_t* cache_valid, int32_t* n_masked) {
   Req* q = get_req(c, r);
   if (!q) { if (c) set_err(&c->err, "dlm_request_info: bad request %d", r); return DLM_E_ARG; }

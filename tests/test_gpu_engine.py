@@ -30,7 +30,7 @@ def _gpu_hidden_block_rows(pkg, eng, rid, arch, o, refresh):
     return x[o.block_lo:o.block_lo + len(o.conf)] if refresh else x
 
 
-def _run_parity(arch, seed, spec, max_steps, teacher_forced, hid_tol, lse_tol, simple=False, flash=True, kv_page_tokens=64):
+def _run_parity(arch, seed, spec, max_steps, teacher_forced, hid_tol, lse_tol, simple=False, flash=True, kv_page_tokens=64, use_cache=True):
     """Step the GPU engine and the oracle side by side; returns counters.  teacher_forced: GPU tokens are reset
     to the oracle's before every step (cache kept)."""
     pkg = _pkg()
@@ -50,7 +50,7 @@ def _run_parity(arch, seed, spec, max_steps, teacher_forced, hid_tol, lse_tol, s
         if eng.info(rid)["cache_valid"] != oreq.cache_valid:      # a resync moved one side across a block boundary
             oreq.cache_valid = False
             eng.set_tokens(rid, oreq.tokens.astype(np.int32), keep_cache=False)
-        refresh = not oreq.cache_valid
+        refresh = not (use_cache and oreq.cache_valid)        # use_cache = False: the paper's no-cache mode (App. E)
         lo, hi = oreq.block_range(oreq.current_block())
         masked_before = oreq.tokens[lo:hi] == arch.mask_id
         o = ostep.refresh_step(oreq, wts) if refresh else ostep.cached_step(oreq, wts)
@@ -83,6 +83,73 @@ def test_c1_fp32_free_running_trajectory():
     s = _run_parity(ARCH_C1, WEIGHT_SEED["C1"], spec, 10 ** 6, teacher_forced=False, hid_tol=1e-4, lse_tol=1e-4)
     print("P-A", s)
     assert s["mismatch"] == 0 and s["steps"] >= 2 * 1 and s["steps"] <= 64
+
+
+def test_c1_fp32_no_cache_mode_free_running_trajectory():
+    """P-A without approximate caching (NEXT-2; App. E): every step is a recompute step."""
+    spec = workload_c1()[0]
+    s = _run_parity(ARCH_C1, WEIGHT_SEED["C1"], spec, 10 ** 6, teacher_forced=False, hid_tol=1e-4, lse_tol=1e-4, use_cache=False)
+    print("P-A no-cache", s)
+    assert s["mismatch"] == 0 and 2 <= s["steps"] <= 64
+
+
+@pytest.mark.parametrize("bf16_model", [False, True])
+def test_request_migration_between_contexts(bf16_model):
+    """NEXT-2 ("migrated ... only at recompute steps"): a request exported at a block's first step and
+    imported into ANOTHER context continues bit-identically to the one that stayed (commits, confidences, lse, Step
+    Predictor features); the blob has the layout include/dlm.h states; the imported request has no cache; malformed
+    blobs are refused and leave the context untouched.  Mirrors oracle.step.Request.migrate."""
+    pkg = _pkg()
+    a = ARCH_C1.replace(weight_dtype=1) if bf16_model else ARCH_C1
+    rng = np.random.default_rng(91)
+    prompt = random_tokens(rng, 37, a.vocab, a.mask_id)
+    A = pkg.Engine(a, WEIGHT_SEED["C1"], max_requests=2, max_seq=128, max_block=16)
+    Bn = pkg.Engine(a, WEIGHT_SEED["C1"], max_requests=2, max_seq=128, max_block=16)
+    ra = A.add_request(prompt, 48, 16, 0.04)
+    steps0 = 0
+    while A.info(ra)["cur_block"] == 0:
+        A.mixed_step([ra])
+        steps0 += 1
+    assert not A.info(ra)["cache_valid"]
+    blob = A.export_request(ra)
+    S = 37 + 48
+    hdr = np.frombuffer(blob[:40], np.int32)
+    assert len(blob) == 40 + 8 * S and hdr[0] == 0x524D4C44 and hdr[1] == 1
+    assert hdr[2:7].tolist() == [37, 48, 16, steps0, 0]
+    assert np.frombuffer(blob[32:36], np.float32)[0] == np.float32(0.04)
+    assert np.array_equal(np.frombuffer(blob[40:40 + 4 * S], np.int32), A.tokens(ra))
+    rb = Bn.import_request(blob)
+    assert np.array_equal(Bn.tokens(rb), A.tokens(ra)) and Bn.info(rb) == A.info(ra)
+    with pytest.raises(pkg.DlmError):
+        Bn.cached_step([rb])                                   # no cache on the receiver
+    n = 0
+    while A.info(ra)["n_masked"]:
+        ga, gb = A.mixed_step([ra], features=True), Bn.mixed_step([rb], features=True)
+        assert ga.commits[0] == gb.commits[0] and len(ga.commits[0]) >= 1
+        assert np.array_equal(ga.lse[0], gb.lse[0]) and np.array_equal(ga.row_conf[0], gb.row_conf[0])
+        assert np.array_equal(ga.features[0], gb.features[0])
+        n += 1
+    assert n >= 2 and np.array_equal(A.tokens(ra), Bn.tokens(rb)) and Bn.info(rb)["n_masked"] == 0
+    # a mid-block export records that a cache existed; the importer still starts from a refresh
+    r2 = A.add_request(prompt, 48, 16, 1.5)
+    A.mixed_step([r2]), A.mixed_step([r2])
+    b2 = A.export_request(r2)
+    assert np.frombuffer(b2[:40], np.int32)[6] == 1
+    r3 = Bn.import_request(b2)
+    assert not Bn.info(r3)["cache_valid"] and Bn.info(r3)["n_masked"] == 46
+    # malformed blobs
+    before = Bn.info(r3)
+    for bad in (b2[:-4], b"\0" * len(b2), b2[:40]):
+        with pytest.raises(pkg.DlmError):
+            Bn.import_request(bad)
+    tok_bad = bytearray(b2)
+    tok_bad[40:44] = np.int32(a.vocab).tobytes()
+    with pytest.raises(pkg.DlmError):
+        Bn.import_request(bytes(tok_bad))
+    assert Bn.info(r3) == before
+    Bn.remove_request(r3)
+    assert Bn.import_request(b2) == r3                          # slot and pages were not leaked by the refusals
+    A.close(), Bn.close()
 
 
 @pytest.mark.parametrize("tau,steps_per_block", [(1.5, 32), (0.0, 1)])

@@ -129,6 +129,31 @@ def test_cached_step_needs_valid_cache_and_block_completion_invalidates(tiny_arc
         step.cached_step(r, wts)
 
 
+@pytest.mark.parametrize("tau", [0.04, 1.5])
+def test_migration_at_a_recompute_step_keeps_the_trajectory(tiny_arch, tau):
+    """at a block's first step the cache is invalid anyway, so a request that drops its cache there (migration)
+    continues exactly as the one that stayed; dropped mid-block it takes a fresh cache instead of the stale one, which
+    is a different (L > 1) computation."""
+    wts = W.Weights(tiny_arch, 48)
+    stay, move = _req(tiny_arch, tau=tau, seed=9), _req(tiny_arch, tau=tau, seed=9)
+    while move.current_block() == 0:
+        step.next_step(stay, wts), step.next_step(move, wts)
+    assert not move.cache_valid
+    moved = move.migrate()
+    assert moved.cache is None and not moved.cache_valid and moved.steps_done == move.steps_done
+    ha, hb = step.run(stay, wts), step.run(moved, wts)
+    assert [[(c.pos, c.tok, c.conf) for c in h.commits] for h in ha] == [[(c.pos, c.tok, c.conf) for c in h.commits] for h in hb]
+    assert np.array_equal(stay.tokens, moved.tokens)
+    assert np.array_equal(step.predictor_features(stay), step.predictor_features(moved))
+    # mid-block: the receiver's first step is a refresh (fresh K/V everywhere), the stayer's a cached one
+    s2 = _req(tiny_arch, tau=1.5, seed=9)
+    step.next_step(s2, wts), step.next_step(s2, wts)
+    assert s2.cache_valid
+    m2 = s2.migrate()
+    a, b = step.next_step(s2, wts), step.next_step(m2, wts)
+    assert (a.kind, b.kind) == ("cached", "refresh") and np.abs(a.conf - b.conf).max() > 1e-12
+
+
 def test_per_step_threshold_override(tiny_arch):
     """the threshold may change at every step."""
     wts = W.Weights(tiny_arch, 47)
