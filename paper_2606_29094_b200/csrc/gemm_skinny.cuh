@@ -37,6 +37,7 @@ struct SkinnyParams {
   bf16* out_bf16;         // SK_SWIGLU:  [T][ldc]
   long long ldc;
   unsigned long long w_policy;
+  int w_box;              // 0: W row-major (2-D map); else tiled storage, rows per TMA box (ptx::tma_load_w_tiled)
 };
 
 constexpr int kSkThreads = 192;
@@ -93,7 +94,14 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
         const uint32_t sw = base + s * stage_bytes;
         const int kcol = (kb0 + kb) * 64;
         ptx::mbar_expect_tx(full_bar(s), tx);
-        if (EPI == SK_SWIGLU) {
+        if (p.w_box) {
+          if (EPI == SK_SWIGLU) {
+            ptx::tma_load_w_tiled(sw, &mapW, kb0 + kb, tile * 64, 64, p.w_box, full_bar(s), p.w_policy);
+            ptx::tma_load_w_tiled(sw + 64 * 128, &mapW, kb0 + kb, p.up_row0 + tile * 64, 64, p.w_box, full_bar(s), p.w_policy);
+          } else {
+            ptx::tma_load_w_tiled(sw, &mapW, kb0 + kb, tile * 128, 128, p.w_box, full_bar(s), p.w_policy);
+          }
+        } else if (EPI == SK_SWIGLU) {
           ptx::tma_load_2d(sw, &mapW, kcol, tile * 64, full_bar(s), p.w_policy);
           ptx::tma_load_2d(sw + 64 * 128, &mapW, kcol, p.up_row0 + tile * 64, full_bar(s), p.w_policy);
         } else {

@@ -30,6 +30,25 @@ __global__ void init_weight_kernel(TW* __restrict__ w, long long n, unsigned lon
   }
 }
 
+// Same values into tiled storage (engine.cu make_tmap_w_tiled): element (row, col) of a [rows, cols] matrix whose first row
+// sits at storage row row0 goes to tile (col / 64, row / 128); rb_pad = padded storage rows of the whole matrix / 128.  The value depends on the logical
+// index row * cols + col only, so the weights are those of Definition W whatever the layout.
+__host__ __device__ inline long long w_tiled_index(long long row, long long col, long long rb_pad) {
+  return (((col >> 6) * rb_pad + (row >> 7)) << 13) + ((row & 127) << 6) + (col & 63);
+}
+template <typename TW>
+__global__ void init_weight_tiled_kernel(TW* __restrict__ w, long long rows, long long cols, long long row0, long long rb_pad,
+                                         unsigned long long key, float c) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long stride = (long long)gridDim.x * blockDim.x;
+  const long long n = rows * cols;
+  for (; i < n; i += stride) {
+    unsigned long long h = mix64(key + DLM_GOLD * (unsigned long long)(i + 1));
+    int s = (int)(h & 0xFFFF) + (int)((h >> 16) & 0xFFFF) + (int)((h >> 32) & 0xFFFF) + (int)(h >> 48) - 131070;
+    w[w_tiled_index(row0 + i / cols, i % cols, rb_pad)] = from_f32<TW>(__fmul_rn((float)s, c));
+  }
+}
+
 // RoPE table: cos/sin(pos * theta^(-2i/d_h)) computed in double, stored fp32. [max_seq, d_h/2]
 __global__ void init_rope_kernel(float* __restrict__ cs, float* __restrict__ sn, int max_seq, int half, double theta) {
   int idx = blockIdx.x * blockDim.x + threadIdx.x;

@@ -75,6 +75,24 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const void* tmap,
       : "memory");
 }
 
+// Tiled weight storage (engine.cu make_tmap_w_tiled): [K/64][rows/128][128 rows][64 columns] bf16, every 128 x 64 tile one
+// contiguous 16 KB run in HBM.  As a 4-D tensor (k_in, r_in, r_blk, k_blk) a box {64, w_box, 1, 1} lands in shared memory
+// exactly as the 2-D box {64, w_box} of the row-major matrix does (128-byte rows, 128-byte swizzle).
+__device__ __forceinline__ void tma_load_4d(uint32_t dst_smem, const void* tmap, int c0, int c1, int c2, int c3, uint32_t bar,
+                                            uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
+      ::"r"(dst_smem), "l"(tmap), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(policy)
+      : "memory");
+}
+// n_rows weight rows from `row` on, K block kb, in boxes of w_box rows (w_box divides 128, row and n_rows)
+__device__ __forceinline__ void tma_load_w_tiled(uint32_t dst_smem, const void* tmap, int kb, int row, int n_rows, int w_box,
+                                                 uint32_t bar, uint64_t policy) {
+  for (int r = 0; r < n_rows; r += w_box)
+    tma_load_4d(dst_smem + (uint32_t)r * 128u, tmap, 0, (row + r) & 127, (row + r) >> 7, kb, bar, policy);
+}
+
 // ---------------- tcgen05 ----------------
 __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
