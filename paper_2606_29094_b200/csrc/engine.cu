@@ -669,7 +669,9 @@ static int norm_threads(int d) { return std::min(1024, ((d / 4) + 31) / 32 * 32)
 template <typename TE>
 static void launch_rmsnorm(dlm_ctx* c, TE* u, float* x, const int* row_src, int rows, int d, float eps, const float* part, int n_part,
                            long long part_stride, bool pdl) {
-  if (rows >= 1024)
+  if (rows >= 1024 && d <= 4096)        // register-resident row: 3.46 -> 2.00 ms per C3 mixed step; slower below ~1000 rows
+    launch_k(rmsnorm_warp_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride);
+  else if (rows >= 1024)
     launch_k(rmsnorm_rows_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride);
   else
   {

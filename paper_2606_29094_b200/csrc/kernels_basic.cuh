@@ -207,6 +207,67 @@ __global__ void __launch_bounds__(512) rmsnorm_rows_kernel(TA* __restrict__ u, f
   }
 }
 
+// Same result (same per-lane summation order), one pass: d <= 4096, the whole row lives in the warp's registers (32 float4 per
+// lane, every load of a row issued before the first use), so x is read once and the second pass costs no memory traffic.
+template <typename TA>
+__global__ void __launch_bounds__(128) rmsnorm_warp_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
+                                                           int n_rows, int d, float eps, const float* __restrict__ part, int n_part,
+                                                           long long part_stride) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int r = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (r >= n_rows) return;
+  const int lane = threadIdx.x & 31;
+  const long long sr = row_src ? row_src[r] : r;
+  float4* xr = reinterpret_cast<float4*>(x + sr * d);
+  const int nvec = d >> 2;
+  float4 a[32];
+#pragma unroll
+  for (int k = 0; k < 32; ++k) {
+    const int i = k * 32 + lane;
+    a[k] = i < nvec ? xr[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  if (n_part > 0) {
+    const float4* pr = reinterpret_cast<const float4*>(part + sr * d);
+    const long long ps4 = part_stride >> 2;
+    for (int s = 0; s < n_part; ++s) {
+#pragma unroll
+      for (int k = 0; k < 32; ++k) {
+        const int i = k * 32 + lane;
+        if (i < nvec) {
+          const float4 q = __ldcg(pr + s * ps4 + i);
+          a[k].x += q.x; a[k].y += q.y; a[k].z += q.z; a[k].w += q.w;
+        }
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      const int i = k * 32 + lane;
+      if (i < nvec) xr[i] = a[k];
+    }
+  }
+  float ss = 0.f;
+#pragma unroll
+  for (int k = 0; k < 32; ++k)
+    if (k * 32 + lane < nvec) ss += a[k].x * a[k].x + a[k].y * a[k].y + a[k].z * a[k].z + a[k].w * a[k].w;
+  ss = warp_sum(ss);
+  const float rs = rsqrtf(ss / (float)d + eps);
+  TA* ur = u + (long long)r * d;
+#pragma unroll
+  for (int k = 0; k < 32; ++k) {
+    const int i = k * 32 + lane;
+    if (i >= nvec) continue;
+    if (sizeof(TA) == 2) {
+      __nv_bfloat162 lo = __floats2bfloat162_rn(a[k].x * rs, a[k].y * rs), hi = __floats2bfloat162_rn(a[k].z * rs, a[k].w * rs);
+      uint2 w;
+      w.x = *reinterpret_cast<uint32_t*>(&lo); w.y = *reinterpret_cast<uint32_t*>(&hi);
+      *reinterpret_cast<uint2*>(reinterpret_cast<bf16*>(ur) + 4 * i) = w;
+    } else {
+      *reinterpret_cast<float4*>(reinterpret_cast<float*>(ur) + 4 * i) = make_float4(a[k].x * rs, a[k].y * rs, a[k].z * rs, a[k].w * rs);
+    }
+  }
+}
+
 // x[row] += sum of split-K partials (debug-dump mode only: makes x complete right after the projection)
 __global__ void add_partials_kernel(float* __restrict__ x, const float* __restrict__ part, int n_part, long long part_stride, long long n) {
   pdl_launch_dependents();
