@@ -432,7 +432,7 @@ static void skinny_plan(int T, int N, int K, int epi, int force_splits, SkinnyPa
   p->splits = (num_kb + p->kb_per_split - 1) / p->kb_per_split;
   p->T = T; p->N = N; p->K = K;
   p->tpad = (T + 31) / 32 * 32;
-  const int budget = 100 * 1024 - (epi == SK_SWIGLU ? 32 * 65 * 4 : 0);
+  const int budget = 100 * 1024 - (epi == SK_SWIGLU ? 32 * 65 * 4 : 0);      // two CTAs per SM; 84 / 72 / 56 KB rings measured 1 / 3 / 14 % slower
   p->stages = std::max(2, std::min(std::min(p->kb_per_split, 8), budget / skinny_stage_bytes(p->tpad)));
   p->w_policy = DLM_L2_EVICT_FIRST;
 }
