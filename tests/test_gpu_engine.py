@@ -559,6 +559,31 @@ def test_c2_full_size_sampled_stages_and_properties():
     clear = margin >= 1e-3
     assert np.array_equal(dump_r.row_tok[0][clear], tok_o[clear])
     assert np.abs(dump_r.row_conf[0] - conf_o).max() < 2e-5 and np.abs(dump_r.lse[0] - lse_o).max() < 1e-4 * np.abs(lse_o).max()
+    # (iv) the CACHED step at full size (T = 32: weight-streaming GEMMs reading the TILED weight copy, mma.sync attention over
+    # cached K/V): dump == production bit for bit, then every projection of layers 0 and L-1 recomputed by the oracle from the
+    # GPU's own stage inputs on all block rows -- the tiled copy holds Definition W's values in every matrix
+    dump_c = eng.cached_step([rid], dry_run=True)
+    assert np.array_equal(dump_c.lse, prod_c.lse) and np.array_equal(dump_c.row_tok, prod_c.row_tok) and dump_c.commits == prod_c.commits
+    lo = S - spec.gen_len + eng.info(rid)["cur_block"] * Bk
+    bpos = np.arange(lo, lo + Bk).astype(np.float64)
+    for l in (0, arch.n_layers - 1):
+        t = lambda which, w: eng.debug_tensor(rid, l, which, Bk, w).astype(np.float64)
+        x_in, u1, q, attn, x_mid, u2, act, x_out = (t(B.T_X_IN, d), t(B.T_NORM1, d), t(B.T_Q, HQ), t(B.T_ATTN, HQ), t(B.T_X_MID, d),
+                                                    t(B.T_NORM2, d), t(B.T_ACT, F), t(B.T_X_OUT, d))
+        kc = eng.debug_tensor(rid, l, B.T_KCACHE, S, HKV).astype(np.float64)
+        vc = eng.debug_tensor(rid, l, B.T_VCACHE, S, HKV).astype(np.float64)
+        wq, wk, wv = (wts.get(ow.layer_tid(l, s)) for s in (ow.SUB_Q, ow.SUB_K, ow.SUB_V))
+        q_o = omodel.rope((u1 @ wq.T).reshape(Bk, arch.n_heads, arch.head_dim), bpos, arch.rope_theta).reshape(Bk, HQ)
+        k_o = omodel.rope((u1 @ wk.T).reshape(Bk, arch.n_kv_heads, arch.head_dim), bpos, arch.rope_theta).reshape(Bk, HKV)
+        assert bf(q_o, q, 3e-4) and bf(k_o, kc[lo:lo + Bk], 3e-4) and bf(u1 @ wv.T, vc[lo:lo + Bk], 3e-4)
+        a_o = omodel.attention(q.reshape(Bk, arch.n_heads, -1), kc.reshape(S, arch.n_kv_heads, -1), vc.reshape(S, arch.n_kv_heads, -1)).reshape(Bk, HQ)
+        assert np.all(np.abs(a_o - attn) <= np.abs(a_o) * 2 ** -8 + 2e-3 * max(1.0, np.abs(a_o).max()))
+        xm_o = x_in + attn @ wts.get(ow.layer_tid(l, ow.SUB_O)).T
+        assert np.abs(xm_o - x_mid).max() <= 1e-4 * max(1.0, np.abs(xm_o).max())
+        act_o = omodel.silu(u2 @ wts.get(ow.layer_tid(l, ow.SUB_G)).T) * (u2 @ wts.get(ow.layer_tid(l, ow.SUB_U)).T)
+        assert bf(act_o, act, 3e-4)
+        xo_o = x_mid + act @ wts.get(ow.layer_tid(l, ow.SUB_D)).T
+        assert np.abs(xo_o - x_out).max() <= 1e-4 * max(1.0, np.abs(xo_o).max())
     eng.set_option(pkg.OPT_DEBUG_DUMP, 0)
     again = eng.cached_step([rid], dry_run=True)
     assert np.array_equal(again.lse, prod_c.lse)
