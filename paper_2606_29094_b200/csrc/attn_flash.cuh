@@ -256,8 +256,16 @@ static int attn_flash_launch(bf16* out, const bf16* q, const bf16* kv_store, con
   const int q_tiles = (bd.max_q_len * r + kFaBM - 1) / kFaBM;
   const long long items = (long long)q_tiles * g.n_kv_heads * bd.n;
   const int kv_tiles = (bd.max_kv_len + kFaBN - 1) / kFaBN;
+  // Split-KV when the items alone cannot fill the GPU: ~4 K/V tiles (256 positions) per CTA, between one and two CTAs per
+  // SM (measured on single-request cached steps at S = 512 ... 4608: one tile per CTA is all ramp, one CTA per SM starves
+  // long sequences).  No empty split.
   int splits = 1;
-  if (items < 2LL * num_sms) splits = (int)std::min<long long>(kv_tiles, (2LL * num_sms + items - 1) / items);
+  if (items < 2LL * num_sms) {
+    const long long lo = std::max<long long>(1, num_sms / items), hi = (2LL * num_sms + items - 1) / items;
+    const int want = (int)std::min<long long>(kv_tiles, std::max(lo, std::min<long long>(hi, kv_tiles / 4)));
+    const int tiles_per = (kv_tiles + want - 1) / want;
+    splits = (kv_tiles + tiles_per - 1) / tiles_per;
+  }
   splits = std::max(1, std::min(splits, 32));
   FaParams p;
   p.out = out; p.q = q; p.kv_store = kv_store; p.page_table = page_table; p.b = bd; p.g = g; p.layer = layer; p.n_heads = n_heads;
