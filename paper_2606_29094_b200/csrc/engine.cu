@@ -245,7 +245,10 @@ static void plan_pair(int M, int N, int K, int epi, int max_splits, int* bn_out,
   static const int cand_lm[] = {256};
   const int* cand = epi == EPI_SWIGLU ? cand_glu : (epi == EPI_LMHEAD ? cand_lm : cand_std);
   const int nc = epi == EPI_SWIGLU ? 4 : (epi == EPI_LMHEAD ? 1 : 7);
-  const int unit_fixed = 8;                           // epilogue tail + ramp, in K-block units
+  // Cost of a unit in 1/256 K-block units of a 256-wide tile.  Measured with two K blocks per ring stage (4096 x 12288 x 4096,
+  // whole kernel): bn 256 / 192 / 128 -> 1.00 / 0.78 / 0.61 of the 256-wide tile per tile, i.e. ~0.22 + 0.78 bn / 256 (the MMA
+  // time is bn / 2 cycles, the stage hand-off is not free); the fixed part (ramp, exposed epilogue) shrinks with the tile too.
+  auto kb_cost = [](int bn) { return 56 + (200 * bn) / 256; };
   long long best = -1;
   *bn_out = cand[0]; *splits_out = 1;
   for (int sp = 1; sp <= std::max(1, max_splits); ++sp) {
@@ -255,7 +258,7 @@ static void plan_pair(int M, int N, int K, int epi, int max_splits, int* bn_out,
       const int per = epi == EPI_SWIGLU ? cand[i] / 2 : cand[i];
       const long long units = (long long)m_tiles * ((N + per - 1) / per) * sp;
       const long long waves = (units + pairs - 1) / pairs;
-      const long long cost = waves * (kb_per + unit_fixed);
+      const long long cost = waves * ((long long)kb_per * kb_cost(cand[i]) + 8LL * (128 + cand[i] / 2));
       if (best < 0 || cost < best) { best = cost; *bn_out = cand[i]; *splits_out = sp; }
     }
   }
@@ -305,7 +308,7 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
   p.splits = (num_kb + p.kb_per_split - 1) / p.kb_per_split;
   p.split_stride = (long long)M * p.ldc;
   if (splits_out) *splits_out = p.splits;
-  p.stages = std::max(2, std::min(std::min(num_kb, 12), (224 * 1024 - kPairEpiStageBytes) / gemm_pair_stage_bytes(bn)));
+  p.stages = std::max(2, std::min(std::min((num_kb + kPairKbPerStage - 1) / kPairKbPerStage, 12), (224 * 1024 - kPairEpiStageBytes) / gemm_pair_stage_bytes(bn)));
   const int per = epi == EPI_SWIGLU ? bn / 2 : bn;
   p.m_tiles = (M + 255) / 256;
   p.n_tiles_n = (N + per - 1) / per;

@@ -61,7 +61,12 @@ struct GemmPairParams {
 constexpr int kPairThreads = 192;
 constexpr int kPairAccCols = 256;       // TMEM columns per accumulator stage
 
-__host__ __device__ inline int gemm_pair_stage_bytes(int bn) { return kATileBytes + bn * 64; }   // A 128x64 + W (bn/2)x64
+// A ring stage holds kPairKbPerStage 64-wide K blocks: [A k0][A k1][W k0][W k1] (A 128 x 64, W (bn/2) x 64 per block).  The
+// stage hand-off (TMA -> full barrier -> MMA -> commit -> empty barrier -> producer) has a floor of ~300 ns that neither the
+// MMAs nor the loads explain (DESIGN.md section 6 (1)); two K blocks per hand-off halve it per K block.
+constexpr int kPairKbPerStage = 2;
+__host__ __device__ inline int gemm_pair_kb_bytes(int bn) { return kATileBytes + bn * 64; }
+__host__ __device__ inline int gemm_pair_stage_bytes(int bn) { return kPairKbPerStage * gemm_pair_kb_bytes(bn); }
 constexpr int kPairEpiStageBytes = 4 * 2 * 4096;      // per epilogue warp: two swizzled 32 x 32 fp32 tiles (coalescing stage)
 __host__ inline int gemm_pair_smem_bytes(int bn, int stages) { return stages * gemm_pair_stage_bytes(bn) + 1024 + 1024 + kPairEpiStageBytes; }
 
@@ -200,10 +205,19 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     if (lane == 0) {
       // ---------------- TMA producer (both CTAs, one lane) ----------------
       const uint32_t half_rows = (uint32_t)BN / 2;
-      const uint32_t tx_pair = 2u * (kATileBytes + half_rows * 128u);
+      const uint32_t w_bytes = half_rows * 128u;
+      const uint32_t tx_kb = 2u * (kATileBytes + w_bytes);          // both CTAs' bytes of one K block
       auto w_row_of = [&](const PairTile& tl) {
         if (EPI == EPI_SWIGLU) return tl.n_blk * (int)half_rows + (leader ? 0 : p.up_row0);
         return tl.n_blk * BN + (int)rank * (int)half_rows;
+      };
+      auto load_w = [&](uint32_t sa, int kb_abs, int cnt, int w_row, uint32_t fb) {
+        for (int h = 0; h < cnt; ++h)
+          ptx::tma_load_2d_pair(sa + kPairKbPerStage * kATileBytes + h * w_bytes, &mapB, (kb_abs + h) * kBK, w_row, fb, p.w_policy);
+      };
+      auto load_a = [&](uint32_t sa, int kb_abs, int cnt, int m0, uint32_t fb) {
+        for (int h = 0; h < cnt; ++h)
+          ptx::tma_load_2d_pair(sa + h * kATileBytes, &mapA, (kb_abs + h) * kBK, m0, fb, p.a_policy);
       };
       // Ring fill of the first tile: weights do not depend on the upstream kernel, so their boxes are issued
       // before the programmatic-dependency wait; A follows once the producer of A has finished.
@@ -212,33 +226,37 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         const PairTile tl = pair_tile(cluster % total_tiles, p.m_tiles, p.n_tiles_n, p.panel);
         const int m0 = tl.m_blk * 256 + (int)rank * 128, w_row = w_row_of(tl);
         const int kb0 = (cluster / total_tiles) * p.kb_per_split;
-        pre = min(stages, min(p.kb_per_split, num_kb - kb0));
-        for (int kb = 0; kb < pre; ++kb) {
-          if (leader) ptx::mbar_expect_tx(full_bar(kb), tx_pair);
-          ptx::tma_load_2d_pair(base + kb * stage_bytes + kATileBytes, &mapB, (kb0 + kb) * kBK, w_row, ptx::mapa(full_bar(kb), 0), p.w_policy);
+        const int nkb = min(p.kb_per_split, num_kb - kb0);
+        pre = min(stages, (nkb + kPairKbPerStage - 1) / kPairKbPerStage);
+        for (int st = 0; st < pre; ++st) {
+          const int cnt = min(kPairKbPerStage, nkb - st * kPairKbPerStage);
+          if (leader) ptx::mbar_expect_tx(full_bar(st), tx_kb * cnt);
+          load_w(base + st * stage_bytes, kb0 + st * kPairKbPerStage, cnt, w_row, ptx::mapa(full_bar(st), 0));
         }
         ptx::pdl_wait();
-        for (int kb = 0; kb < pre; ++kb)
-          ptx::tma_load_2d_pair(base + kb * stage_bytes, &mapA, (kb0 + kb) * kBK, m0, ptx::mapa(full_bar(kb), 0), p.a_policy);
+        for (int st = 0; st < pre; ++st)
+          load_a(base + st * stage_bytes, kb0 + st * kPairKbPerStage, min(kPairKbPerStage, nkb - st * kPairKbPerStage), m0, ptx::mapa(full_bar(st), 0));
       } else {
         ptx::pdl_wait();
       }
-      int it = 0;
+      // ring position kept as running (stage, phase) counters: `it % stages` with a run-time divisor is a ~30-instruction
+      // sequence with a MUFU in the middle, once per stage on the critical path of the pipeline
+      int it = 0, s = 0;
+      uint32_t ph = 0;
       for (int u = cluster; u < total_units; u += n_clusters) {
         const PairTile tl = pair_tile(u % total_tiles, p.m_tiles, p.n_tiles_n, p.panel);
         const int m0 = tl.m_blk * 256 + (int)rank * 128, w_row = w_row_of(tl);
         const int kb0 = (u / total_tiles) * p.kb_per_split;
         const int nkb = min(p.kb_per_split, num_kb - kb0);
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
+        for (int kb = 0; kb < nkb; kb += kPairKbPerStage, ++it, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1u : 0u)) {
           if (it < pre) continue;                       // issued by the ring fill above
-          const int s = it % stages;
-          const uint32_t ph = (uint32_t)(it / stages) & 1u;
+          const int cnt = min(kPairKbPerStage, nkb - kb);
           ptx::mbar_wait(empty_bar(s), ph ^ 1u);
           const uint32_t fb = ptx::mapa(full_bar(s), 0);
-          if (leader) ptx::mbar_expect_tx(full_bar(s), tx_pair);
+          if (leader) ptx::mbar_expect_tx(full_bar(s), tx_kb * cnt);
           const uint32_t sa = base + s * stage_bytes;
-          ptx::tma_load_2d_pair(sa + kATileBytes, &mapB, (kb0 + kb) * kBK, w_row, fb, p.w_policy);
-          ptx::tma_load_2d_pair(sa, &mapA, (kb0 + kb) * kBK, m0, fb, p.a_policy);
+          load_w(sa, kb0 + kb, cnt, w_row, fb);
+          load_a(sa, kb0 + kb, cnt, m0, fb);
         }
       }
     }
@@ -246,26 +264,37 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     if (leader) {
       // ---------------- MMA issuer (leader CTA; the whole warp walks the loop, one elected lane issues) ----------------
       const uint32_t idesc = ptx::umma_idesc_bf16(256, BN);
-      int it = 0, i = 0;
+      int i = 0, s = 0;
+      uint32_t ph = 0;
       for (int u = cluster; u < total_units; u += n_clusters, ++i) {
         const uint32_t as = (uint32_t)i & 1u, aph = ((uint32_t)i >> 1) & 1u;
         ptx::mbar_wait(tmem_empty_bar + 8u * as, aph ^ 1u);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kPairAccCols;
         const int nkb = min(p.kb_per_split, num_kb - (u / total_tiles) * p.kb_per_split);
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
-          const int s = it % stages;
-          const uint32_t ph = (uint32_t)(it / stages) & 1u;
+        const uint32_t w_bytes = (uint32_t)BN * 64u;
+        for (int kb = 0; kb < nkb; kb += kPairKbPerStage, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1u : 0u)) {
+          const int cnt = min(kPairKbPerStage, nkb - kb);
           ptx::mbar_wait(full_bar(s), ph);
           ptx::tc_fence_after();
           if (ptx::elect_one()) {
             const uint32_t sa = base + s * stage_bytes;
-            const uint32_t a_lo = ptx::umma_desc_lo(sa), b_lo = ptx::umma_desc_lo(sa + kATileBytes);
+            const uint32_t a_lo = ptx::umma_desc_lo(sa), b_lo = ptx::umma_desc_lo(sa + kPairKbPerStage * kATileBytes);
+            const uint32_t a_step = kATileBytes >> 4, b_step = w_bytes >> 4;      // next K block, in encoded (16-byte) units
+            if (cnt == kPairKbPerStage) {                 // the common case, straight-line
 #pragma unroll
-            for (int k = 0; k < kBK / 16; ++k)        // +32 bytes along K inside the 128-byte swizzle row = +2 in the encoded address
-              ptx::umma_bf16_pair_lo(d_tmem, a_lo + 2 * k, b_lo + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+              for (int h = 0; h < kPairKbPerStage; ++h)
+#pragma unroll
+                for (int k = 0; k < kBK / 16; ++k)    // +32 bytes along K inside the 128-byte swizzle row = +2 in the encoded address
+                  ptx::umma_bf16_pair_lo(d_tmem, a_lo + h * a_step + 2 * k, b_lo + h * b_step + 2 * k, idesc, (kb | h | k) != 0 ? 1u : 0u);
+            } else {
+              for (int h = 0; h < cnt; ++h)
+#pragma unroll
+                for (int k = 0; k < kBK / 16; ++k)
+                  ptx::umma_bf16_pair_lo(d_tmem, a_lo + h * a_step + 2 * k, b_lo + h * b_step + 2 * k, idesc, (kb | h | k) != 0 ? 1u : 0u);
+            }
             ptx::umma_commit_pair(empty_bar(s));          // both CTAs' producers may refill the stage
-            if (kb + 1 == nkb) ptx::umma_commit_pair(tmem_full_bar + 8u * as);   // accumulator complete in both CTAs' TMEM
+            if (kb + cnt == nkb) ptx::umma_commit_pair(tmem_full_bar + 8u * as);   // accumulator complete in both CTAs' TMEM
           }
           __syncwarp();
         }

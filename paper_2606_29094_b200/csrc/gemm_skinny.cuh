@@ -115,10 +115,9 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
       for (int kb = 0; kb < pre; ++kb) load_w(kb, kb);          // weights: independent of the upstream kernel
       ptx::pdl_wait();                                           // activations: written by the upstream kernel
       for (int kb = 0; kb < pre; ++kb) load_x(kb, kb);
-      for (int kb = pre; kb < nkb; ++kb) {
-        const int s = kb % stages;
-        const uint32_t ph = (uint32_t)(kb / stages) & 1u;
-        ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+      // ring position as running (stage, phase) counters (no run-time division per K block); pre == stages here
+      for (int kb = pre, s = 0, ph = 1; kb < nkb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
+        ptx::mbar_wait(empty_bar(s), (uint32_t)ph ^ 1u);
         load_w(kb, s);
         load_x(kb, s);
       }
@@ -127,10 +126,8 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
     if (lane == 0) {
       // ---------------- MMA issuer: D[128 features, tpad tokens] += W_tile . X_tile^T ----------------
       const uint32_t idesc = ptx::umma_idesc_bf16(128, p.tpad);
-      for (int kb = 0; kb < nkb; ++kb) {
-        const int s = kb % stages;
-        const uint32_t ph = (uint32_t)(kb / stages) & 1u;
-        ptx::mbar_wait(full_bar(s), ph);
+      for (int kb = 0, s = 0, ph = 0; kb < nkb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
+        ptx::mbar_wait(full_bar(s), (uint32_t)ph);
         ptx::tc_fence_after();
         const uint32_t sw = base + s * stage_bytes, sx = sw + kSkWBytes;
 #pragma unroll

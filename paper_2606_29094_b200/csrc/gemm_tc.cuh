@@ -104,10 +104,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       for (int kb = 0; kb < pre; ++kb) load_w(kb, kb);
       ptx::pdl_wait();
       for (int kb = 0; kb < pre; ++kb) load_a(kb, kb);
-      for (int kb = pre; kb < num_kb; ++kb) {
-        const int s = kb % stages;
-        const uint32_t ph = (uint32_t)(kb / stages) & 1u;
-        ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+      // ring position as running (stage, phase) counters (no run-time division per K block); pre == stages here
+      for (int kb = pre, s = 0, ph = 1; kb < num_kb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
+        ptx::mbar_wait(empty_bar(s), (uint32_t)ph ^ 1u);
         load_w(kb, s);
         load_a(kb, s);
       }
@@ -116,10 +115,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
     if (lane == 0) {
       // ---------------- MMA issuer ----------------
       const uint32_t idesc = ptx::umma_idesc_bf16(128, BN);
-      for (int kb = 0; kb < num_kb; ++kb) {
-        const int s = kb % stages;
-        const uint32_t ph = (uint32_t)(kb / stages) & 1u;
-        ptx::mbar_wait(full_bar(s), ph);
+      for (int kb = 0, s = 0, ph = 0; kb < num_kb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
+        ptx::mbar_wait(full_bar(s), (uint32_t)ph);
         ptx::tc_fence_after();
         const uint32_t sa = base + s * stage_bytes, sb = sa + kATileBytes;
 #pragma unroll
