@@ -243,8 +243,9 @@ static void plan_pair(int M, int N, int K, int epi, int max_splits, int* bn_out,
   static const int cand_std[] = {256, 224, 192, 160, 128, 96, 64};
   static const int cand_glu[] = {256, 192, 128, 64};
   static const int cand_lm[] = {256};
-  const int* cand = epi == EPI_SWIGLU ? cand_glu : (epi == EPI_LMHEAD ? cand_lm : cand_std);
-  const int nc = epi == EPI_SWIGLU ? 4 : (epi == EPI_LMHEAD ? 1 : 7);
+  static const int cand_rope[] = {256, 128};          // whole 128-wide heads per tile
+  const int* cand = epi == EPI_SWIGLU ? cand_glu : (epi == EPI_LMHEAD ? cand_lm : (epi == EPI_ROPE ? cand_rope : cand_std));
+  const int nc = epi == EPI_SWIGLU ? 4 : (epi == EPI_LMHEAD ? 1 : (epi == EPI_ROPE ? 2 : 7));
   // Cost of a unit in 1/256 K-block units of a 256-wide tile.  Measured with two K blocks per ring stage (4096 x 12288 x 4096,
   // whole kernel): bn 256 / 192 / 128 -> 1.00 / 0.78 / 0.61 of the 256-wide tile per tile, i.e. ~0.22 + 0.78 bn / 256 (the MMA
   // time is bn / 2 cycles, the stage hand-off is not free); the fixed part (ramp, exposed epilogue) shrinks with the tile too.
@@ -297,7 +298,7 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
   if (epi != EPI_LMHEAD && epi != EPI_ROPE && p.ldc % 8) { set_err(err, "gemm_pair: output row pitch %lld must be a multiple of 8 elements", p.ldc); return DLM_E_ARG; }
   if (epi != EPI_F32) max_splits = 1;
   int splits = 1;
-  if (epi == EPI_ROPE) bn = 256;                                 // two 128-wide heads per tile
+  if (epi == EPI_ROPE && bn != 128 && bn != 256) bn = 0;         // whole 128-wide heads per tile: 256 or 128, planned
   if (bn <= 0) plan_pair(M, N, K, epi, max_splits, &bn, &splits);
   else if (max_splits < 0) splits = -max_splits;                 // test hook: forced split count
   if (bn % 32 || bn < 64 || bn > 256 || (epi == EPI_SWIGLU && bn % 64)) { set_err(err, "gemm_pair: bad bn=%d", bn); return DLM_E_ARG; }
@@ -1208,7 +1209,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
         GemmPairParams p = {};
         p.rope.q = (bf16*)c->q; p.rope.kv_store = (bf16*)c->kv_store; p.rope.rope_cos = c->rope_cos; p.rope.rope_sin = c->rope_sin;
         p.rope.page_table = c->page_table; p.rope.b = bd; p.rope.g = c->kg; p.rope.layer = l; p.rope.n_heads = a.n_heads;
-        int rc = gemm_pair(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_ROPE, 256, p, st, pdl);
+        int rc = gemm_pair(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_ROPE, 0, p, st, pdl);
         if (rc) return rc;
       } else if (tc) {
         int rc = gemm_big(c, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_F32, c->qkv, nullptr, NQKV, 0, pdl, c->qkv_rows, &nq);

@@ -412,7 +412,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
           }
         }
       } else if (EPI == EPI_ROPE) {
-        // tile = 256 columns = two heads of 128; pairs (i, i + 64) live in chunks (a, a + 2) of a head
+        // tile = BN / 128 whole heads of 128 columns (BN = 256 or 128); pairs (i, i + 64) live in chunks (a, a + 2) of a head
         const RopeEpi& e = p.rope;
         int pos = 0, page = 0, slot_in_page = 0;
         if (row_ok) {
@@ -423,8 +423,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         }
         uint32_t u2[32];
 #pragma unroll 1
-        for (int hh = 0; hh < 2; ++hh) {
-          const int hg = tl.n_blk * 2 + hh;                     // global head index: Q heads, then K heads, then V heads
+        for (int hh = 0; hh < (BN >> 7); ++hh) {
+          const int hg = tl.n_blk * (BN >> 7) + hh;             // global head index: Q heads, then K heads, then V heads
           const bool head_ok = hg < e.n_heads + 2 * e.g.n_kv_heads;
           const bool rotate = hg < e.n_heads + e.g.n_kv_heads;
           long long dst_own = 0;                                // element offset of this thread's row in its destination, -1: none
