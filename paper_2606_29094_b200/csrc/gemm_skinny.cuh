@@ -123,19 +123,21 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      // ---------------- MMA issuer: D[128 features, tpad tokens] += W_tile . X_tile^T ----------------
-      const uint32_t idesc = ptx::umma_idesc_bf16(128, p.tpad);
-      for (int kb = 0, s = 0, ph = 0; kb < nkb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
-        ptx::mbar_wait(full_bar(s), (uint32_t)ph);
-        ptx::tc_fence_after();
-        const uint32_t sw = base + s * stage_bytes, sx = sw + kSkWBytes;
+    // ---------------- MMA issuer: D[128 features, tpad tokens] += W_tile . X_tile^T (whole warp walks, one elected lane issues) ----------------
+    const uint32_t idesc = ptx::umma_idesc_bf16(128, p.tpad);
+    for (int kb = 0, s = 0, ph = 0; kb < nkb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
+      ptx::mbar_wait(full_bar(s), (uint32_t)ph);
+      ptx::tc_fence_after();
+      if (ptx::elect_one()) {
+        const uint32_t sw = base + s * stage_bytes;
+        const uint32_t w_lo = ptx::umma_desc_lo(sw), x_lo = ptx::umma_desc_lo(sw + kSkWBytes);
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-          ptx::umma_bf16(tmem_base, ptx::umma_desc_sw128(sw + k * 32), ptx::umma_desc_sw128(sx + k * 32), idesc, (kb | k) != 0 ? 1u : 0u);
+          ptx::umma_bf16_lo(tmem_base, w_lo + 2 * k, x_lo + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
         ptx::umma_commit(empty_bar(s));
+        if (kb + 1 == nkb) ptx::umma_commit(tmem_full_bar);
       }
-      ptx::umma_commit(tmem_full_bar);
+      __syncwarp();
     }
   } else {
     // ---------------- epilogue (warps 2..5; TMEM lane quarter = warp % 4; lane = output feature) ----------------

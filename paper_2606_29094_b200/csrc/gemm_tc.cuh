@@ -112,21 +112,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      // ---------------- MMA issuer ----------------
-      const uint32_t idesc = ptx::umma_idesc_bf16(128, BN);
-      for (int kb = 0, s = 0, ph = 0; kb < num_kb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
-        ptx::mbar_wait(full_bar(s), (uint32_t)ph);
-        ptx::tc_fence_after();
-        const uint32_t sa = base + s * stage_bytes, sb = sa + kATileBytes;
+    // ---------------- MMA issuer (the whole warp walks the loop, one elected lane issues) ----------------
+    const uint32_t idesc = ptx::umma_idesc_bf16(128, BN);
+    for (int kb = 0, s = 0, ph = 0; kb < num_kb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
+      ptx::mbar_wait(full_bar(s), (uint32_t)ph);
+      ptx::tc_fence_after();
+      if (ptx::elect_one()) {
+        const uint32_t sa = base + s * stage_bytes;
+        const uint32_t a_lo = ptx::umma_desc_lo(sa), b_lo = ptx::umma_desc_lo(sa + kATileBytes);
 #pragma unroll
-        for (int k = 0; k < kBK / 16; ++k) {
-          ptx::umma_bf16(tmem_base, ptx::umma_desc_sw128(sa + k * 32), ptx::umma_desc_sw128(sb + k * 32), idesc,
-                         (kb | k) != 0 ? 1u : 0u);
-        }
-        ptx::umma_commit(empty_bar(s));      // frees the stage when these MMAs have read it
+        for (int k = 0; k < kBK / 16; ++k)            // +32 bytes along K inside the 128-byte swizzle row = +2 in the encoded address
+          ptx::umma_bf16_lo(tmem_base, a_lo + 2 * k, b_lo + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+        ptx::umma_commit(empty_bar(s));            // frees the stage once these MMAs have read it
+        if (kb + 1 == num_kb) ptx::umma_commit(tmem_full_bar);       // accumulator complete
       }
-      ptx::umma_commit(tmem_full_bar);       // accumulator complete
+      __syncwarp();
     }
   } else {
     // ---------------- epilogue (warps 2..5; TMEM lane quarter = warp % 4) ----------------

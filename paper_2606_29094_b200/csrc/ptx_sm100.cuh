@@ -150,6 +150,22 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
 }
 // Instruction descriptor, kind::f16: D fp32 (bits[4,6)=1), A,B bf16 (bits[7,10)=1, [10,13)=1), both K-major
 // (bits 15,16 = 0), N>>3 at [17,23), M>>4 at [24,29).
+// Low word of the SWIZZLE_128B K-major descriptor (see umma_desc_sw128); the high word is the constant kDescHiSw128.
+constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (2u << 29);
+__device__ __forceinline__ uint32_t umma_desc_lo(uint32_t smem_addr) { return ((smem_addr & 0x3FFFFu) >> 4) | (1u << 16); }
+// cta_group::1 MMA from descriptor low words (both operands SWIZZLE_128B K-major): issued under elect_one() by a CONVERGED warp.
+// From a divergent `if (lane == 0)` branch every tcgen05 instruction compiles to an ELECT / BRA.U.ANY waterfall (~16 SASS
+// instructions and >100 cycles per issue).
+__device__ __forceinline__ void umma_bf16_lo(uint32_t tmem_d, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "mov.b64 da, {%1, %5};\n\t"
+      "mov.b64 db, {%2, %5};\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n\t}"
+      ::"r"(tmem_d), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(accumulate), "r"(kDescHiSw128)
+      : "memory");
+}
 __device__ __forceinline__ uint32_t umma_idesc_bf16(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
