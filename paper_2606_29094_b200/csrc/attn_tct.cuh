@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
   pdl_wait();
 
   if (warp == 0) {
-    if (lane == 0) {
+    if (ptx::elect_one()) {        // one elected lane of the converged warp: TMA issues compile straight-line
       // ---------------- TMA producer: K ring and V ring ----------------
       int kc = 0, vc = 0;
       for (int it = blockIdx.x; it < p.n_items; it += gridDim.x) {

@@ -199,7 +199,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr));
 
   if (warp == 0) {
-    if (lane == 0) {
+    if (ptx::elect_one()) {        // one elected lane of the converged warp: TMA issues compile straight-line
       // ---------------- TMA producer (both CTAs, one lane) ----------------
       const uint32_t half_rows = (uint32_t)BN / 2;
       const uint32_t w_bytes = half_rows * 128u;

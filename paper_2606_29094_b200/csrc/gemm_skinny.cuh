@@ -87,7 +87,7 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr));
 
   if (warp == 0) {
-    if (lane == 0) {
+    if (ptx::elect_one()) {        // one elected lane of the converged warp: TMA issues compile straight-line
       // ---------------- TMA producer ----------------
       const uint32_t tx = (uint32_t)kSkWBytes + (uint32_t)p.tpad * 128u;
       auto load_w = [&](int kb, int s) {

@@ -83,7 +83,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr));
 
   if (warp == 0) {
-    if (lane == 0) {
+    if (ptx::elect_one()) {        // one elected lane of the converged warp: TMA issues compile straight-line
       // ---------------- TMA producer ----------------
       const uint32_t a_bytes = (uint32_t)p.a_box_rows * 128u;
       const uint32_t tx = a_bytes + (uint32_t)BN * 128u;
