@@ -520,8 +520,8 @@ def kernel_pass(run, pkg, arch, peaks, n_steps=24):
         ach = flops / (g_launch / n_cached) / per_launch_s * 1e-12
         rf = {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"]}
     # dram__bytes_read + dram__bytes_write per launch, from the committed ncu --set full capture of this workload
-    # (profiles/r01_ncu_kernels.md: 15.47 GB over the 129 GEMM launches of a C2 cached step); other workloads: not captured
-    traffic = 119.9e6 if (T == 32 and arch.n_layers == 32 and arch.d_model == 4096) else None
+    # (profiles/r01_ncu_kernels.md: 15.39 GB over the 129 GEMM launches of a C2 cached step); other workloads: not captured
+    traffic = 119.3e6 if (T == 32 and arch.n_layers == 32 and arch.d_model == 4096) else None
     big = T > 128
     rf.update({"traffic": traffic, "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_kernels.md)",
                "algorithmic_bytes_per_launch": w_bytes / (g_launch / n_cached),
