@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
     if (ptx::elect_one()) {        // one elected lane of the converged warp: TMA issues compile straight-line
       // ---------------- TMA producer: K ring and V ring ----------------
       int kc = 0, vc = 0;
-      for (int it = blockIdx.x; it < p.n_items; it += gridDim.x) {
+      for (int k = 0, it; (it = ta_sched(k, p.n_items)) >= 0; ++k) {
         const TaItem im = ta_item(it, p);
         int t0, t1, n_rows, S;
         ta_range(im, p, &t0, &t1, &n_rows, &S);
@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
       __syncwarp();
       ++vc; ++pc;
     };
-    for (int it = blockIdx.x; it < p.n_items; it += gridDim.x) {
+    for (int k = 0, it; (it = ta_sched(k, p.n_items)) >= 0; ++k) {
       const TaItem im = ta_item(it, p);
       int t0, t1, n_rows, S;
       ta_range(im, p, &t0, &t1, &n_rows, &S);
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
   } else if (warp == 2) {
     // ---------------- Q loader: <= 64 stacked rows x 128 into two swizzled [64 x 64] boxes (rows past the end: zeros) ----------------
     int qc = 0;
-    for (int it = blockIdx.x; it < p.n_items; it += gridDim.x) {
+    for (int k = 0, it; (it = ta_sched(k, p.n_items)) >= 0; ++k) {
       const TaItem im = ta_item(it, p);
       int t0, t1, n_rows, S;
       ta_range(im, p, &t0, &t1, &n_rows, &S);
@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
       return out != 0;
     };
     int sc = 0, pc = 0;
-    for (int it = blockIdx.x; it < p.n_items; it += gridDim.x) {
+    for (int k = 0, it; (it = ta_sched(k, p.n_items)) >= 0; ++k) {
       const TaItem im = ta_item(it, p);
       int t0, t1, n_rows, S;
       ta_range(im, p, &t0, &t1, &n_rows, &S);

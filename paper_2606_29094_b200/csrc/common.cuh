@@ -53,6 +53,7 @@ struct BatchDesc {
   const int* row_off;// [n] offset of the request's block rows in the [R, *] buffers
   const float* tau;  // [n]
   const int* tok_bi; // [T] batch index of each computed token
+  const int* order;  // [n] batch indices by decreasing K/V length (work order of the persistent attention kernels)
 };
 
 // Paged K/V store geometry: [layer][page][K|V][H_kv][page_tokens][d_h]

@@ -512,6 +512,7 @@ static int attn_op_contiguous(const void* q, const void* k, const void* v, void*
   bd.n = 1; bd.T = Tq; bd.max_q_len = Tq; bd.max_kv_len = S; bd.min_q_len = Tq;
   int* md = meta + g.n_pages;
   bd.slot = md; bd.q_off = md + 1; bd.q_len = md + 2; bd.q_pos0 = md + 3; bd.kv_len = md + 4; bd.tok_bi = md + 16;
+  bd.order = md + 5;                                  // one request: [0]
   const float scale = 1.f / sqrtf((float)dh);
   int rc = DLM_OK;
   bool done = false;
@@ -559,7 +560,7 @@ struct LayerW { void *wqkv, *wo, *wgu, *wd; };
 
 struct HostBatch {
   int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0, min_q = 1 << 30;
-  std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, gen_lo, gen_len, tok_bi;
+  std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, gen_lo, gen_len, tok_bi, order;
   std::vector<float> tau;
   std::vector<char> refresh;     // per request: whole sequence recomputed this step
 };
@@ -834,7 +835,7 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
     c->attn_ws_bytes = (size_t)8 * std::min(c->Tmax, 1024) * a.n_heads * (128 + 2) * 4;
     ALLOC(c->attn_ws, c->attn_ws_bytes);
   }
-  c->desc_cap_ints = (size_t)12 * a.max_requests + c->Tmax + 64;      // 11 n + T used
+  c->desc_cap_ints = (size_t)12 * a.max_requests + c->Tmax + 64;      // 12 n + T used
   ALLOC(c->desc_dev, c->desc_cap_ints * 4);
   if (cudaMallocHost(&c->desc_host, c->desc_cap_ints * 4) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
   c->out_bytes = (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6 + (size_t)a.max_requests * 5 * 4;     // + confidence features
@@ -1088,11 +1089,19 @@ static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override
     if (qlen > 0) hb.min_q = std::min(hb.min_q, qlen);
   }
   if (hb.T > c->Tmax) { set_err(&c->err, "step: %d tokens exceed max_batch_tokens=%d", hb.T, c->Tmax); return DLM_E_CAPACITY; }
+  // work order of the persistent attention kernels: longest K/V first (requests that compute nothing last); results do not
+  // depend on it, every item is computed independently
+  hb.order.resize(hb.n);
+  for (int i = 0; i < hb.n; ++i) hb.order[i] = i;
+  std::stable_sort(hb.order.begin(), hb.order.end(), [&](int x, int y) {
+    const long long wx = hb.q_len[x] > 0 ? hb.kv_len[x] : -1, wy = hb.q_len[y] > 0 ? hb.kv_len[y] : -1;
+    return wx > wy;
+  });
   return DLM_OK;
 }
 
-// Descriptor layout in desc_host / desc_dev (ints): slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, tau [n each],
-// then tok_bi [T].  Offsets depend on (n, T) only, so a captured graph of the same batch shape can be replayed.
+// Descriptor layout in desc_host / desc_dev (ints): slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, tau, gen_lo,
+// gen_len, order [n each], then tok_bi [T].  Offsets depend on (n, T) only, so a captured graph of the same batch shape can be replayed.
 static size_t fill_desc_host(dlm_ctx* c, const HostBatch& hb) {
   int* h = c->desc_host;
   const size_t n = hb.n;
@@ -1101,8 +1110,9 @@ static size_t fill_desc_host(dlm_ctx* c, const HostBatch& hb) {
   memcpy(h + 8 * n, hb.tau.data(), n * 4);
   memcpy(h + 9 * n, hb.gen_lo.data(), n * 4);
   memcpy(h + 10 * n, hb.gen_len.data(), n * 4);
-  memcpy(h + 11 * n, hb.tok_bi.data(), hb.tok_bi.size() * 4);
-  return 11 * n + hb.tok_bi.size();
+  memcpy(h + 11 * n, hb.order.data(), n * 4);
+  memcpy(h + 12 * n, hb.tok_bi.data(), hb.tok_bi.size() * 4);
+  return 12 * n + hb.tok_bi.size();
 }
 static BatchDesc make_desc(dlm_ctx* c, const HostBatch& hb) {
   BatchDesc d;
@@ -1110,7 +1120,7 @@ static BatchDesc make_desc(dlm_ctx* c, const HostBatch& hb) {
   const int* b = c->desc_dev;
   d.n = hb.n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv; d.min_q_len = std::min(hb.min_q, hb.max_q);
   d.slot = b; d.q_off = b + n; d.q_len = b + 2 * n; d.q_pos0 = b + 3 * n; d.kv_len = b + 4 * n; d.blk_lo = b + 5 * n;
-  d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.tok_bi = b + 11 * n;
+  d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.order = b + 11 * n; d.tok_bi = b + 12 * n;
   return d;
 }
 
