@@ -47,6 +47,8 @@ struct TaParams {
   float* ws_ml;             // [splits, T*H, 2]
   unsigned long long kv_policy;
   int row_filter;           // mixed steps: 0 all requests, 1 only those with <= 64 stacked rows, 2 only those with more
+  int req_lo, req_n;        // entries [req_lo, req_lo + req_n) of BatchDesc::order are this launch's requests
+  int ragged_q;             // 1: items enumerate the requests' own query tiles (BatchDesc::qt_off), no empty slots for short requests
 };
 
 namespace ptx {
@@ -77,7 +79,8 @@ __device__ __forceinline__ float ex2(float x) { float y; asm("ex2.approx.ftz.f32
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 }  // namespace ptx
 
-// item -> (batch index, KV head, query tile, split).  Items are numbered request-major over the requests in order of
+// item -> (batch index, KV head, query tile, split).  Items are numbered request-major (each request with its own number of
+// query tiles) over the requests in order of
 // DECREASING K/V length (BatchDesc::order, sorted on the host) and dealt to the persistent CTAs in a snake (round k runs
 // left to right for even k, right to left for odd k): longest-first + alternating direction keeps the CTAs' K/V tile totals
 // within a few tiles of each other on ragged batches (plain round-robin over unsorted requests: +25 % on the slowest CTA).
@@ -86,8 +89,21 @@ __device__ __forceinline__ TaItem ta_item(int it, const TaParams& p) {
   TaItem r;
   r.split = it % p.splits; it /= p.splits;
   r.kvh = it % p.g.n_kv_heads; it /= p.g.n_kv_heads;
+  if (p.ragged_q) {
+    // `it` is a query-tile index over the launch's requests: find the request by its prefix sum (n <= a few dozen)
+    const int* off = p.b.qt_off + p.req_lo;
+    const int base = off[0];
+    int lo = 0, hi = p.req_n;                       // off[lo] - base <= it < off[hi] - base
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (off[mid] - base <= it) lo = mid; else hi = mid;
+    }
+    r.qt = it - (off[lo] - base);
+    r.bi = p.b.order[p.req_lo + lo];
+    return r;
+  }
   r.qt = it % p.q_tiles_max;
-  r.bi = p.b.order[it / p.q_tiles_max];
+  r.bi = p.b.order[p.req_lo + it / p.q_tiles_max];
   return r;
 }
 // k-th item of this CTA, or -1 when it has none left

@@ -43,6 +43,8 @@ struct BatchDesc {
   int max_q_len;     // max over requests (attention grid sizing)
   int max_kv_len;
   int min_q_len;     // min over requests that compute anything (mixed steps: block rows of the cached requests)
+  int n_big;         // requests with more than 64 stacked query rows per KV head: they come first in `order`
+  int qt_big, qt_total; // 128-row query tiles of the first n_big / of all requests of `order` (qt_off[n_big], qt_off[n])
   const int* slot;   // [n] request slot (row of tokens / page table)
   const int* q_off;  // [n]
   const int* q_len;  // [n]
@@ -53,7 +55,8 @@ struct BatchDesc {
   const int* row_off;// [n] offset of the request's block rows in the [R, *] buffers
   const float* tau;  // [n]
   const int* tok_bi; // [T] batch index of each computed token
-  const int* order;  // [n] batch indices by decreasing K/V length (work order of the persistent attention kernels)
+  const int* qt_off; // [n + 1] prefix sums, over `order`, of the requests' 128-row query tiles (nullptr: q_tiles_max each)
+  const int* order;  // [n] batch indices: the n_big requests first, each group by decreasing K/V length (work order of the attention kernels)
 };
 
 // Paged K/V store geometry: [layer][page][K|V][H_kv][page_tokens][d_h]

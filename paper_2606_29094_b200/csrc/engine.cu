@@ -351,7 +351,8 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   if (g.head_dim != 128 || g.page_tokens != 64 || bd.T <= 0) return 0;
   const int r = n_heads / g.n_kv_heads;
   const int q_tiles = (bd.max_q_len * r + kTaTile - 1) / kTaTile;
-  const long long items = (long long)bd.n * g.n_kv_heads * q_tiles;
+  const bool ragged = bd.qt_off != nullptr && bd.max_q_len * r > kTtNQ;      // row-major kernel over the requests' own query tiles
+  const long long items = ragged ? (long long)bd.qt_total * g.n_kv_heads : (long long)bd.n * g.n_kv_heads * q_tiles;
   const int kv_tiles = (bd.max_kv_len + kTaTile - 1) / kTaTile;
   const bool no_transposed = force >= 100;      // test hook: 100 + f = attn_tc_kernel even when the transposed kernel fits
   if (no_transposed) force -= 100;
@@ -390,7 +391,7 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   p.splits = splits; p.q_tiles_max = q_tiles; p.n_items = (int)(items * splits);
   p.scale_log2 = scale * 1.4426950408889634f; p.ws_o = nullptr; p.ws_ml = nullptr;
   p.kv_policy = q_tiles == 1 ? DLM_L2_EVICT_FIRST : DLM_L2_EVICT_NORMAL;
-  p.row_filter = 0;
+  p.row_filter = 0; p.req_lo = 0; p.req_n = bd.n; p.ragged_q = 0;
   const long long TH = (long long)bd.T * n_heads;
   while (splits > 1 && (size_t)splits * TH * (128 + 2) * 4 > *ws_bytes) --splits;     // fixed workspace (see attn_flash_launch)
   p.splits = splits; p.n_items = (int)(items * splits);
@@ -400,8 +401,11 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   }
   if (two_kernels) {
     TaParams pt = p;
-    pt.row_filter = 1; pt.q_tiles_max = 1; pt.n_items = bd.n * g.n_kv_heads; pt.kv_policy = DLM_L2_EVICT_FIRST;
-    p.row_filter = 2;
+    // `order` lists the n_big requests of the row-major kernel first: each launch walks its own requests only
+    pt.row_filter = 1; pt.q_tiles_max = 1; pt.req_lo = bd.n_big; pt.n_items = (bd.n - bd.n_big) * g.n_kv_heads; pt.kv_policy = DLM_L2_EVICT_FIRST;
+    pt.req_n = bd.n - bd.n_big;
+    p.row_filter = 2; p.req_n = bd.n_big; p.ragged_q = 1; p.n_items = bd.qt_big * g.n_kv_heads;
+    if (pt.n_items <= 0 || p.n_items <= 0) { set_err(err, "attn_tc: inconsistent mixed batch (%d of %d requests above 64 rows)", bd.n_big, bd.n); return DLM_E_ARG; }
     cudaError_t e2 = launch_k(attn_tct_kernel, dim3((unsigned)std::min(g_num_sms, pt.n_items)), dim3(kTaThreads), (size_t)kTtSmem, st, pdl, *mkv, pt);
     if (e2 == cudaSuccess)
       e2 = launch_k(attn_tc_kernel, dim3((unsigned)std::min<long long>(g_num_sms, p.n_items)), dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
@@ -409,6 +413,7 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
     *done = true;
     return 0;
   }
+  if (ragged && !transposed) p.ragged_q = 1;
   const dim3 grid((unsigned)std::min<long long>(g_num_sms, p.n_items));
   cudaError_t e = transposed ? launch_k(attn_tct_kernel, grid, dim3(kTaThreads), (size_t)kTtSmem, st, pdl, *mkv, p)
                              : launch_k(attn_tc_kernel, grid, dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
@@ -559,8 +564,8 @@ struct Req {
 struct LayerW { void *wqkv, *wo, *wgu, *wd; };
 
 struct HostBatch {
-  int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0, min_q = 1 << 30;
-  std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, gen_lo, gen_len, tok_bi, order;
+  int n = 0, T = 0, R = 0, max_q = 0, max_kv = 0, min_q = 1 << 30, n_big = 0, qt_big = 0, qt_total = 0;
+  std::vector<int> slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, gen_lo, gen_len, tok_bi, order, qt_off;
   std::vector<float> tau;
   std::vector<char> refresh;     // per request: whole sequence recomputed this step
 };
@@ -591,7 +596,7 @@ struct KProf {
   ~KProf() { for (auto e : ev) cudaEventDestroy(e); }
 };
 
-typedef std::tuple<int, int, int, int, int, int, int, int> GraphKey;   // kind, dry, n, T, R, max_q, max_kv, options
+typedef std::tuple<int, int, int, int, int, int, int, int, int, int, int> GraphKey;   // kind, dry, n, T, R, max_q, max_kv, options, n_big, qt_big, qt_total
 struct GraphEntry { int seen = 0; cudaGraphExec_t exec = nullptr; long long launches = 0; };
 
 struct dlm_ctx {
@@ -835,7 +840,7 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
     c->attn_ws_bytes = (size_t)8 * std::min(c->Tmax, 1024) * a.n_heads * (128 + 2) * 4;
     ALLOC(c->attn_ws, c->attn_ws_bytes);
   }
-  c->desc_cap_ints = (size_t)12 * a.max_requests + c->Tmax + 64;      // 12 n + T used
+  c->desc_cap_ints = (size_t)14 * a.max_requests + c->Tmax + 64;      // 13 n + 1 + T used
   ALLOC(c->desc_dev, c->desc_cap_ints * 4);
   if (cudaMallocHost(&c->desc_host, c->desc_cap_ints * 4) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
   c->out_bytes = (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6 + (size_t)a.max_requests * 5 * 4;     // + confidence features
@@ -1093,15 +1098,23 @@ static int build_batch(dlm_ctx* c, const dlm_batch* b, const float* thr_override
   // depend on it, every item is computed independently
   hb.order.resize(hb.n);
   for (int i = 0; i < hb.n; ++i) hb.order[i] = i;
+  const int rq = c->a.n_heads / c->a.n_kv_heads;
+  auto big = [&](int x) { return hb.q_len[x] * rq > 64; };     // kTtNQ: above it the row-major attention kernel takes the request
   std::stable_sort(hb.order.begin(), hb.order.end(), [&](int x, int y) {
+    if (big(x) != big(y)) return big(x);
     const long long wx = hb.q_len[x] > 0 ? hb.kv_len[x] : -1, wy = hb.q_len[y] > 0 ? hb.kv_len[y] : -1;
     return wx > wy;
   });
+  hb.n_big = 0;
+  for (int i = 0; i < hb.n; ++i) hb.n_big += big(i) ? 1 : 0;
+  hb.qt_off.assign(hb.n + 1, 0);                               // 128-row query tiles per request, prefix sums over `order`
+  for (int i = 0; i < hb.n; ++i) hb.qt_off[i + 1] = hb.qt_off[i] + (hb.q_len[hb.order[i]] * rq + 127) / 128;
+  hb.qt_big = hb.qt_off[hb.n_big]; hb.qt_total = hb.qt_off[hb.n];
   return DLM_OK;
 }
 
 // Descriptor layout in desc_host / desc_dev (ints): slot, q_off, q_len, q_pos0, kv_len, blk_lo, blk_len, row_off, tau, gen_lo,
-// gen_len, order [n each], then tok_bi [T].  Offsets depend on (n, T) only, so a captured graph of the same batch shape can be replayed.
+// gen_len, order [n each], qt_off [n + 1], then tok_bi [T].  Offsets depend on (n, T) only, so a captured graph of the same batch shape can be replayed.
 static size_t fill_desc_host(dlm_ctx* c, const HostBatch& hb) {
   int* h = c->desc_host;
   const size_t n = hb.n;
@@ -1111,16 +1124,17 @@ static size_t fill_desc_host(dlm_ctx* c, const HostBatch& hb) {
   memcpy(h + 9 * n, hb.gen_lo.data(), n * 4);
   memcpy(h + 10 * n, hb.gen_len.data(), n * 4);
   memcpy(h + 11 * n, hb.order.data(), n * 4);
-  memcpy(h + 12 * n, hb.tok_bi.data(), hb.tok_bi.size() * 4);
-  return 12 * n + hb.tok_bi.size();
+  memcpy(h + 12 * n, hb.qt_off.data(), (n + 1) * 4);
+  memcpy(h + 13 * n + 1, hb.tok_bi.data(), hb.tok_bi.size() * 4);
+  return 13 * n + 1 + hb.tok_bi.size();
 }
 static BatchDesc make_desc(dlm_ctx* c, const HostBatch& hb) {
   BatchDesc d;
   const size_t n = hb.n;
   const int* b = c->desc_dev;
-  d.n = hb.n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv; d.min_q_len = std::min(hb.min_q, hb.max_q);
+  d.n = hb.n; d.T = hb.T; d.R = hb.R; d.max_q_len = hb.max_q; d.max_kv_len = hb.max_kv; d.min_q_len = std::min(hb.min_q, hb.max_q); d.n_big = hb.n_big; d.qt_big = hb.qt_big; d.qt_total = hb.qt_total;
   d.slot = b; d.q_off = b + n; d.q_len = b + 2 * n; d.q_pos0 = b + 3 * n; d.kv_len = b + 4 * n; d.blk_lo = b + 5 * n;
-  d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.order = b + 11 * n; d.tok_bi = b + 12 * n;
+  d.blk_len = b + 6 * n; d.row_off = b + 7 * n; d.tau = (const float*)(b + 8 * n); d.order = b + 11 * n; d.qt_off = b + 12 * n; d.tok_bi = b + 13 * n + 1;
   return d;
 }
 
@@ -1392,7 +1406,7 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   const bool use_graph = c->opt_graph && !c->kprof.on && !c->opt_dump;
   bool launched = false;
   if (use_graph) {
-    GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask() | (c->want_feat ? 1 << 16 : 0) | (std::min(hb.min_q, 255) << 20));
+    GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask() | (c->want_feat ? 1 << 16 : 0) | (std::min(hb.min_q, 255) << 20), hb.n_big, hb.qt_big, hb.qt_total);
     GraphEntry& g = c->graphs[key];
     if (g.seen == 1) {                         // second sighting of this batch shape: capture it
       const long long l0 = g_launches;
