@@ -61,9 +61,10 @@ struct GemmPairParams {
 constexpr int kPairThreads = 192;
 constexpr int kPairAccCols = 256;       // TMEM columns per accumulator stage
 
-// A ring stage holds kPairKbPerStage 64-wide K blocks: [A k0][A k1][W k0][W k1] (A 128 x 64, W (bn/2) x 64 per block).  The
-// stage hand-off (TMA -> full barrier -> MMA -> commit -> empty barrier -> producer) has a floor of ~300 ns that neither the
-// MMAs nor the loads explain (DESIGN.md section 6 (1)); two K blocks per hand-off halve it per K block.
+// A ring stage holds kPairKbPerStage 64-wide K blocks: [A k0][A k1][W k0][W k1] (A 128 x 64, W (bn/2) x 64 per block).  Every
+// stage hand-off (full-barrier wait, fence, election, commits in the issuing warp; empty-barrier wait and TMA issue in the
+// producer) costs a few hundred cycles whatever the tile width (DESIGN.md section 6 (1)); with two K blocks per hand-off
+// (eight straight-line MMAs) a 192- or 128-wide tile costs 0.78 / 0.61 of a 256-wide one instead of ~1.
 constexpr int kPairKbPerStage = 2;
 __host__ __device__ inline int gemm_pair_kb_bytes(int bn) { return kATileBytes + bn * 64; }
 __host__ __device__ inline int gemm_pair_stage_bytes(int bn) { return kPairKbPerStage * gemm_pair_kb_bytes(bn); }
