@@ -42,6 +42,11 @@ extern "C" {
 
 #define DLM_DTYPE_F32   0
 #define DLM_DTYPE_BF16  1
+#define DLM_DTYPE_BF16_PRECISE 2   /* precise mode (SURVEY 8(c) protocol P-D): the bf16 model's weight VALUES (Definition W rounded
+                                      to bf16) held in fp32, activations, K/V store and every product in fp32 on the plain CUDA
+                                      kernels.  No activation is rounded to bf16, so committed tokens match the fp64 oracle
+                                      outside the 1e-3 band; slow (SIMT), for parity runs.  Chosen at init because it changes
+                                      the storage type of the weights and of the K/V pages (it is SURVEY's DLM_OPT_PRECISE). */
 
 typedef struct dlm_ctx dlm_ctx;          /* opaque; owns all device memory */
 
@@ -49,7 +54,8 @@ typedef struct dlm_ctx dlm_ctx;          /* opaque; owns all device memory */
 typedef struct {
   int32_t n_layers, d_model, n_heads, n_kv_heads, head_dim, d_ffn, vocab, mask_id;
   int32_t weight_dtype;          /* DLM_DTYPE_F32: fp32 weights, all-fp32 arithmetic (config 1);
-                                    DLM_DTYPE_BF16: bf16 weights, tcgen05 GEMMs, fp32 accumulate/residual */
+                                    DLM_DTYPE_BF16: bf16 weights, tcgen05 GEMMs, fp32 accumulate/residual;
+                                    DLM_DTYPE_BF16_PRECISE: bf16 weight values, all-fp32 arithmetic        */
   float   logit_scale, rms_eps, rope_theta, init_std;
   int32_t max_requests;          /* request slots (cf. maxNumSeqPerBatch)                       */
   int32_t max_seq;               /* longest prompt + generation per request                             */

@@ -703,7 +703,7 @@ static void gen_weight(dlm_ctx* c, void* dst, long long n, int tid) {
   unsigned long long key = mix64(c->seed + DLM_GOLD * (unsigned long long)(tid + 1));
   float cst = (float)((double)c->a.init_std / sqrt(4294967295.0 / 3.0));
   int blocks = (int)std::min<long long>((n + 255) / 256, 148 * 16);
-  init_weight_kernel<TW><<<blocks, 256, 0, c->st>>>((TW*)dst, n, key, cst);
+  init_weight_kernel<TW><<<blocks, 256, 0, c->st>>>((TW*)dst, n, key, cst, c->a.weight_dtype == DLM_DTYPE_BF16_PRECISE ? 1 : 0);
   DLM_LAUNCH_CHECK();
 }
 static void gen_weight_any(dlm_ctx* c, void* dst, long long n, int tid) {
@@ -729,7 +729,7 @@ static int validate_arch(const dlm_arch* a, std::string* err) {
   REQ(a->vocab > 1 && a->mask_id >= 0 && a->mask_id < a->vocab);
   REQ(a->n_heads % a->n_kv_heads == 0 && a->head_dim % 2 == 0 && a->head_dim <= 256);
   REQ(a->d_model % 4 == 0 && a->d_model <= 16384);
-  REQ(a->weight_dtype == DLM_DTYPE_F32 || a->weight_dtype == DLM_DTYPE_BF16);
+  REQ(a->weight_dtype == DLM_DTYPE_F32 || a->weight_dtype == DLM_DTYPE_BF16 || a->weight_dtype == DLM_DTYPE_BF16_PRECISE);
   REQ(a->max_requests > 0 && a->max_seq > 0 && a->max_block > 0 && a->max_block <= 64);
   REQ(a->kv_page_tokens > 0 && a->max_batch_tokens > 0);
   if (a->weight_dtype == DLM_DTYPE_BF16) {

@@ -19,14 +19,18 @@ __host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long 
 }
 #define DLM_GOLD 0x9E3779B97F4A7C15ULL
 
+// round_bf16 (fp32 storage only): the value is rounded to bf16 first, so an fp32-activation instance (DLM_DTYPE_BF16_PRECISE)
+// holds exactly the weights of the bf16 model.
 template <typename TW>
-__global__ void init_weight_kernel(TW* __restrict__ w, long long n, unsigned long long key, float c) {
+__global__ void init_weight_kernel(TW* __restrict__ w, long long n, unsigned long long key, float c, int round_bf16) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   long long stride = (long long)gridDim.x * blockDim.x;
   for (; i < n; i += stride) {
     unsigned long long h = mix64(key + DLM_GOLD * (unsigned long long)(i + 1));
     int s = (int)(h & 0xFFFF) + (int)((h >> 16) & 0xFFFF) + (int)((h >> 32) & 0xFFFF) + (int)(h >> 48) - 131070;
-    w[i] = from_f32<TW>(__fmul_rn((float)s, c));
+    float v = __fmul_rn((float)s, c);
+    if (round_bf16) v = __bfloat162float(__float2bfloat16_rn(v));
+    w[i] = from_f32<TW>(v);
   }
 }
 
