@@ -171,6 +171,14 @@ DLM_API int  dlm_mixed_step(dlm_ctx*, const dlm_batch*, const float* per_request
 /* One-time latency profiling: times synthetic refresh and cached steps over a grid of (requests,
  * tokens, K/V length) with CUDA events and fills rows[0..*n_rows).  Uses scratch requests; needs free slots. */
 DLM_API int  dlm_profile_step_costs(dlm_ctx*, dlm_cost_row* rows, int32_t cap, int32_t* n_rows);
+/* The same with the denoising block length B (<= max_block; dlm_profile_step_costs uses min(32, max_block)) and the number of
+ * timed repeats per row (at least 10 are always taken; a row is their MEDIAN, after two untimed runs).  Rows:
+ *   DLM_KIND_CACHED   n in {1,2,4,8,16,32,64} requests x per-request K/V length in {512,1024,2048,4608}: n_tokens = n*B
+ *                     (the paper's index cacheBlockSize x numReqs; K/V length added), caches built untimed;
+ *   DLM_KIND_REFRESH  total tokens 128, 256, ... 32768 (LP[tp][numTokens]) as one request while it fits max_seq,
+ *                     then as several requests of the largest power of two <= max_seq (kv_tokens = tokens per request).
+ * Combinations that exceed max_requests, max_seq, max_batch_tokens or the free K/V pages are skipped. */
+DLM_API int  dlm_profile_step_costs_ex(dlm_ctx*, int32_t block_len, int32_t repeats, dlm_cost_row* rows, int32_t cap, int32_t* n_rows);
 
 /* Options. */
 #define DLM_OPT_SIMPLE_KERNELS 1   /* 1: run the bf16 model through the plain SIMT kernels (on-device debugging
@@ -184,7 +192,34 @@ DLM_API int  dlm_profile_step_costs(dlm_ctx*, dlm_cost_row* rows, int32_t cap, i
 #define DLM_OPT_TC_ATTENTION   9   /* 1 (default): tcgen05/TMEM attention kernel when a step has enough (request, head) work; 0: mma.sync kernel */
 #define DLM_OPT_FUSE_ROPE     10   /* 1 (default): above 128 tokens RoPE + K/V page write run in the QKV GEMM's epilogue; 0: separate kernel */
 #define DLM_OPT_PAIR_GEMM      8   /* 1 (default): persistent CTA-pair (cta_group::2) GEMM above 128 tokens; 0: single-CTA tile GEMM */
+#define DLM_OPT_TRACE         11   /* 1: every kernel of the next steps stamps %globaltimer into its own record (dlm_step_trace); works
+                                      under CUDA-graph replay and programmatic dependent launch, costs ~3 atomics per CTA      */
+#define DLM_OPT_TCT_MIN_ITEMS 12   /* fewest (request, KV head, query tile) work items for which a step takes the tcgen05 attention
+                                      kernels (default 1: always); below it the mma.sync kernel runs (debugging / A-B timing)  */
 DLM_API int  dlm_set_option(dlm_ctx*, int32_t key, int32_t value);
+
+/* Which kernel families the LAST step launched (bit set), so that a caller -- and the parity tests -- can see when a step
+ * left the tcgen05 / TMA kernels: DLM_PATH_ATTN_PLAIN or DLM_PATH_GEMM_PLAIN on a bf16 model means the SIMT debugging
+ * kernels ran (head_dim != 128 or page_tokens != 64 for attention; DLM_OPT_SIMPLE_KERNELS), which is ~100x slower. */
+#define DLM_PATH_GEMM_SKINNY  0x001u   /* weight-streaming split-K tcgen05 GEMM (<= 128 tokens)          */
+#define DLM_PATH_GEMM_PAIR    0x002u   /* persistent CTA-pair tcgen05 GEMM                               */
+#define DLM_PATH_GEMM_TC      0x004u   /* single-CTA tcgen05 GEMM (LM head <= 128 rows, fallbacks)        */
+#define DLM_PATH_GEMM_PLAIN   0x008u   /* SIMT GEMM (fp32 models, DLM_OPT_SIMPLE_KERNELS)                 */
+#define DLM_PATH_ATTN_TC      0x010u   /* row-major tcgen05 attention                                    */
+#define DLM_PATH_ATTN_TCT     0x020u   /* transposed-score tcgen05 attention                             */
+#define DLM_PATH_ATTN_FLASH   0x040u   /* mma.sync attention                                             */
+#define DLM_PATH_ATTN_PLAIN   0x080u   /* SIMT attention                                                 */
+#define DLM_PATH_ROPE_FUSED   0x100u   /* RoPE + K/V page write in the QKV GEMM's epilogue                */
+#define DLM_PATH_GRAPH_REPLAY 0x200u   /* the step was one CUDA-graph launch                             */
+DLM_API uint32_t dlm_last_step_kernels(dlm_ctx*);
+
+/* Timeline of the LAST step taken with DLM_OPT_TRACE = 1, one row per kernel launch in launch order: microseconds since the
+ * step's first kernel began -- begin: first CTA entered the kernel; wait: griddepcontrol.wait first returned in it, i.e. the
+ * kernel before it in the stream had completed (= begin without programmatic dependent launch); end: last CTA left.
+ * The time a launch holds the step's critical path is wait(next launch) - wait(this launch); these sum to the step's
+ * duration, which overlapping CUDA-event pairs cannot give.  kernel = DLM_K_* class. */
+typedef struct { int32_t kernel, slot; float begin_us, wait_us, end_us; } dlm_trace_row;
+DLM_API int  dlm_step_trace(dlm_ctx*, dlm_trace_row* rows, int32_t cap, int32_t* n_rows);
 
 /* Per-kernel-class device time accumulated over the steps run with DLM_OPT_KERNEL_TIMING = 1 (CUDA events on
  * the library's stream around each launch; the measurement behind bench.py's roofline object, P:123 profiling).
@@ -209,8 +244,8 @@ DLM_API int  dlm_kernel_times(dlm_ctx*, dlm_kernel_time* rows, int32_t cap, int3
 #define DLM_T_X_IN    0   /* residual stream entering the layer        [rows, d]      fp32 */
 #define DLM_T_NORM1   1   /* RMSNorm(x) fed to the QKV GEMM            [rows, d]           */
 #define DLM_T_Q       2   /* Q after RoPE                              [rows, H*d_h]       */
-#define DLM_T_K       3   /* K after RoPE, as written to the store     [rows, H_kv*d_h]    */
-#define DLM_T_V       4   /* V as written to the store                 [rows, H_kv*d_h]    */
+#define DLM_T_K       3   /* K after RoPE, as written to the store     [rows, H_kv*d_h]    (read back from the pages; needs no dump) */
+#define DLM_T_V       4   /* V as written to the store                 [rows, H_kv*d_h]    (read back from the pages; needs no dump) */
 #define DLM_T_ATTN    5   /* attention output                          [rows, H*d_h]       */
 #define DLM_T_X_MID   6   /* residual after O-proj                     [rows, d]      fp32 */
 #define DLM_T_NORM2   7   /* RMSNorm(x_mid) fed to gate/up             [rows, d]           */
@@ -221,7 +256,7 @@ DLM_API int  dlm_kernel_times(dlm_ctx*, dlm_kernel_time* rows, int32_t cap, int3
 #define DLM_T_VCACHE  12  /* the request's stored V for ALL S positions [S, H_kv*d_h]      */
 DLM_API int64_t dlm_debug_tensor(dlm_ctx*, int32_t req, int32_t layer, int32_t which, float* out, int64_t cap_floats);
 
-/* Counters: kernels launched by this library since dlm_init (bench.py's gpu_launches). */
+/* Counters: kernels launched for this context since dlm_init returned (bench.py's gpu_launches). */
 DLM_API int64_t dlm_launch_count(dlm_ctx*);
 /* Device time of the last step in microseconds (CUDA events on the library's stream). */
 DLM_API float dlm_last_step_usec(dlm_ctx*);

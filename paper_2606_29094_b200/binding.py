@@ -19,6 +19,9 @@ LIB_PATH = os.path.join(_HERE, "libdlm.so")
 DLM_OK, DLM_E_ARG, DLM_E_CAPACITY, DLM_E_STATE, DLM_E_CUDA = 0, -1, -2, -3, -4
 DLM_DRY_RUN = 1
 OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM, OPT_PAIR_GEMM, OPT_TC_ATTENTION, OPT_FUSE_ROPE = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
+OPT_TRACE, OPT_TCT_MIN_ITEMS = 11, 12
+DTYPE_F32, DTYPE_BF16, DTYPE_BF16_PRECISE = 0, 1, 2
+PATH_GEMM_SKINNY, PATH_GEMM_PAIR, PATH_GEMM_TC, PATH_GEMM_PLAIN, PATH_ATTN_TC, PATH_ATTN_TCT, PATH_ATTN_FLASH, PATH_ATTN_PLAIN, PATH_ROPE_FUSED, PATH_GRAPH_REPLAY = (1 << i for i in range(10))
 KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
                 "combine_unmask")
 KIND_REFRESH, KIND_CACHED, KIND_MIXED = 0, 1, 2
@@ -71,6 +74,10 @@ class _KernelTime(C.Structure):
     _fields_ = [("kernel", C.c_int32), ("launches", C.c_int32), ("usec", C.c_float)]
 
 
+class _TraceRow(C.Structure):
+    _fields_ = [("kernel", C.c_int32), ("slot", C.c_int32), ("begin_us", C.c_float), ("wait_us", C.c_float), ("end_us", C.c_float)]
+
+
 _lib = None
 
 
@@ -99,6 +106,10 @@ def lib() -> C.CDLL:
         L.dlm_cached_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(f32), C.POINTER(_Result)]
         L.dlm_mixed_step.argtypes = [vp, C.POINTER(_Batch), C.POINTER(f32), C.POINTER(_Result)]
         L.dlm_profile_step_costs.argtypes = [vp, C.POINTER(_CostRow), i32, C.POINTER(i32)]
+        L.dlm_profile_step_costs_ex.argtypes = [vp, i32, i32, C.POINTER(_CostRow), i32, C.POINTER(i32)]
+        L.dlm_last_step_kernels.argtypes = [vp]
+        L.dlm_last_step_kernels.restype = C.c_uint32
+        L.dlm_step_trace.argtypes = [vp, C.POINTER(_TraceRow), i32, C.POINTER(i32)]
         L.dlm_set_option.argtypes = [vp, i32, i32]
         L.dlm_kernel_times.argtypes = [vp, C.POINTER(_KernelTime), i32, C.POINTER(i32), i32]
         L.dlm_debug_tensor.argtypes = [vp, i32, i32, i32, C.POINTER(f32), i64]
@@ -323,10 +334,24 @@ class Engine:
         self._check(lib().dlm_kernel_times(self._h, rows, 32, C.byref(n), 1 if reset else 0))
         return {KERNEL_NAMES[rows[i].kernel]: (rows[i].launches, rows[i].usec) for i in range(n.value)}
 
-    def profile_step_costs(self, cap: int = 128):
+    def last_step_kernels(self) -> int:
+        """PATH_* bit set of the kernel families the last step launched."""
+        return int(lib().dlm_last_step_kernels(self._h))
+
+    def step_trace(self):
+        """Timeline of the last step taken with OPT_TRACE: [(kernel class name, begin_us, wait_us, end_us)] in launch order."""
+        rows = (_TraceRow * 2048)()
+        n = C.c_int32(0)
+        self._check(lib().dlm_step_trace(self._h, rows, 2048, C.byref(n)))
+        return [(KERNEL_NAMES[rows[i].kernel], rows[i].begin_us, rows[i].wait_us, rows[i].end_us) for i in range(n.value)]
+
+    def profile_step_costs(self, cap: int = 128, block_len: Optional[int] = None, repeats: int = 10):
         rows = (_CostRow * cap)()
         n = C.c_int32(0)
-        self._check(lib().dlm_profile_step_costs(self._h, rows, cap, C.byref(n)))
+        if block_len is None:
+            self._check(lib().dlm_profile_step_costs(self._h, rows, cap, C.byref(n)))
+        else:
+            self._check(lib().dlm_profile_step_costs_ex(self._h, block_len, repeats, rows, cap, C.byref(n)))
         return [dict(kind="refresh" if rows[i].kind == KIND_REFRESH else "cached", n_requests=rows[i].n_requests,
                      n_tokens=rows[i].n_tokens, kv_tokens=rows[i].kv_tokens, usec=rows[i].usec) for i in range(n.value)]
 

@@ -61,12 +61,12 @@ struct FaParams {
   float scale_log2;         // (1/sqrt(d_h)) * log2(e)
   float* ws_o;              // [splits, T*H, 128] unnormalised partial outputs (splits > 1)
   float* ws_ml;             // [splits, T*H, 2]   (running max in log2 units, running sum)
+  TraceSlot tr;             // DLM_OPT_TRACE record of this launch (null: off)
 };
 
 __global__ void __launch_bounds__(kFaThreads) attn_flash_kernel(const FaParams p) {
   extern __shared__ __align__(128) uint8_t fa_smem[];
-  pdl_launch_dependents();
-  pdl_wait();
+  DLM_PROLOGUE(p.tr);
   const int bi = blockIdx.z / p.splits, split = blockIdx.z % p.splits;
   const int kvh = blockIdx.y;
   const int r = p.n_heads / p.g.n_kv_heads;
@@ -222,9 +222,9 @@ __global__ void __launch_bounds__(kFaThreads) attn_flash_kernel(const FaParams p
 
 // merge split partials: out = sum_s o_s 2^(m_s - m) / sum_s l_s 2^(m_s - m)
 __global__ void __launch_bounds__(kFaDh) attn_combine_kernel(bf16* __restrict__ out, const float* __restrict__ ws_o,
-                                                             const float* __restrict__ ws_ml, long long TH, int splits) {
-  pdl_launch_dependents();
-  pdl_wait();
+                                                             const float* __restrict__ ws_ml, long long TH, int splits,
+                                                             TraceSlot tr = TraceSlot{nullptr}) {
+  DLM_PROLOGUE(tr);
   const long long row = blockIdx.x;
   const int e = threadIdx.x;
   float m = -CUDART_INF_F;
@@ -238,19 +238,21 @@ __global__ void __launch_bounds__(kFaDh) attn_combine_kernel(bf16* __restrict__ 
     acc += ws_o[(s * TH + row) * kFaDh + e] * w;
   }
   out[row * kFaDh + e] = __float2bfloat16_rn(acc / l);
+  DLM_EPILOGUE(tr);
 }
 
 // Host launcher.  *done = false when the shape is not supported (caller falls back to the plain kernel).
 static int attn_flash_launch(bf16* out, const bf16* q, const bf16* kv_store, const int* page_table, const BatchDesc& bd,
                              const KvGeom& g, int layer, int n_heads, float scale, float** ws, size_t* ws_bytes, int num_sms,
-                             cudaStream_t st, bool pdl, std::string* err, bool* done) {
+                             cudaStream_t st, bool pdl, std::string* err, bool* done, TraceSlot tr0 = TraceSlot{nullptr},
+                             TraceSlot tr1 = TraceSlot{nullptr}) {
   *done = false;
   if (g.head_dim != kFaDh || g.page_tokens % kFaBN != 0 || bd.T <= 0) return 0;
-  static bool configured = false;
-  if (!configured) {
+  static bool configured[kMaxDevices] = {};
+  if (!configured[g_dev]) {
     cudaError_t e = cudaFuncSetAttribute(attn_flash_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kFaSmem);
     if (e != cudaSuccess) { *err = std::string("attn_flash: ") + cudaGetErrorString(e); return -4; }
-    configured = true;
+    configured[g_dev] = true;
   }
   const int r = n_heads / g.n_kv_heads;
   const int q_tiles = (bd.max_q_len * r + kFaBM - 1) / kFaBM;
@@ -269,7 +271,7 @@ static int attn_flash_launch(bf16* out, const bf16* q, const bf16* kv_store, con
   splits = std::max(1, std::min(splits, 32));
   FaParams p;
   p.out = out; p.q = q; p.kv_store = kv_store; p.page_table = page_table; p.b = bd; p.g = g; p.layer = layer; p.n_heads = n_heads;
-  p.splits = splits; p.scale_log2 = scale * 1.4426950408889634f; p.ws_o = nullptr; p.ws_ml = nullptr;
+  p.splits = splits; p.scale_log2 = scale * 1.4426950408889634f; p.ws_o = nullptr; p.ws_ml = nullptr; p.tr = tr0;
   const long long TH = (long long)bd.T * n_heads;
   // the split-KV workspace is allocated once by the caller (captured CUDA graphs keep its address): fit the split to it
   while (splits > 1 && (size_t)splits * TH * (kFaDh + 2) * 4 > *ws_bytes) --splits;
@@ -289,7 +291,7 @@ static int attn_flash_launch(bf16* out, const bf16* q, const bf16* kv_store, con
   DLM_LAUNCH_CHECK();
   if (splits > 1 && e == cudaSuccess) {
     cfg.gridDim = dim3((unsigned)TH); cfg.blockDim = dim3(kFaDh); cfg.dynamicSmemBytes = 0;
-    e = cudaLaunchKernelEx(&cfg, attn_combine_kernel, out, (const float*)p.ws_o, (const float*)p.ws_ml, TH, splits);
+    e = cudaLaunchKernelEx(&cfg, attn_combine_kernel, out, (const float*)p.ws_o, (const float*)p.ws_ml, TH, splits, tr1);
     DLM_LAUNCH_CHECK();
   }
   if (e != cudaSuccess) { *err = std::string("attn_flash launch: ") + cudaGetErrorString(e); return -4; }

@@ -49,6 +49,7 @@ struct TaParams {
   int row_filter;           // mixed steps: 0 all requests, 1 only those with <= 64 stacked rows, 2 only those with more
   int req_lo, req_n;        // entries [req_lo, req_lo + req_n) of BatchDesc::order are this launch's requests
   int ragged_q;             // 1: items enumerate the requests' own query tiles (BatchDesc::qt_off), no empty slots for short requests
+  TraceSlot tr;             // DLM_OPT_TRACE record of this launch (null: off)
 };
 
 namespace ptx {
@@ -148,6 +149,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tc_kernel(const __grid_con
   const int H = p.n_heads;
 
   pdl_launch_dependents();
+  if (threadIdx.x == 0) trace_begin(p.tr);
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&mapKV);
     for (int s = 0; s < kTaKStages; ++s) { ptx::mbar_init(k_full(s), 1); ptx::mbar_init(k_empty(s), 1); }
@@ -168,6 +170,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tc_kernel(const __grid_con
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr));
   const uint32_t tmem_o = tmem_base + 256;          // S buffers at columns 0 and 128, O at 256
   pdl_wait();                                       // q and the block's fresh K/V come from the upstream kernels
+  if (threadIdx.x == 0) trace_wait(p.tr);
 
   if (warp == 0) {
     if (ptx::elect_one()) {        // one elected lane of the converged warp: TMA issues compile straight-line
@@ -478,6 +481,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tc_kernel(const __grid_con
   }
   ptx::tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) trace_end(p.tr);
   if (warp == 2) ptx::tmem_dealloc(tmem_base, 512);
 }
 

@@ -53,6 +53,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
   const int H = p.n_heads;
 
   pdl_launch_dependents();
+  if (threadIdx.x == 0) trace_begin(p.tr);
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&mapKV);
     for (int s = 0; s < kTaKStages; ++s) { ptx::mbar_init(k_full(s), 1); ptx::mbar_init(k_empty(s), 1); }
@@ -73,6 +74,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr));
   const uint32_t tmem_o = tmem_base + 128;          // S^T buffers at columns 0 and 64, O^T at 128
   pdl_wait();
+  if (threadIdx.x == 0) trace_wait(p.tr);
 
   if (warp == 0) {
     if (ptx::elect_one()) {        // one elected lane of the converged warp: TMA issues compile straight-line
@@ -400,6 +402,7 @@ __global__ void __launch_bounds__(kTaThreads, 1) attn_tct_kernel(const __grid_co
   }
   ptx::tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) trace_end(p.tr);
   if (warp == 2) ptx::tmem_dealloc(tmem_base, 256);
 }
 

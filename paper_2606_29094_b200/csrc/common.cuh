@@ -70,8 +70,31 @@ struct KvGeom {
   }
 };
 
-extern long long g_launches;   // kernels launched by this library (dlm_launch_count)
+// Per-thread launch bookkeeping: a ctx is used from one thread at a time, so the entry points (DevGuard in engine.cu) bind
+// the thread to the context's device and credit the kernels launched in between to that context (dlm_launch_count).
+extern thread_local long long g_launches;   // kernels launched by this thread
+extern thread_local int g_num_sms;          // SM count of the device the thread is bound to
+extern thread_local int g_dev;              // that device's ordinal (index of the per-device one-time kernel configuration)
+constexpr int kMaxDevices = 64;
 
 #define DLM_LAUNCH_CHECK() do { ::dlm::g_launches++; } while (0)
+
+// In-kernel timeline (DLM_OPT_TRACE): every launch of a step owns one record of three 64-bit words in global memory,
+//   [0] min over CTAs of %globaltimer at kernel entry, [1] min of the time griddepcontrol.wait returned (= the upstream
+//   kernel has completed), [2] min of ~%globaltimer at exit (i.e. the complement of the latest exit).
+// A null pointer (tracing off, the default) costs one predicated branch per CTA.  Works under CUDA-graph replay and
+// programmatic dependent launch, where host-side events cannot separate overlapping kernels.
+struct TraceSlot { unsigned long long* p; };
+__device__ __forceinline__ unsigned long long gtimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ void trace_begin(const TraceSlot& tr) { if (tr.p) atomicMin(tr.p, gtimer_ns()); }
+__device__ __forceinline__ void trace_wait(const TraceSlot& tr) { if (tr.p) atomicMin(tr.p + 1, gtimer_ns()); }
+__device__ __forceinline__ void trace_end(const TraceSlot& tr) { if (tr.p) atomicMin(tr.p + 2, ~gtimer_ns()); }
+// prologue of the small kernels: let the successor start, stamp, wait for the predecessor, stamp
+#define DLM_PROLOGUE(tr) do { pdl_launch_dependents(); if (threadIdx.x == 0) trace_begin(tr); pdl_wait(); if (threadIdx.x == 0) trace_wait(tr); } while (0)
+#define DLM_EPILOGUE(tr) do { if (threadIdx.x == 0) trace_end(tr); } while (0)
 
 }  // namespace dlm

@@ -26,8 +26,10 @@
 #include "kernels_basic.cuh"
 
 namespace dlm {
-long long g_launches = 0;
-static std::string g_init_error;
+thread_local long long g_launches = 0;
+thread_local int g_num_sms = 148;
+thread_local int g_dev = 0;
+static thread_local std::string g_init_error;
 
 static void set_err(std::string* dst, const char* fmt, ...) {
   char buf[1024];
@@ -51,7 +53,10 @@ static cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_
     cfg.attrs = at; cfg.numAttrs = 1;
   }
   g_launches++;
-  return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+  if constexpr (sizeof...(Args) + 1 == sizeof...(KArgs))       // caller left out the trailing TraceSlot: tracing off for this launch
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)..., TraceSlot{nullptr});
+  else
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
 }
 
 #define CU_TRY(ctx_err, expr)                                                                         \
@@ -163,8 +168,6 @@ struct TmapCache {
 // ------------------------------------------------------------------------------------------------
 // tcgen05 GEMM launcher
 // ------------------------------------------------------------------------------------------------
-static int g_num_sms = 148;
-
 static int pick_bn(int M, int N, int epi) {
   // N = output features (SwiGLU: F, each tile covers bn/2).  Aim for one resident wave of equal tiles:
   // the largest tile that still yields >= ~0.8 * SMs CTAs; when even the smallest cannot, take the smallest.
@@ -185,12 +188,12 @@ static int pick_bn(int M, int N, int epi) {
 template <int EPI>
 static cudaError_t launch_gemm_tc_t(const CUtensorMap* ma, const CUtensorMap* mb, const GemmTcParams& p, int n_tiles_x,
                                     cudaStream_t st, bool pdl) {
-  static int configured = 0;
+  static bool configured[kMaxDevices] = {};     // one-time per device (a process may hold contexts on several GPUs)
   const int smem = gemm_tc_smem_bytes(p.bn, p.stages);
-  if (configured < smem) {
+  if (!configured[g_dev]) {
     cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    configured = 227 * 1024;
+    configured[g_dev] = true;
   }
   dim3 grid(n_tiles_x, (p.M + 127) / 128);
   return launch_k(gemm_tc_kernel<EPI>, grid, dim3(kGemmThreads), (size_t)smem, st, pdl, *ma, *mb, p);
@@ -267,11 +270,11 @@ static void plan_pair(int M, int N, int K, int epi, int max_splits, int* bn_out,
 
 template <int EPI>
 static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* mb, const CUtensorMap* mc, const GemmPairParams& p, cudaStream_t st, bool pdl) {
-  static bool configured = false;
-  if (!configured) {
+  static bool configured[kMaxDevices] = {};
+  if (!configured[g_dev]) {
     cudaError_t e = cudaFuncSetAttribute(gemm_pair_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    configured = true;
+    configured[g_dev] = true;
   }
   const int pairs = std::max(1, std::min(g_num_sms / 2, p.m_tiles * p.n_tiles_n * p.splits));
   cudaLaunchConfig_t cfg = {};
@@ -346,8 +349,13 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
 // ------------------------------------------------------------------------------------------------
 static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* kv_store, int n_layers_total, const int* page_table,
                           const BatchDesc& bd, const KvGeom& g, int layer, int n_heads, float scale, float** ws, size_t* ws_bytes,
-                          cudaStream_t st, bool pdl, std::string* err, bool* done, int force = 0) {
+                          cudaStream_t st, bool pdl, std::string* err, bool* done, int force = 0, const TraceSlot* tr = nullptr,
+                          unsigned* paths = nullptr, int min_items = 64) {
   *done = false;
+  static const TraceSlot no_trace[3] = {{nullptr}, {nullptr}, {nullptr}};
+  if (!tr) tr = no_trace;                      // tr[0..2]: records of up to three launches (DLM_OPT_TRACE)
+  unsigned path_dummy = 0;
+  if (!paths) paths = &path_dummy;
   if (g.head_dim != 128 || g.page_tokens != 64 || bd.T <= 0) return 0;
   const int r = n_heads / g.n_kv_heads;
   const int q_tiles = (bd.max_q_len * r + kTaTile - 1) / kTaTile;
@@ -356,7 +364,7 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   const int kv_tiles = (bd.max_kv_len + kTaTile - 1) / kTaTile;
   const bool no_transposed = force >= 100;      // test hook: 100 + f = attn_tc_kernel even when the transposed kernel fits
   if (no_transposed) force -= 100;
-  if (!force && items < 64) return 0;       // too few (request, head, query tile) items to fill the SMs with one CTA each
+  if (!force && items < min_items) return 0;       // too few (request, head, query tile) items to fill the SMs with one CTA each
   const long long rows = (long long)n_layers_total * g.n_pages * 2 * g.n_kv_heads * g.page_tokens;
   if (rows >= (1LL << 31)) return 0;
   int splits = 1;
@@ -379,19 +387,19 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
   if (two_kernels) splits = 1;
   const CUtensorMap* mkv = tc.get(kv_store, rows, 128, 64);
   if (!mkv) { set_err(err, "cuTensorMapEncodeTiled failed (attention K/V store %p, %lld rows)", (const void*)kv_store, rows); return DLM_E_CUDA; }
-  static bool configured = false;
-  if (!configured) {
+  static bool configured[kMaxDevices] = {};
+  if (!configured[g_dev]) {
     cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTaSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(attn_tct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTtSmem);
     if (e != cudaSuccess) { set_err(err, "attn_tc: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
-    configured = true;
+    configured[g_dev] = true;
   }
   TaParams p;
   p.out = out; p.q = q; p.page_table = page_table; p.b = bd; p.g = g; p.layer = layer; p.n_heads = n_heads;
   p.splits = splits; p.q_tiles_max = q_tiles; p.n_items = (int)(items * splits);
   p.scale_log2 = scale * 1.4426950408889634f; p.ws_o = nullptr; p.ws_ml = nullptr;
   p.kv_policy = q_tiles == 1 ? DLM_L2_EVICT_FIRST : DLM_L2_EVICT_NORMAL;
-  p.row_filter = 0; p.req_lo = 0; p.req_n = bd.n; p.ragged_q = 0;
+  p.row_filter = 0; p.req_lo = 0; p.req_n = bd.n; p.ragged_q = 0; p.tr = TraceSlot{nullptr};
   const long long TH = (long long)bd.T * n_heads;
   while (splits > 1 && (size_t)splits * TH * (128 + 2) * 4 > *ws_bytes) --splits;     // fixed workspace (see attn_flash_launch)
   p.splits = splits; p.n_items = (int)(items * splits);
@@ -406,19 +414,23 @@ static int attn_tc_launch(TmapCache& tc, bf16* out, const bf16* q, const bf16* k
     pt.req_n = bd.n - bd.n_big;
     p.row_filter = 2; p.req_n = bd.n_big; p.ragged_q = 1; p.n_items = bd.qt_big * g.n_kv_heads;
     if (pt.n_items <= 0 || p.n_items <= 0) { set_err(err, "attn_tc: inconsistent mixed batch (%d of %d requests above 64 rows)", bd.n_big, bd.n); return DLM_E_ARG; }
+    pt.tr = tr[0]; p.tr = tr[1];
     cudaError_t e2 = launch_k(attn_tct_kernel, dim3((unsigned)std::min(g_num_sms, pt.n_items)), dim3(kTaThreads), (size_t)kTtSmem, st, pdl, *mkv, pt);
     if (e2 == cudaSuccess)
       e2 = launch_k(attn_tc_kernel, dim3((unsigned)std::min<long long>(g_num_sms, p.n_items)), dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
     if (e2 != cudaSuccess) { set_err(err, "attn_tc launch: %s", cudaGetErrorString(e2)); return DLM_E_CUDA; }
+    *paths |= DLM_PATH_ATTN_TC | DLM_PATH_ATTN_TCT;
     *done = true;
     return 0;
   }
   if (ragged && !transposed) p.ragged_q = 1;
+  p.tr = tr[0];
+  *paths |= transposed ? DLM_PATH_ATTN_TCT : DLM_PATH_ATTN_TC;
   const dim3 grid((unsigned)std::min<long long>(g_num_sms, p.n_items));
   cudaError_t e = transposed ? launch_k(attn_tct_kernel, grid, dim3(kTaThreads), (size_t)kTtSmem, st, pdl, *mkv, p)
                              : launch_k(attn_tc_kernel, grid, dim3(kTaThreads), (size_t)kTaSmem, st, pdl, *mkv, p);
   if (splits > 1 && e == cudaSuccess)
-    e = launch_k(attn_combine_kernel, dim3((unsigned)TH), dim3(kFaDh), 0, st, pdl, out, (const float*)p.ws_o, (const float*)p.ws_ml, TH, splits);
+    e = launch_k(attn_combine_kernel, dim3((unsigned)TH), dim3(kFaDh), 0, st, pdl, out, (const float*)p.ws_o, (const float*)p.ws_ml, TH, splits, tr[1]);
   if (e != cudaSuccess) { set_err(err, "attn_tc launch: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
   *done = true;
   return 0;
@@ -461,13 +473,13 @@ static int gemm_skinny(TmapCache& tc, std::string* err, const void* X, long long
   const CUtensorMap* mx = tc.get(X, x_rows_cap, K, p.tpad);
   if (!mw || !mx) { set_err(err, "cuTensorMapEncodeTiled failed (gemm_skinny X=%p W=%p)", X, W); return DLM_E_CUDA; }
   const int smem = skinny_smem_bytes(p.tpad, p.stages, epi);
-  static bool configured[2] = {false, false};
+  static bool configured[kMaxDevices][2] = {};
   cudaError_t e = cudaSuccess;
-  if (!configured[epi]) {
+  if (!configured[g_dev][epi]) {
     e = epi == SK_SWIGLU ? cudaFuncSetAttribute(gemm_skinny_kernel<SK_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024)
                          : cudaFuncSetAttribute(gemm_skinny_kernel<SK_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024);
     if (e != cudaSuccess) { set_err(err, "gemm_skinny: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
-    configured[epi] = true;
+    configured[g_dev][epi] = true;
   }
   dim3 grid(n_tiles, p.splits);
   e = epi == SK_SWIGLU ? launch_k(gemm_skinny_kernel<SK_SWIGLU>, grid, dim3(kSkThreads), (size_t)smem, st, pdl, *mw, *mx, p)
@@ -597,12 +609,17 @@ struct KProf {
 };
 
 typedef std::tuple<int, int, int, int, int, int, int, int, int, int, int> GraphKey;   // kind, dry, n, T, R, max_q, max_kv, options, n_big, qt_big, qt_total
-struct GraphEntry { int seen = 0; cudaGraphExec_t exec = nullptr; long long launches = 0; };
+struct GraphEntry { int seen = 0; cudaGraphExec_t exec = nullptr; long long launches = 0; unsigned paths = 0; unsigned long long used = 0; std::vector<int> trace_cls; };
+constexpr size_t kMaxGraphs = 64;          // captured step graphs kept per context (least recently used evicted)
+constexpr int kMaxTraceSlots = 2048;       // launches of one step that DLM_OPT_TRACE can record
 
 struct dlm_ctx {
   dlm_arch a;
   uint64_t seed;
   dlm_mem mem;
+  int device = 0;              // the CUDA device the context lives on; every entry point binds the calling thread to it
+  int num_sms = 148;
+  long long launches = 0;      // kernels launched for this context (dlm_launch_count)
   bool own_stream = false;
   cudaStream_t st = nullptr;
   std::string err;
@@ -639,8 +656,22 @@ struct dlm_ctx {
   long long part_rows = 0, qkv_rows = 0;
   // options
   int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1, opt_tcattn = 1, opt_fuse_rope = 1;
-  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4) | (opt_tcattn << 5) | (opt_fuse_rope << 6); }
+  int opt_trace = 0;
+  int opt_tct_min_items = 64;  // fewest (request, KV head, query tile) items for which a step takes the tcgen05 attention kernels
+  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4) | (opt_tcattn << 5) | (opt_fuse_rope << 6) | (opt_trace << 7); }
   std::map<GraphKey, GraphEntry> graphs;
+  unsigned long long graph_clock = 0;
+  unsigned paths = 0, last_paths = 0;   // DLM_PATH_* of the step being enqueued / of the last step
+  // in-kernel timeline (DLM_OPT_TRACE): one record of 3 x u64 per launch, classes in launch order
+  unsigned long long* trace_dev = nullptr;
+  std::vector<int> trace_cls, last_trace_cls;
+  std::vector<unsigned long long> trace_host;
+  int cur_cls = 0;
+  TraceSlot tslot() {
+    if (!opt_trace || !trace_dev || (int)trace_cls.size() >= kMaxTraceSlots) return TraceSlot{nullptr};
+    trace_cls.push_back(cur_cls);
+    return TraceSlot{trace_dev + 3 * (trace_cls.size() - 1)};
+  }
   // debug dump
   std::map<std::pair<int, int>, void*> dump;   // (layer, which) -> device copy [T, width]
   HostBatch last_batch;
@@ -668,8 +699,27 @@ struct dlm_ctx {
 
 struct KScope {
   dlm_ctx* c;
-  KScope(dlm_ctx* c_, int k) : c(c_) { if (c->kprof.on) c->kprof.begin(k, c->st); }
+  KScope(dlm_ctx* c_, int k) : c(c_) { c->cur_cls = k; if (c->kprof.on) c->kprof.begin(k, c->st); }
   ~KScope() { if (c->kprof.on) c->kprof.end(c->st); }
+};
+
+// Every entry point that takes a ctx binds the calling thread to the context's device for the duration of the call (a
+// request may be imported into a context on another GPU of the same process) and credits its launches to the context.
+struct DevGuard {
+  dlm_ctx* c;
+  int prev = -1;
+  long long l0;
+  explicit DevGuard(dlm_ctx* c_) : c(c_), l0(g_launches) {
+    if (!c) return;
+    cudaGetDevice(&prev);
+    if (prev != c->device) cudaSetDevice(c->device);
+    g_dev = c->device; g_num_sms = c->num_sms;
+  }
+  ~DevGuard() {
+    if (!c) return;
+    c->launches += g_launches - l0;
+    if (prev >= 0 && prev != c->device) cudaSetDevice(prev);
+  }
 };
 
 static int norm_threads(int d) { return std::min(1024, ((d / 4) + 31) / 32 * 32); }
@@ -679,17 +729,18 @@ static int norm_threads(int d) { return std::min(1024, ((d / 4) + 31) / 32 * 32)
 template <typename TE>
 static void launch_rmsnorm(dlm_ctx* c, TE* u, float* x, const int* row_src, int rows, int d, float eps, const float* part, int n_part,
                            long long part_stride, bool pdl) {
+  const TraceSlot tr = c->tslot();
   if (rows >= 1024 && d <= 4096)        // register-resident row: 3.46 -> 2.00 ms per C3 mixed step; slower below ~1000 rows
-    launch_k(rmsnorm_warp_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride);
+    launch_k(rmsnorm_warp_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride, tr);
   else if (rows >= 1024)
-    launch_k(rmsnorm_rows_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride);
+    launch_k(rmsnorm_rows_kernel<TE>, dim3((rows + 3) / 4), dim3(128), 0, c->st, pdl, u, x, row_src, rows, d, eps, part, n_part, part_stride, tr);
   else
   {
     // more rows than two resident 1024-thread blocks per SM can hold: 256-thread blocks (4 float4 per thread) keep every
     // row of a 512-token step in flight in one wave
     int threads = norm_threads(d);
     if (rows > 2 * g_num_sms && d >= 1024 && d <= 4096) threads = 256;
-    launch_k(rmsnorm_kernel<TE>, dim3(rows), dim3(threads), 0, c->st, pdl, u, x, row_src, d, eps, part, n_part, part_stride);
+    launch_k(rmsnorm_kernel<TE>, dim3(rows), dim3(threads), 0, c->st, pdl, u, x, row_src, d, eps, part, n_part, part_stride, tr);
   }
 }
 
@@ -755,6 +806,7 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   c->seed = seed;
   if (mem) c->mem = *mem; else memset(&c->mem, 0, sizeof c->mem);
   std::string* err = &g_init_error;
+  cudaGetDevice(&c->device);             // the context lives on the caller's current device
 #define FAIL(code, ...) do { set_err(err, __VA_ARGS__); dlm_destroy(c); return code; } while (0)
   if (c->mem.cuda_stream) c->st = (cudaStream_t)c->mem.cuda_stream;
   else { if (cudaStreamCreateWithFlags(&c->st, cudaStreamNonBlocking) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaStreamCreate failed"); c->own_stream = true; }
@@ -762,7 +814,9 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   int dev = 0;
   cudaGetDevice(&dev);
   cudaGetDeviceProperties(&prop, dev);
-  g_num_sms = prop.multiProcessorCount;
+  if (dev < 0 || dev >= kMaxDevices) FAIL(DLM_E_CUDA, "device ordinal %d not supported", dev);
+  c->device = dev; c->num_sms = prop.multiProcessorCount;
+  g_dev = dev; g_num_sms = c->num_sms;
   const dlm_arch& a = c->a;
   c->bf16_model = a.weight_dtype == DLM_DTYPE_BF16;
   c->esize = c->bf16_model ? 2 : 4;
@@ -848,12 +902,14 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   cudaMemsetAsync(c->conf_state, 0, (size_t)a.max_requests * a.max_seq * 4, c->st);
   ALLOC(c->out_dev, c->out_bytes);
   if (cudaMallocHost(&c->out_host, c->out_bytes) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
+  ALLOC(c->trace_dev, (size_t)kMaxTraceSlots * 3 * 8);
   cudaEventCreate(&c->ev0);
   cudaEventCreate(&c->ev1);
   cudaError_t e = cudaStreamSynchronize(c->st);
   if (e != cudaSuccess) FAIL(DLM_E_CUDA, "weight generation failed: %s", cudaGetErrorString(e));
 #undef ALLOC
 #undef FAIL
+  c->launches = 0;                       // weight generation is set-up, not step work
   *out = c;
   return DLM_OK;
 }
@@ -862,6 +918,9 @@ extern "C" int dlm_init(const dlm_arch* arch, uint64_t seed, dlm_ctx** out) { re
 
 extern "C" void dlm_destroy(dlm_ctx* c) {
   if (!c) return;
+  int prev = -1;
+  cudaGetDevice(&prev);
+  if (prev != c->device) cudaSetDevice(c->device);
   if (c->st) cudaStreamSynchronize(c->st);
   for (auto& kv : c->dump) cudaFree(kv.second);
   for (auto& g : c->graphs) if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
@@ -873,11 +932,13 @@ extern "C" void dlm_destroy(dlm_ctx* c) {
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);
   if (c->own_stream && c->st) cudaStreamDestroy(c->st);
+  if (prev >= 0 && prev != c->device) cudaSetDevice(prev);
   delete c;
 }
 
 extern "C" const char* dlm_last_error(dlm_ctx* c) { return c ? c->err.c_str() : g_init_error.c_str(); }
-extern "C" int64_t dlm_launch_count(dlm_ctx*) { return g_launches; }
+extern "C" int64_t dlm_launch_count(dlm_ctx* c) { return c ? c->launches : 0; }
+extern "C" uint32_t dlm_last_step_kernels(dlm_ctx* c) { return c ? c->last_paths : 0; }
 extern "C" float dlm_last_step_usec(dlm_ctx* c) { return c ? c->last_usec : 0.f; }
 
 extern "C" int dlm_kernel_times(dlm_ctx* c, dlm_kernel_time* rows, int32_t cap, int32_t* n_rows, int32_t reset) {
@@ -889,6 +950,24 @@ extern "C" int dlm_kernel_times(dlm_ctx* c, dlm_kernel_time* rows, int32_t cap, 
     (*n_rows)++;
   }
   if (reset) c->kprof.reset();
+  return DLM_OK;
+}
+
+extern "C" int dlm_step_trace(dlm_ctx* c, dlm_trace_row* rows, int32_t cap, int32_t* n_rows) {
+  if (!c || !rows || !n_rows) return DLM_E_ARG;
+  *n_rows = 0;
+  const size_t n = std::min(c->last_trace_cls.size(), c->trace_host.size() / 3);
+  unsigned long long t0 = ~0ULL;
+  for (size_t i = 0; i < n; ++i) t0 = std::min(t0, c->trace_host[3 * i]);
+  for (size_t i = 0; i < n && *n_rows < cap; ++i) {
+    const unsigned long long b = c->trace_host[3 * i], w = c->trace_host[3 * i + 1], e = ~c->trace_host[3 * i + 2];
+    if (b == ~0ULL) continue;                  // a record that no launch used
+    dlm_trace_row& r = rows[(*n_rows)++];
+    r.kernel = c->last_trace_cls[i]; r.slot = (int32_t)i;
+    r.begin_us = (float)((double)(b - t0) * 1e-3);
+    r.wait_us = w == ~0ULL ? r.begin_us : (float)((double)(w - t0) * 1e-3);
+    r.end_us = c->trace_host[3 * i + 2] == ~0ULL ? r.wait_us : (float)((double)(e - t0) * 1e-3);
+  }
   return DLM_OK;
 }
 
@@ -905,6 +984,8 @@ extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
     case DLM_OPT_PAIR_GEMM: c->opt_pair = value != 0; return DLM_OK;
     case DLM_OPT_TC_ATTENTION: c->opt_tcattn = value != 0; return DLM_OK;
     case DLM_OPT_FUSE_ROPE: c->opt_fuse_rope = value != 0; return DLM_OK;
+    case DLM_OPT_TRACE: c->opt_trace = value != 0; return DLM_OK;
+    case DLM_OPT_TCT_MIN_ITEMS: c->opt_tct_min_items = std::max(1, value); return DLM_OK;
   }
   set_err(&c->err, "unknown option %d", key);
   return DLM_E_ARG;
@@ -931,6 +1012,7 @@ static void recount(const dlm_arch& a, Req& q, const int* tok) {
 }
 
 extern "C" int dlm_request_add(dlm_ctx* c, const int32_t* prompt, int32_t P, int32_t G, int32_t B, float tau, int32_t* out_req) {
+  DevGuard dev_guard(c);
   if (!c) return DLM_E_ARG;
   const dlm_arch& a = c->a;
   if (!prompt || !out_req || P < 0 || G <= 0 || B <= 0 || B > a.max_block || G % B) {
@@ -955,15 +1037,22 @@ extern "C" int dlm_request_add(dlm_ctx* c, const int32_t* prompt, int32_t P, int
   std::vector<int> tok(S);
   for (int i = 0; i < P; ++i) tok[i] = prompt[i];
   for (int i = P; i < S; ++i) tok[i] = a.mask_id;
-  CU_TRY(&c->err, cudaMemcpyAsync(c->tokens + (size_t)slot * a.max_seq, tok.data(), (size_t)S * 4, cudaMemcpyHostToDevice, c->st));
-  CU_TRY(&c->err, cudaMemsetAsync(c->conf_state + (size_t)slot * a.max_seq, 0, (size_t)a.max_seq * 4, c->st));
-  CU_TRY(&c->err, cudaMemcpyAsync(c->page_table + (size_t)slot * c->kg.max_pages_per_req, row.data(), row.size() * 4, cudaMemcpyHostToDevice, c->st));
-  CU_TRY(&c->err, cudaStreamSynchronize(c->st));
+  cudaError_t e = cudaMemcpyAsync(c->tokens + (size_t)slot * a.max_seq, tok.data(), (size_t)S * 4, cudaMemcpyHostToDevice, c->st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->conf_state + (size_t)slot * a.max_seq, 0, (size_t)a.max_seq * 4, c->st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(c->page_table + (size_t)slot * c->kg.max_pages_per_req, row.data(), row.size() * 4, cudaMemcpyHostToDevice, c->st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+  if (e != cudaSuccess) {                      // nothing is partially applied: give the slot and its pages back
+    for (int pg : q.pages) c->free_pages.push_back(pg);
+    q = Req();
+    set_err(&c->err, "dlm_request_add: %s", cudaGetErrorString(e));
+    return DLM_E_CUDA;
+  }
   *out_req = slot;
   return DLM_OK;
 }
 
 extern "C" int dlm_request_set_tokens(dlm_ctx* c, int32_t r, const int32_t* tokens, int32_t n, int32_t keep_cache) {
+  DevGuard dev_guard(c);
   Req* q = get_req(c, r);
   if (!q || !tokens) { if (c) set_err(&c->err, "dlm_request_set_tokens: bad request %d", r); return DLM_E_ARG; }
   if (n != q->S) { set_err(&c->err, "dlm_request_set_tokens: n=%d != S=%d", n, q->S); return DLM_E_ARG; }
@@ -986,6 +1075,7 @@ extern "C" int dlm_request_remove(dlm_ctx* c, int32_t r) {
 }
 
 extern "C" int dlm_request_tokens(dlm_ctx* c, int32_t r, int32_t* out, int32_t cap) {
+  DevGuard dev_guard(c);
   Req* q = get_req(c, r);
   if (!q || !out) { if (c) set_err(&c->err, "dlm_request_tokens: bad request %d", r); return DLM_E_ARG; }
   if (cap < q->S) { set_err(&c->err, "dlm_request_tokens: cap=%d < S=%d", cap, q->S); return DLM_E_CAPACITY; }
@@ -1000,6 +1090,7 @@ constexpr int32_t kBlobMagic = 0x524D4C44, kBlobVersion = 1, kBlobHeaderWords = 
 }
 
 extern "C" int64_t dlm_request_export(dlm_ctx* c, int32_t r, void* blob, int64_t cap) {
+  DevGuard dev_guard(c);
   Req* q = get_req(c, r);
   if (!q) { if (c) set_err(&c->err, "dlm_request_export: bad request %d", r); return DLM_E_ARG; }
   const int64_t need = (int64_t)kBlobHeaderWords * 4 + (int64_t)q->S * 8;
@@ -1015,6 +1106,7 @@ extern "C" int64_t dlm_request_export(dlm_ctx* c, int32_t r, void* blob, int64_t
 }
 
 extern "C" int dlm_request_import(dlm_ctx* c, const void* blob, int64_t bytes, int32_t* out_req) {
+  DevGuard dev_guard(c);
   if (!c) return DLM_E_ARG;
   const int32_t* h = static_cast<const int32_t*>(blob);
   if (!blob || !out_req || bytes < (int64_t)kBlobHeaderWords * 4 || h[0] != kBlobMagic || h[1] != kBlobVersion) {
@@ -1156,12 +1248,14 @@ static int gemm_big(dlm_ctx* c, const void* A, long long a_rows_cap, const void*
   if (n_slices) *n_slices = 1;
   if (M > 128 && c->opt_pair) {
     GemmPairParams p = {};
-    p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0;
+    p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0; p.tr = c->tslot();
+    c->paths |= DLM_PATH_GEMM_PAIR;
     const int max_splits = (n_slices && slice_rows_cap > 0) ? (int)std::min<long long>(4, slice_rows_cap / M) : 1;
     return gemm_pair(c->tmaps, &c->err, A, a_rows_cap, W, w_rows, M, N, K, epi, 0, p, c->st, pdl, max_splits, n_slices);
   }
   GemmTcParams p = {};
-  p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0;
+  p.out_f32 = out_f32; p.out_bf16 = out_bf16; p.ldc = ldc; p.up_row0 = up_row0; p.tr = c->tslot();
+  c->paths |= DLM_PATH_GEMM_TC;
   return gemm_tc(c->tmaps, &c->err, A, a_rows_cap, W, w_rows, M, N, K, epi, 0, p, c->st, pdl);
 }
 
@@ -1195,6 +1289,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   const float scale = 1.f / sqrtf((float)a.head_dim);
   std::string* err = &c->err;
   if (!tc) {   // scratch of the plain path, allocated on first use
+    c->paths |= DLM_PATH_GEMM_PLAIN;
     if (!c->tmp) CU_TRY(err, cudaMalloc(&c->tmp, (size_t)c->Tmax * std::max(d, 2 * F) * 4));
     if (!c->logits) CU_TRY(err, cudaMalloc(&c->logits, (size_t)c->Rmax * V * 4));
   }
@@ -1204,13 +1299,13 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   auto flush_partials = [&]() {
     if (pend > 0 && c->opt_dump) {
       KScope ks(c, DLM_K_RMSNORM);
-      launch_k(add_partials_kernel, dim3((unsigned)((pstride + 255) / 256)), dim3(256), 0, st, pdl, c->x, (const float*)c->part_x, pend, pstride, pstride);
+      launch_k(add_partials_kernel, dim3((unsigned)((pstride + 255) / 256)), dim3(256), 0, st, pdl, c->x, (const float*)c->part_x, pend, pstride, pstride, c->tslot());
       pend = 0;
     }
   };
   if (T > 0) {
     KScope ks(c, DLM_K_EMBED);                    // first kernel of the step: plain launch (stream order vs. the previous step)
-    launch_k(embed_kernel<TE>, dim3(T), dim3(256), 0, st, false, c->x, (const TE*)c->E, (const int*)c->tokens, a.max_seq, bd, d);
+    launch_k(embed_kernel<TE>, dim3(T), dim3(256), 0, st, false, c->x, (const TE*)c->E, (const int*)c->tokens, a.max_seq, bd, d, c->tslot());
   }
   for (int l = 0; l < a.n_layers && T > 0; ++l) {
     const LayerW& w = c->L[l];
@@ -1226,13 +1321,16 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
       KScope ks(c, DLM_K_GEMM_QKV);
       if (skinny) {
         SkinnyParams p = {};
-        p.out_f32 = c->qkv; p.ldc = NQKV;
+        p.out_f32 = c->qkv; p.ldc = NQKV; p.tr = c->tslot();
+        c->paths |= DLM_PATH_GEMM_SKINNY;
         int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, SK_PARTIAL, 0, p, &nq, st, pdl);
         if (rc) return rc;
       } else if (fuse_rope) {
         GemmPairParams p = {};
         p.rope.q = (bf16*)c->q; p.rope.kv_store = (bf16*)c->kv_store; p.rope.rope_cos = c->rope_cos; p.rope.rope_sin = c->rope_sin;
         p.rope.page_table = c->page_table; p.rope.b = bd; p.rope.g = c->kg; p.rope.layer = l; p.rope.n_heads = a.n_heads;
+        p.tr = c->tslot();
+        c->paths |= DLM_PATH_GEMM_PAIR | DLM_PATH_ROPE_FUSED;
         int rc = gemm_pair(c->tmaps, err, c->u, c->Tmax, w.wqkv, NQKV, T, NQKV, d, EPI_ROPE, 0, p, st, pdl);
         if (rc) return rc;
       } else if (tc) {
@@ -1246,24 +1344,30 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
       KScope ks(c, DLM_K_ROPE_KV);
       const int hpb = std::max(1, 256 / (a.head_dim / 2));       // heads per block
       launch_k(rope_kv_write_kernel<TE>, dim3(T, (a.n_heads + 2 * a.n_kv_heads + hpb - 1) / hpb), dim3(hpb * (a.head_dim / 2)), 0, st, pdl, (TE*)c->q, (TE*)c->kv_store, (const float*)c->qkv, (const float*)c->rope_cos,
-               (const float*)c->rope_sin, (const int*)c->page_table, bd, c->kg, l, a.n_heads, nq, (long long)T * NQKV);
+               (const float*)c->rope_sin, (const int*)c->page_table, bd, c->kg, l, a.n_heads, nq, (long long)T * NQKV, c->tslot());
     }
     dump_stage(c, l, DLM_T_Q, c->q, (size_t)HQ * sizeof(TE), T);
     bool flash_done = false;
     if (tc && c->opt_flash && c->opt_tcattn) {
       KScope ks(c, DLM_K_ATTENTION);
+      const TraceSlot tr3[3] = {c->tslot(), c->tslot(), c->tslot()};
       int rc = attn_tc_launch(c->tmaps, (bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, a.n_layers, c->page_table, bd, c->kg, l,
-                              a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, st, pdl, err, &flash_done, 0);
+                              a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, st, pdl, err, &flash_done, 0, tr3, &c->paths, c->opt_tct_min_items);
       if (rc) return rc;
+      if (!flash_done && c->opt_trace) c->trace_cls.resize(c->trace_cls.size() - 3);      // nothing launched: give the records back
     }
     if (tc && c->opt_flash && !flash_done) {
       KScope ks(c, DLM_K_ATTENTION);
+      const TraceSlot t0 = c->tslot(), t1 = c->tslot();
       int rc = attn_flash_launch((bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, c->page_table, bd, c->kg, l,
-                                 a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, pdl, err, &flash_done);
+                                 a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, pdl, err, &flash_done, t0, t1);
       if (rc) return rc;
+      if (flash_done) c->paths |= DLM_PATH_ATTN_FLASH;
+      else if (c->opt_trace) c->trace_cls.resize(c->trace_cls.size() - 2);
     }
     if (!flash_done) {
       KScope ks(c, DLM_K_ATTENTION);
+      c->paths |= DLM_PATH_ATTN_PLAIN;
       launch_k(attention_plain_kernel<TE>, dim3(T, a.n_heads), dim3(128), (size_t)bd.max_kv_len * 4, st, pdl, (TE*)c->attn, (const TE*)c->q,
                (const TE*)c->kv_store, (const int*)c->page_table, bd, c->kg, l, a.n_heads, scale);
     }
@@ -1272,7 +1376,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
       KScope ks(c, DLM_K_GEMM_O);
       if (skinny) {
         SkinnyParams p = {};
-        p.out_f32 = c->part_x; p.ldc = d;
+        p.out_f32 = c->part_x; p.ldc = d; p.tr = c->tslot();
         int rc = gemm_skinny(c->tmaps, err, c->attn, c->Tmax, w.wo, d, T, d, HQ, SK_PARTIAL, 0, p, &pend, st, pdl);
         if (rc) return rc;
       } else if (tc) {
@@ -1295,7 +1399,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
       KScope ks(c, DLM_K_GEMM_GATEUP);
       if (skinny) {
         SkinnyParams p = {};
-        p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F;
+        p.out_bf16 = (bf16*)c->act; p.ldc = F; p.up_row0 = F; p.tr = c->tslot();
         int rc = gemm_skinny(c->tmaps, err, c->u, c->Tmax, w.wgu, 2LL * F, T, F, d, SK_SWIGLU, 0, p, nullptr, st, pdl);
         if (rc) return rc;
       } else if (tc) {
@@ -1311,7 +1415,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
       KScope ks(c, DLM_K_GEMM_DOWN);
       if (skinny) {
         SkinnyParams p = {};
-        p.out_f32 = c->part_x; p.ldc = d;
+        p.out_f32 = c->part_x; p.ldc = d; p.tr = c->tslot();
         int rc = gemm_skinny(c->tmaps, err, c->act, c->Tmax, w.wd, d, T, d, F, SK_PARTIAL, 0, p, &pend, st, pdl);
         if (rc) return rc;
       } else if (tc) {
@@ -1337,7 +1441,7 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   if (R > 0) {
     {
       KScope ks(c, DLM_K_RMSNORM);
-      launch_k(build_row_src_kernel, dim3(bd.n), dim3(64), 0, st, pdl, c->row_src, bd);
+      launch_k(build_row_src_kernel, dim3(bd.n), dim3(64), 0, st, pdl, c->row_src, bd, c->tslot());
       launch_rmsnorm<TE>(c, (TE*)c->hf, c->x, (const int*)c->row_src, R, d, a.rms_eps, (const float*)c->part_x, pend, pstride, pdl);
       pend = 0;
     }
@@ -1346,13 +1450,15 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     if (tc && R > 128 && c->opt_pair) {          // compute-bound head: CTA-pair kernel, 256-wide vocabulary tiles
       n_tiles = (V + 255) / 256;
       GemmPairParams p = {};
-      p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale;
+      p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale; p.tr = c->tslot();
+      c->paths |= DLM_PATH_GEMM_PAIR;
       int rc = gemm_pair(c->tmaps, err, c->hf, std::max(c->Rmax, 128), c->Wlm, V, R, V, d, EPI_LMHEAD, 256, p, st, pdl);
       if (rc) return rc;
     } else if (tc) {
       n_tiles = c->n_tiles;
       GemmTcParams p = {};
-      p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale;
+      p.part = c->part; p.n_tiles = n_tiles; p.mask_id = a.mask_id; p.scale = a.logit_scale; p.tr = c->tslot();
+      c->paths |= DLM_PATH_GEMM_TC;
       int rc = gemm_tc(c->tmaps, err, c->hf, std::max(c->Rmax, 128), c->Wlm, V, R, V, d, EPI_LMHEAD, 128, p, st, pdl);
       if (rc) return rc;
     } else {
@@ -1363,12 +1469,12 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   {
     KScope ks(c, DLM_K_COMBINE_UNMASK);
     launch_k(combine_unmask_kernel, dim3(bd.n), dim3(1024), 0, st, pdl, so, (const RowPartial*)c->part, n_tiles, c->tokens, a.max_seq, a.max_block, a.mask_id, bd,
-             dry_run ? 1 : 0);
+             dry_run ? 1 : 0, c->tslot());
     if (c->want_feat) {
       float* feats = (float*)(c->out_dev + (size_t)a.max_requests * 4 + (size_t)c->Rmax * 4 * 6);
       const int* gl = c->desc_dev + 9 * (size_t)bd.n;
       launch_k(conf_features_kernel, dim3(bd.n), dim3(1024), 0, st, pdl, feats, c->conf_state, (const int*)c->tokens, a.max_seq, a.max_block, a.mask_id, so, bd,
-               gl, gl + bd.n, dry_run ? 1 : 0);
+               gl, gl + bd.n, dry_run ? 1 : 0, c->tslot());
     }
   }
   CU_TRY(err, cudaGetLastError());
@@ -1380,6 +1486,9 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
 static int enqueue_step(dlm_ctx* c, const HostBatch& hb, bool dry, size_t desc_ints, bool capturing) {
   std::string* err = &c->err;
   CU_TRY(err, cudaMemcpyAsync(c->desc_dev, c->desc_host, desc_ints * 4, cudaMemcpyHostToDevice, c->st));
+  c->paths = 0;
+  c->trace_cls.clear();
+  if (c->opt_trace) CU_TRY(err, cudaMemsetAsync(c->trace_dev, 0xFF, (size_t)kMaxTraceSlots * 3 * 8, c->st));   // all three words are minima
   BatchDesc bd = make_desc(c, hb);
   if (capturing) CU_TRY(err, cudaEventRecordWithFlags(c->ev0, c->st, cudaEventRecordExternal));
   else CU_TRY(err, cudaEventRecord(c->ev0, c->st));        // device time of the step: first kernel .. last kernel
@@ -1393,6 +1502,7 @@ static int enqueue_step(dlm_ctx* c, const HostBatch& hb, bool dry, size_t desc_i
 
 static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, dlm_result* res, int kind) {
   if (!c) return DLM_E_ARG;
+  DevGuard dev_guard(c);
   if (!res || !res->n_committed || !res->pos || !res->tok || !res->conf) { set_err(&c->err, "step: result buffers missing"); return DLM_E_ARG; }
   HostBatch hb;
   int rc = build_batch(c, b, thr_override, kind, hb);
@@ -1400,6 +1510,12 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   const dlm_arch& a = c->a;
   const bool dry = (b->flags & DLM_DRY_RUN) != 0;
   if (res->capacity < hb.R) { set_err(&c->err, "step: result capacity %d < %d block rows", res->capacity, hb.R); return DLM_E_CAPACITY; }
+  if (res->features)
+    for (int i = 0; i < hb.n; ++i)
+      if (c->reqs[hb.slot[i]].G > kFeatMaxGen) {
+        set_err(&c->err, "step: the Step Predictor features support at most %d output positions per request (request %d has %d)", kFeatMaxGen, hb.slot[i], c->reqs[hb.slot[i]].G);
+        return DLM_E_CAPACITY;
+      }
   std::string* err = &c->err;
   const size_t desc_ints = fill_desc_host(c, hb);
   c->want_feat = res->features != nullptr;
@@ -1408,6 +1524,7 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   if (use_graph) {
     GraphKey key = std::make_tuple(kind, dry ? 1 : 0, hb.n, hb.T, hb.R, hb.max_q, hb.max_kv, c->opt_mask() | (c->want_feat ? 1 << 16 : 0) | (std::min(hb.min_q, 255) << 20), hb.n_big, hb.qt_big, hb.qt_total);
     GraphEntry& g = c->graphs[key];
+    g.used = ++c->graph_clock;
     if (g.seen == 1) {                         // second sighting of this batch shape: capture it
       const long long l0 = g_launches;
       cudaGraph_t graph = nullptr;
@@ -1416,6 +1533,7 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
         cudaError_t e = cudaStreamEndCapture(c->st, &graph);
         if (rc == DLM_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) == cudaSuccess) {
           g.launches = g_launches - l0;
+          g.paths = c->paths; g.trace_cls = c->trace_cls;
           g.seen = 2;
         } else {
           g.seen = 3;                            // capture not possible for this shape: stay on eager launches
@@ -1429,9 +1547,23 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
     if (g.seen == 2) {
       CU_TRY(err, cudaGraphLaunch(g.exec, c->st));
       g_launches += g.launches;
+      c->paths = g.paths | DLM_PATH_GRAPH_REPLAY; c->trace_cls = g.trace_cls;
       launched = true;
     } else if (g.seen == 0) {
       g.seen = 1;
+    }
+    // bounded cache: a serving loop with drifting ragged shapes must not grow host / device memory without limit.  The
+    // least recently used entry goes (its executable graph is destroyed; the shape is captured again if it comes back).
+    while (c->graphs.size() > kMaxGraphs) {
+      auto victim = c->graphs.end();
+      for (auto it = c->graphs.begin(); it != c->graphs.end(); ++it)
+        if (&it->second != &g && (victim == c->graphs.end() || it->second.used < victim->second.used)) victim = it;
+      if (victim == c->graphs.end()) break;
+      if (victim->second.exec) {
+        if (launched) cudaStreamSynchronize(c->st);          // never destroy a graph the stream may still be running
+        cudaGraphExecDestroy(victim->second.exec);
+      }
+      c->graphs.erase(victim);
     }
   }
   if (!launched) {
@@ -1442,6 +1574,14 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
   cudaEventElapsedTime(&c->last_usec, c->ev0, c->ev1);
   c->last_usec *= 1000.f;
   if (c->kprof.on) c->kprof.collect();
+  c->last_paths = c->paths;
+  c->last_trace_cls = c->trace_cls;
+  if (c->opt_trace && !c->last_trace_cls.empty()) {
+    c->trace_host.resize(c->last_trace_cls.size() * 3);
+    CU_TRY(err, cudaMemcpy(c->trace_host.data(), c->trace_dev, c->trace_host.size() * 8, cudaMemcpyDeviceToHost));
+  } else {
+    c->trace_host.clear();
+  }
   // ---- unpack, update host-side request state ----
   const char* ob = c->out_host;
   const int* n_comm = (const int*)ob; ob += (size_t)a.max_requests * 4;
@@ -1477,12 +1617,17 @@ static int run_step(dlm_ctx* c, const dlm_batch* b, const float* thr_override, d
       }
     }
     if (res->n_masked_left) res->n_masked_left[i] = q.n_masked;
-    if (res->features) {          // App. A order; the request's state AFTER this step (a dry run reports, like everything else, without mutating)
-      float* f = res->features + (size_t)i * DLM_N_FEATURES;
+    if (res->features) {          // App. A order; the request's state AFTER this step.  A dry run reports the state the step WOULD
+      float* f = res->features + (size_t)i * DLM_N_FEATURES;      // leave (progress from the reported commits) without mutating anything
       const int nb = q.G / q.B;
-      const bool fin = q.cur_block >= nb;
-      f[0] = hb.tau[i]; f[1] = (float)q.G; f[2] = (float)q.steps_done / q.G; f[3] = (float)(q.G - q.n_masked) / q.G;
-      f[4] = fin ? 1.f : (float)q.cur_block / nb; f[5] = fin ? 1.f : (float)(q.B - q.n_masked_block) / q.B;
+      int steps = q.steps_done, n_masked = q.n_masked, n_masked_block = q.n_masked_block, cur_block = q.cur_block;
+      if (dry && hb.blk_len[i]) {
+        steps++; n_masked -= k; n_masked_block -= k;
+        if (n_masked_block == 0) { cur_block++; n_masked_block = cur_block < nb ? q.B : 0; }
+      }
+      const bool fin = cur_block >= nb;
+      f[0] = hb.tau[i]; f[1] = (float)q.G; f[2] = (float)steps / q.G; f[3] = (float)(q.G - n_masked) / q.G;
+      f[4] = fin ? 1.f : (float)cur_block / nb; f[5] = fin ? 1.f : (float)(q.B - n_masked_block) / q.B;
       for (int j = 0; j < 5; ++j) f[6 + j] = feats[i * 5 + j];
     }
   }
@@ -1506,23 +1651,35 @@ static void to_f32_host(const void* src, float* dst, size_t n, bool is_bf16) {
 }
 
 extern "C" int64_t dlm_debug_tensor(dlm_ctx* c, int32_t r, int32_t layer, int32_t which, float* out, int64_t cap) {
+  DevGuard dev_guard(c);
   Req* q = get_req(c, r);
   if (!q || !out) { if (c) set_err(&c->err, "dlm_debug_tensor: bad request %d", r); return DLM_E_ARG; }
   const dlm_arch& a = c->a;
   const int HQ = a.n_heads * a.head_dim, HKV = a.n_kv_heads * a.head_dim;
-  if (which == DLM_T_KCACHE || which == DLM_T_VCACHE) {
+  if (which == DLM_T_KCACHE || which == DLM_T_VCACHE || which == DLM_T_K || which == DLM_T_V) {
+    // K (post-RoPE) / V as they sit in the request's pages: all S positions (DLM_T_*CACHE), or the rows the last step
+    // computed for this request (DLM_T_K / DLM_T_V: the step wrote exactly those slots)
     if (layer < 0 || layer >= a.n_layers) { set_err(&c->err, "dlm_debug_tensor: bad layer"); return DLM_E_ARG; }
-    const int64_t n = (int64_t)q->S * HKV;
+    int p0 = 0, rows = q->S;
+    if (which == DLM_T_K || which == DLM_T_V) {
+      int bi = -1;
+      for (int i = 0; i < c->last_batch.n; ++i) if (c->last_batch.slot[i] == r) bi = i;
+      if (bi < 0) { set_err(&c->err, "dlm_debug_tensor: request %d was not in the last step", r); return DLM_E_STATE; }
+      p0 = c->last_batch.q_pos0[bi]; rows = c->last_batch.q_len[bi];
+    }
+    const int64_t n = (int64_t)rows * HKV;
     if (cap < n) { set_err(&c->err, "dlm_debug_tensor: cap too small"); return DLM_E_CAPACITY; }
     std::vector<char> page((size_t)c->kg.page_elems() * c->esize);
-    const int PT = a.kv_page_tokens, kv = which == DLM_T_VCACHE;
-    for (int pi = 0; pi * PT < q->S; ++pi) {
+    const int PT = a.kv_page_tokens, kv = (which == DLM_T_VCACHE || which == DLM_T_V);
+    for (int pi = p0 / PT; pi * PT < p0 + rows; ++pi) {
       const char* src = (const char*)c->kv_store + (size_t)c->kg.offset(layer, q->pages[pi], 0, 0, 0) * c->esize;
       if (cudaMemcpy(page.data(), src, page.size(), cudaMemcpyDeviceToHost) != cudaSuccess) { set_err(&c->err, "dlm_debug_tensor: copy failed"); return DLM_E_CUDA; }
       for (int h = 0; h < a.n_kv_heads; ++h)
-        for (int t = 0; t < PT && pi * PT + t < q->S; ++t) {
+        for (int t = 0; t < PT; ++t) {
+          const int pos = pi * PT + t;
+          if (pos < p0 || pos >= p0 + rows) continue;
           size_t so = ((size_t)(kv * a.n_kv_heads + h) * PT + t) * a.head_dim;
-          to_f32_host(page.data() + so * c->esize, out + ((size_t)(pi * PT + t) * HKV + (size_t)h * a.head_dim), a.head_dim, c->bf16_model);
+          to_f32_host(page.data() + so * c->esize, out + ((size_t)(pos - p0) * HKV + (size_t)h * a.head_dim), a.head_dim, c->bf16_model);
         }
     }
     return n;
@@ -1556,11 +1713,27 @@ extern "C" int64_t dlm_debug_tensor(dlm_ctx* c, int32_t r, int32_t layer, int32_
 // ------------------------------------------------------------------------------------------------
 // a15  cost table (P:123 one-time latency profiling; P:599-618 LP[tp][tokens], tp = 1)
 // ------------------------------------------------------------------------------------------------
-extern "C" int dlm_profile_step_costs(dlm_ctx* c, dlm_cost_row* rows, int32_t cap, int32_t* n_rows) {
+// Median of `reps` timed dry-run steps after two untimed ones (the second sighting of a shape captures its CUDA graph).
+static int time_steps(dlm_ctx* c, const dlm_batch* b, dlm_result* res, int kind, int reps, float* usec) {
+  std::vector<float> t;
+  for (int it = 0; it < reps + 2; ++it) {
+    int rc = kind == DLM_KIND_REFRESH ? dlm_refresh_step(c, b, res) : dlm_cached_step(c, b, nullptr, res);
+    if (rc) return rc;
+    if (it >= 2) t.push_back(c->last_usec);
+  }
+  std::sort(t.begin(), t.end());
+  *usec = t.size() % 2 ? t[t.size() / 2] : 0.5f * (t[t.size() / 2 - 1] + t[t.size() / 2]);
+  return DLM_OK;
+}
+
+extern "C" int dlm_profile_step_costs_ex(dlm_ctx* c, int32_t block_len, int32_t repeats, dlm_cost_row* rows, int32_t cap, int32_t* n_rows) {
   if (!c || !rows || !n_rows) return DLM_E_ARG;
+  DevGuard dev_guard(c);
   const dlm_arch& a = c->a;
   *n_rows = 0;
-  const int B = std::min(32, a.max_block);
+  const int B = block_len;
+  if (B <= 0 || B > a.max_block) { set_err(&c->err, "dlm_profile_step_costs: block length %d outside [1, max_block=%d]", B, a.max_block); return DLM_E_ARG; }
+  const int reps = std::max(10, repeats);                       // median of >= 10 timed repeats
   static const int kv_lens[] = {512, 1024, 2048, 4608};
   static const int ns[] = {1, 2, 4, 8, 16, 32, 64};
   int free_slots = 0;
@@ -1569,41 +1742,67 @@ extern "C" int dlm_profile_step_costs(dlm_ctx* c, dlm_cost_row* rows, int32_t ca
   std::vector<float> conf(c->Rmax);
   dlm_result res = {};
   res.n_committed = n_comm.data(); res.pos = pos.data(); res.tok = tok.data(); res.conf = conf.data(); res.capacity = c->Rmax;
-  const int reps = 5;
+  std::vector<int32_t> ids;
+  auto drop = [&]() { for (int r : ids) dlm_request_remove(c, r); ids.clear(); };
+  auto add = [&](int n, int S) {                                 // n scratch requests of S positions, the last B of them one MASK block
+    std::vector<int32_t> prompt(S - B);
+    for (int i = 0; i < n; ++i) {
+      for (int j = 0; j < S - B; ++j) prompt[j] = (int32_t)(mix64(0x5eedULL + 977ULL * i + j) % (unsigned)(a.vocab - 1));
+      for (auto& t : prompt) if (t >= a.mask_id) t++;
+      int32_t id;
+      int rc = dlm_request_add(c, prompt.data(), S - B, B, B, 2.0f, &id);
+      if (rc) { drop(); return rc; }
+      ids.push_back(id);
+    }
+    return (int)DLM_OK;
+  };
+  auto fits = [&](long long n, long long S) {
+    return n <= free_slots && S <= a.max_seq && S > B && n * ((S + a.kv_page_tokens - 1) / a.kv_page_tokens) <= (long long)c->free_pages.size();
+  };
+  // ---- cache steps: n requests x per-request K/V length (the paper's LP is indexed by cacheBlockSize x numReqs, P:615-617;
+  // the K/V length is added because the cached step's attention reads all of it).  The caches are built by untimed refresh
+  // steps over as many requests as max_batch_tokens admits at a time.
   for (int kv : kv_lens) {
-    if (kv > a.max_seq) continue;
     for (int n : ns) {
-      if (n > free_slots || (long long)n * kv > c->Tmax) continue;
-      if ((long long)n * ((kv + a.kv_page_tokens - 1) / a.kv_page_tokens) > (long long)c->free_pages.size()) continue;
-      if (*n_rows + 2 > cap) return DLM_OK;
-      std::vector<int32_t> ids;
-      std::vector<int32_t> prompt(kv - B);
-      for (int i = 0; i < n; ++i) {
-        for (int j = 0; j < kv - B; ++j) prompt[j] = (int32_t)(mix64(0x5eedULL + 977ULL * i + j) % (unsigned)(a.vocab - 1));
-        for (auto& t : prompt) if (t >= a.mask_id) t++;
-        int32_t id;
-        int rc = dlm_request_add(c, prompt.data(), kv - B, B, B, 2.0f, &id);
-        if (rc) { for (int r : ids) dlm_request_remove(c, r); return rc; }
-        ids.push_back(id);
-      }
-      dlm_batch b = {n, ids.data(), nullptr, DLM_DRY_RUN};
-      float best_r = 1e30f, best_c = 1e30f;
-      int rc = DLM_OK;
-      for (int it = 0; it < reps + 1 && !rc; ++it) {
-        rc = dlm_refresh_step(c, &b, &res);
-        if (it) best_r = std::min(best_r, c->last_usec);
-      }
-      for (int it = 0; it < reps + 1 && !rc; ++it) {
-        rc = dlm_cached_step(c, &b, nullptr, &res);
-        if (it) best_c = std::min(best_c, c->last_usec);
-      }
-      for (int r : ids) dlm_request_remove(c, r);
+      if (!fits(n, kv) || (long long)n * B > c->Tmax || kv > c->Tmax) continue;
+      if (*n_rows + 1 > cap) return DLM_OK;
+      int rc = add(n, kv);
       if (rc) return rc;
-      rows[*n_rows] = {DLM_KIND_REFRESH, n, n * kv, kv, best_r}; (*n_rows)++;
-      rows[*n_rows] = {DLM_KIND_CACHED, n, n * B, kv, best_c}; (*n_rows)++;
+      const int per = std::max(1, c->Tmax / kv);
+      for (int i0 = 0; i0 < n && !rc; i0 += per) {
+        dlm_batch rb = {std::min(per, n - i0), ids.data() + i0, nullptr, DLM_DRY_RUN};
+        rc = dlm_refresh_step(c, &rb, &res);
+      }
+      float us = 0.f;
+      dlm_batch b = {n, ids.data(), nullptr, DLM_DRY_RUN};
+      if (!rc) rc = time_steps(c, &b, &res, DLM_KIND_CACHED, reps, &us);
+      drop();
+      if (rc) return rc;
+      rows[(*n_rows)++] = {DLM_KIND_CACHED, n, n * B, kv, us};
     }
   }
+  // ---- recompute steps: total tokens in powers of two (LP[tp][numTokens]), as ONE request up to max_seq, then as
+  // several requests of the largest power of two that fits
+  int s_big = 128;
+  while (2 * s_big <= a.max_seq) s_big *= 2;
+  for (long long t = 128; t <= 32768; t *= 2) {
+    const long long S = std::min<long long>(t, s_big), n = t / S;
+    if (t > c->Tmax || !fits(n, S)) continue;
+    if (*n_rows + 1 > cap) return DLM_OK;
+    int rc = add((int)n, (int)S);
+    if (rc) return rc;
+    float us = 0.f;
+    dlm_batch b = {(int)n, ids.data(), nullptr, DLM_DRY_RUN};
+    rc = time_steps(c, &b, &res, DLM_KIND_REFRESH, reps, &us);
+    drop();
+    if (rc) return rc;
+    rows[(*n_rows)++] = {DLM_KIND_REFRESH, (int)n, (int)t, (int)S, us};
+  }
   return DLM_OK;
+}
+
+extern "C" int dlm_profile_step_costs(dlm_ctx* c, dlm_cost_row* rows, int32_t cap, int32_t* n_rows) {
+  return dlm_profile_step_costs_ex(c, c ? std::min(32, c->a.max_block) : 32, 10, rows, cap, n_rows);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1618,8 +1817,12 @@ static int op_check_device() {
     set_err(&g_init_error, "no CUDA device: libdlm has no CPU fallback");
     return DLM_E_CUDA;
   }
-  static bool init = false;
-  if (!init) { cudaDeviceProp p; int d = 0; cudaGetDevice(&d); cudaGetDeviceProperties(&p, d); g_num_sms = p.multiProcessorCount; init = true; }
+  static int sms[kMaxDevices] = {};
+  int d = 0;
+  cudaGetDevice(&d);
+  if (d < 0 || d >= kMaxDevices) { set_err(&g_init_error, "device ordinal %d not supported", d); return DLM_E_CUDA; }
+  if (!sms[d]) { cudaDeviceProp p; cudaGetDeviceProperties(&p, d); sms[d] = p.multiProcessorCount; }
+  g_dev = d; g_num_sms = sms[d];
   return DLM_OK;
 }
 

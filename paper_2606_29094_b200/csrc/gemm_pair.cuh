@@ -56,6 +56,7 @@ struct GemmPairParams {
   float scale;
   unsigned long long w_policy, a_policy;
   RopeEpi rope;       // EPI_ROPE
+  TraceSlot tr;       // DLM_OPT_TRACE record of this launch (null: off)
 };
 
 constexpr int kPairThreads = 192;
@@ -181,6 +182,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
   const int total_units = total_tiles * p.splits;      // unit u: tile u % total_tiles, K split u / total_tiles
 
   ptx::pdl_launch_dependents();
+  if (threadIdx.x == 0) trace_begin(p.tr);
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&mapA);
     ptx::prefetch_tmap(&mapB);
@@ -232,10 +234,12 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
           load_w(base + st * stage_bytes, kb0 + st * kPairKbPerStage, cnt, w_row, ptx::mapa(full_bar(st), 0));
         }
         ptx::pdl_wait();
+        trace_wait(p.tr);
         for (int st = 0; st < pre; ++st)
           load_a(base + st * stage_bytes, kb0 + st * kPairKbPerStage, min(kPairKbPerStage, nkb - st * kPairKbPerStage), m0, ptx::mapa(full_bar(st), 0));
       } else {
         ptx::pdl_wait();
+        trace_wait(p.tr);
       }
       // ring position kept as running (stage, phase) counters: `it % stages` with a run-time divisor is a ~30-instruction
       // sequence with a MUFU in the middle, once per stage on the critical path of the pipeline
@@ -508,6 +512,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
   if ((EPI == EPI_F32 || EPI == EPI_RESID) && warp >= 2 && lane == 0) ptx::bulk_wait<0>();   // bulk stores / reductions have landed
   ptx::tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) trace_end(p.tr);
   ptx::cluster_sync();          // no CTA of the pair frees TMEM / leaves while its peer may still signal it
   if (warp == 1) ptx::tmem_dealloc_pair(tmem_base, 512);
 }

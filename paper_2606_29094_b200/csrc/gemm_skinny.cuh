@@ -38,6 +38,7 @@ struct SkinnyParams {
   long long ldc;
   unsigned long long w_policy;
   int w_box;              // 0: W row-major (2-D map); else tiled storage, rows per TMA box (ptx::tma_load_w_tiled)
+  TraceSlot tr;           // DLM_OPT_TRACE record of this launch (null: off)
 };
 
 constexpr int kSkThreads = 192;
@@ -69,6 +70,7 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
   const uint32_t tmem_cols = p.tpad <= 32 ? 32u : (p.tpad <= 64 ? 64u : 128u);
 
   ptx::pdl_launch_dependents();            // the next kernel may start its own weight prefetch
+  if (threadIdx.x == 0) trace_begin(p.tr);
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&mapW);
     ptx::prefetch_tmap(&mapX);
@@ -114,6 +116,7 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
       const int pre = min(stages, nkb);
       for (int kb = 0; kb < pre; ++kb) load_w(kb, kb);          // weights: independent of the upstream kernel
       ptx::pdl_wait();                                           // activations: written by the upstream kernel
+      trace_wait(p.tr);
       for (int kb = 0; kb < pre; ++kb) load_x(kb, kb);
       // ring position as running (stage, phase) counters (no run-time division per K block); pre == stages here
       for (int kb = pre, s = 0, ph = 1; kb < nkb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
@@ -189,6 +192,7 @@ gemm_skinny_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_consta
   }
   ptx::tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) trace_end(p.tr);
   if (warp == 1) ptx::tmem_dealloc(tmem_base, tmem_cols);
 }
 

@@ -34,6 +34,7 @@ struct GemmTcParams {
   int mask_id;
   float scale;
   unsigned long long w_policy;   // L2 cache hint for the weight stream
+  TraceSlot tr;                  // DLM_OPT_TRACE record of this launch (null: off)
 };
 
 constexpr int kGemmThreads = 192;
@@ -65,6 +66,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   while ((int)tmem_cols < BN) tmem_cols <<= 1;
 
   ptx::pdl_launch_dependents();
+  if (threadIdx.x == 0) trace_begin(p.tr);
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&mapA);
     ptx::prefetch_tmap(&mapB);
@@ -103,6 +105,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
       const int pre = min(stages, num_kb);
       for (int kb = 0; kb < pre; ++kb) load_w(kb, kb);
       ptx::pdl_wait();
+      trace_wait(p.tr);
       for (int kb = 0; kb < pre; ++kb) load_a(kb, kb);
       // ring position as running (stage, phase) counters (no run-time division per K block); pre == stages here
       for (int kb = pre, s = 0, ph = 1; kb < num_kb; ++kb, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1 : 0)) {
@@ -256,6 +259,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__
   }
   ptx::tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) trace_end(p.tr);
   if (warp == 1) ptx::tmem_dealloc(tmem_base, tmem_cols);
 }
 

@@ -68,9 +68,8 @@ __global__ void init_rope_kernel(float* __restrict__ cs, float* __restrict__ sn,
 // ------------------------------------------------------------------------------------------------
 template <typename TW>
 __global__ void embed_kernel(float* __restrict__ x, const TW* __restrict__ E, const int* __restrict__ tokens,
-                             int max_seq, BatchDesc b, int d) {
-  pdl_launch_dependents();
-  pdl_wait();
+                             int max_seq, BatchDesc b, int d, TraceSlot tr = TraceSlot{nullptr}) {
+  DLM_PROLOGUE(tr);
   int t = blockIdx.x;
   int bi = b.tok_bi[t];
   int pos = b.q_pos0[bi] + (t - b.q_off[bi]);
@@ -88,6 +87,7 @@ __global__ void embed_kernel(float* __restrict__ x, const TW* __restrict__ E, co
   } else {
     for (int i = threadIdx.x; i < d; i += blockDim.x) xr[i] = to_f32(e[i]);
   }
+  DLM_EPILOGUE(tr);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -115,10 +115,9 @@ constexpr int kNormMaxChunks = 4;     // d <= 4 * 4 * 1024
 template <typename TA>
 __global__ void __launch_bounds__(1024) rmsnorm_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
                                                       int d, float eps, const float* __restrict__ part, int n_part,
-                                                      long long part_stride) {
+                                                      long long part_stride, TraceSlot tr = TraceSlot{nullptr}) {
   __shared__ float red[33];
-  pdl_launch_dependents();
-  pdl_wait();
+  DLM_PROLOGUE(tr);
   const int r = blockIdx.x;
   const long long sr = row_src ? row_src[r] : r;
   float4* xr = reinterpret_cast<float4*>(x + sr * d);
@@ -162,6 +161,7 @@ __global__ void __launch_bounds__(1024) rmsnorm_kernel(TA* __restrict__ u, float
       }
     }
   }
+  DLM_EPILOGUE(tr);
 }
 
 // Throughput variant for large token counts (T >= 1024): one WARP per row, no block barrier, two passes (sum of
@@ -170,9 +170,8 @@ __global__ void __launch_bounds__(1024) rmsnorm_kernel(TA* __restrict__ u, float
 template <typename TA>
 __global__ void __launch_bounds__(512) rmsnorm_rows_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
                                                            int n_rows, int d, float eps, const float* __restrict__ part, int n_part,
-                                                           long long part_stride) {
-  pdl_launch_dependents();
-  pdl_wait();
+                                                           long long part_stride, TraceSlot tr = TraceSlot{nullptr}) {
+  DLM_PROLOGUE(tr);
   const int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (r >= n_rows) return;
   const int lane = threadIdx.x & 31;
@@ -209,6 +208,7 @@ __global__ void __launch_bounds__(512) rmsnorm_rows_kernel(TA* __restrict__ u, f
       *reinterpret_cast<float4*>(reinterpret_cast<float*>(ur) + 4 * i) = make_float4(a.x * rs, a.y * rs, a.z * rs, a.w * rs);
     }
   }
+  DLM_EPILOGUE(tr);
 }
 
 // Same result (same per-lane summation order), one pass: d <= 4096, the whole row lives in the warp's registers (32 float4 per
@@ -216,9 +216,8 @@ __global__ void __launch_bounds__(512) rmsnorm_rows_kernel(TA* __restrict__ u, f
 template <typename TA>
 __global__ void __launch_bounds__(128) rmsnorm_warp_kernel(TA* __restrict__ u, float* __restrict__ x, const int* __restrict__ row_src,
                                                            int n_rows, int d, float eps, const float* __restrict__ part, int n_part,
-                                                           long long part_stride) {
-  pdl_launch_dependents();
-  pdl_wait();
+                                                           long long part_stride, TraceSlot tr = TraceSlot{nullptr}) {
+  DLM_PROLOGUE(tr);
   const int r = blockIdx.x * 4 + (threadIdx.x >> 5);
   if (r >= n_rows) return;
   const int lane = threadIdx.x & 31;
@@ -270,17 +269,18 @@ __global__ void __launch_bounds__(128) rmsnorm_warp_kernel(TA* __restrict__ u, f
       *reinterpret_cast<float4*>(reinterpret_cast<float*>(ur) + 4 * i) = make_float4(a[k].x * rs, a[k].y * rs, a[k].z * rs, a[k].w * rs);
     }
   }
+  DLM_EPILOGUE(tr);
 }
 
 // x[row] += sum of split-K partials (debug-dump mode only: makes x complete right after the projection)
-__global__ void add_partials_kernel(float* __restrict__ x, const float* __restrict__ part, int n_part, long long part_stride, long long n) {
-  pdl_launch_dependents();
-  pdl_wait();
+__global__ void add_partials_kernel(float* __restrict__ x, const float* __restrict__ part, int n_part, long long part_stride, long long n, TraceSlot tr = TraceSlot{nullptr}) {
+  DLM_PROLOGUE(tr);
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float v = x[i];
   for (int s = 0; s < n_part; ++s) v += part[s * part_stride + i];
   x[i] = v;
+  DLM_EPILOGUE(tr);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -292,9 +292,8 @@ template <typename TA>
 __global__ void __launch_bounds__(256) rope_kv_write_kernel(TA* __restrict__ q, TA* __restrict__ kv_store, const float* __restrict__ qkv,
                                                            const float* __restrict__ rope_cos, const float* __restrict__ rope_sin,
                                                            const int* __restrict__ page_table, BatchDesc b, KvGeom g, int layer,
-                                                           int n_heads, int n_part, long long part_stride) {
-  pdl_launch_dependents();
-  pdl_wait();
+                                                           int n_heads, int n_part, long long part_stride, TraceSlot tr = TraceSlot{nullptr}) {
+  DLM_PROLOGUE(tr);
   const int t = blockIdx.x;
   const int dh = g.head_dim, half = dh >> 1;
   const int h = blockIdx.y * (blockDim.x / half) + threadIdx.x / half;       // 0..H-1 query, then K heads, then V heads
@@ -323,6 +322,7 @@ __global__ void __launch_bounds__(256) rope_kv_write_kernel(TA* __restrict__ q, 
   }
   dst[i] = from_f32<TA>(a);
   dst[i + half] = from_f32<TA>(c);
+  DLM_EPILOGUE(tr);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -444,12 +444,12 @@ __global__ void swiglu_kernel(TA* __restrict__ act, const float* __restrict__ gu
 }
 
 // row_src[r] for a10: index into [T, d] of each block row
-__global__ void build_row_src_kernel(int* __restrict__ row_src, BatchDesc b) {
-  pdl_launch_dependents();
-  pdl_wait();
+__global__ void build_row_src_kernel(int* __restrict__ row_src, BatchDesc b, TraceSlot tr = TraceSlot{nullptr}) {
+  DLM_PROLOGUE(tr);
   int bi = blockIdx.x;
   int base = b.q_off[bi] + (b.blk_lo[bi] - b.q_pos0[bi]);
   for (int j = threadIdx.x; j < b.blk_len[bi]; j += blockDim.x) row_src[b.row_off[bi] + j] = base + j;
+  DLM_EPILOGUE(tr);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -513,11 +513,10 @@ struct StepOut {              // device-side result arrays, fixed stride max_blo
 
 __global__ void __launch_bounds__(1024) combine_unmask_kernel(StepOut o, const RowPartial* __restrict__ part,
                                                              int n_tiles, int* __restrict__ tokens, int max_seq,
-                                                             int max_block, int mask_id, BatchDesc b, int dry_run) {
+                                                             int max_block, int mask_id, BatchDesc b, int dry_run, TraceSlot tr = TraceSlot{nullptr}) {
   __shared__ float s_conf[64];
   __shared__ int s_tok[64];
-  pdl_launch_dependents();
-  pdl_wait();
+  DLM_PROLOGUE(tr);
   int bi = blockIdx.x;
   int B = b.blk_len[bi];
   int w = threadIdx.x >> 5, l = threadIdx.x & 31;
@@ -582,6 +581,7 @@ __global__ void __launch_bounds__(1024) combine_unmask_kernel(StepOut o, const R
     count += __popc(bal);
   }
   if (l == 0) o.n_committed[bi] = count;
+  DLM_EPILOGUE(tr);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -595,11 +595,10 @@ constexpr int kFeatMaxGen = 2048;
 __global__ void __launch_bounds__(1024) conf_features_kernel(float* __restrict__ feats, float* __restrict__ conf_state,
                                                             const int* __restrict__ tokens, int max_seq, int max_block, int mask_id,
                                                             StepOut o, BatchDesc b, const int* __restrict__ gen_lo,
-                                                            const int* __restrict__ gen_len, int dry_run) {
+                                                            const int* __restrict__ gen_len, int dry_run, TraceSlot tr = TraceSlot{nullptr}) {
   __shared__ float s[kFeatMaxGen];
   __shared__ float red[33];
-  pdl_launch_dependents();
-  pdl_wait();
+  DLM_PROLOGUE(tr);
   const int bi = blockIdx.x, tid = threadIdx.x;
   const int P = gen_lo[bi], G = gen_len[bi], B = b.blk_len[bi], lo = b.blk_lo[bi];
   float* f = feats + bi * 5;
@@ -653,6 +652,7 @@ __global__ void __launch_bounds__(1024) conf_features_kernel(float* __restrict__
     };
     f[0] = s[0]; f[1] = quant(0.25f); f[2] = quant(0.5f); f[3] = total / (float)G; f[4] = quant(0.75f);
   }
+  DLM_EPILOGUE(tr);
 }
 
 }  // namespace dlm
