@@ -92,11 +92,12 @@ class Weights:
     """All tensors of one model, generated on demand and kept as float32 (exact values);
     `get` returns float64 copies so the forward pass runs in fp64."""
 
-    def __init__(self, arch, seed: int, cache_bytes: int = 24 << 30):
+    def __init__(self, arch, seed: int, cache_bytes: int = 24 << 30, keep_f64: bool = False):
         self.arch, self.seed = arch, int(seed)
         self._cache: dict = {}
         self._bytes = 0
         self._cap = cache_bytes
+        self._f64: dict | None = {} if keep_f64 else None      # memo of the float64 copies (many requests through one small model)
 
     def shape(self, tid: int):
         a = self.arch
@@ -118,7 +119,12 @@ class Weights:
         return w
 
     def get(self, tid: int) -> np.ndarray:
-        return self.f32(tid).astype(np.float64)
+        if self._f64 is None:
+            return self.f32(tid).astype(np.float64)
+        w = self._f64.get(tid)
+        if w is None:
+            w = self._f64[tid] = self.f32(tid).astype(np.float64)
+        return w
 
     def rows(self, tid: int, idx: np.ndarray) -> np.ndarray:
         """Selected rows (embedding gather) without materialising the whole tensor when uncached."""
