@@ -5,12 +5,21 @@ tokens/s on 1 B200, LLaDA-8B shape; % of roofline).
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3|C4|C5] [--impl ours|reference]
 
 A "step" is one denoising step of the workload's batch through the whole hot path (DESIGN.md rows a0-a14): refresh
-steps where a block starts, cached steps inside a block, exactly as the free-running trajectory demands.
+steps where a block starts, cached steps inside a block, exactly as the free-running trajectory demands.  After the
+warm-up the run advances (untimed) to the next block boundary, so the K timed steps start with the refresh step of a
+block and contain both step kinds in the workload's own proportion (`config.step_mix`).
 `value`  = steps / device time (CUDA events on the library's stream around each step's kernels, inputs resident).
 `e2e`    = steps / wall time of the same C-ABI calls with HOST buffers (request upload, per-step descriptor H2D,
            result D2H and the synchronize all inside the timed region).
-`roofline` = the tcgen05 GEMM kernel (the dominant kernel) inside cached steps, from per-launch CUDA events.
-`cpu_baseline` = the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample.
+`step_roofline` = per step kind, measured ms against the step's roofline (sum of rooflines / sum of times), plus the
+           block-cycle figure (1 refresh + B-1 cached steps).
+`roofline` = the dominant kernel class of the cached steps (the weight-streaming / CTA-pair tcgen05 GEMMs), timed INSIDE the
+           production launch (CUDA graph + programmatic dependent launch) by the library's in-kernel %globaltimer trace
+           (DLM_OPT_TRACE): a launch's time = wait(next launch) - wait(this launch), so the classes add up to the step.
+`kernels`  = the same attribution for every kernel class, with achieved HBM GB/s of attention (K/V bytes) and of the
+           combine + unmask pass (LM-head partials).
+`cpu_baseline` = the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample, for the same
+           mix of step kinds as the timed region.
 N > 1: one process per GPU (torchrun), independent replicas of the workload (requests are independent, P:426
 "16 TP-1 workers"), no data-path collective; time = max over ranks; scaling "weak".
 """
@@ -263,14 +272,26 @@ def mix_steps_per_s(spec, t_refresh, t_cached):
     return b / (t_refresh + (b - 1) * t_cached)
 
 
-def cpu_baseline(arch, seed, specs, layers=1, n_cached=2):
+def nominal_mix(spec, steps):
+    """Step kinds of `steps` steps that start at a block boundary in the paper's worst-case block shape: one recompute step
+    and B - 1 cache steps per block."""
+    n_refresh = (steps + spec.block_len - 1) // spec.block_len
+    return n_refresh, steps - n_refresh
+
+
+def cpu_baseline(arch, seed, specs, layers=1, n_cached=2, mix=None):
+    """The oracle on request 0, one layer + the LM head, extrapolated to the full depth; steps/s of the batch for the given
+    (refresh request-steps, cached request-steps) mix -- the oracle processes requests one after the other."""
     spec = specs[0]
     o = oracle_sample(arch, seed, spec, layers, n_cached)
     n = len(specs)
-    return {"value": mix_steps_per_s(spec, o["t_refresh"], o["t_cached"]) / n, "unit": "steps/s", "cores": blas_threads(), "kind": "oracle",
+    n_ref, n_cac = mix if mix is not None else (1, spec.block_len - 1)
+    batch_steps = (n_ref + n_cac) / n
+    value = batch_steps / (n_ref * o["t_refresh"] + n_cac * o["t_cached"])
+    return {"value": value, "unit": "steps/s", "cores": blas_threads(), "kind": "oracle",
             "sample": f"fp64 numpy oracle, request 0 of {n}, first {layers} of {arch.n_layers} layers + LM head: 1 refresh step and "
-                      f"{o['n_cached']} cached steps timed, layer time x{arch.n_layers // layers}, block cycle 1 refresh + {spec.block_len - 1} cached"
-                      + (f", divided by {n} requests processed serially" if n > 1 else ""),
+                      f"{o['n_cached']} cached steps timed, layer time x{arch.n_layers // layers}; mix of {n_ref} refresh + {n_cac} cached request-steps"
+                      + (f" = {batch_steps:g} steps of the {n}-request batch, requests processed serially" if n > 1 else ""),
             "t_refresh_s": round(o["t_refresh"], 3), "t_cached_s": round(o["t_cached"], 3), "weight_gen_s": round(o["t_gen"], 1)}
 
 
@@ -282,14 +303,15 @@ def run_reference(args):
     arch, seed, specs, desc = get_workload(args.workload)
     steps, warm = max(1, args.steps), max(0, args.warmup)
     vals = []
+    mix = nominal_mix(specs[0], steps) if len(specs) == 1 else None
     for i in range(warm + steps):
-        cb = cpu_baseline(arch, seed, specs, layers=1, n_cached=1)
+        cb = cpu_baseline(arch, seed, specs, layers=1, n_cached=1, mix=mix)
         if i >= warm:
             vals.append(cb)
     v = float(np.mean([c["value"] for c in vals]))
     out = {"impl": "reference", "metric": "denoise_steps_per_s", "value": v, "unit": "steps/s", "n_gpus": args.gpus, "steps": steps,
            "warmup": warm, "ms_per_step": 1e3 / v, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-           "data": "synthetic", "config": {"workload": f"{args.workload}: {desc}"},
+           "data": "synthetic", "config": {"workload": f"{args.workload}: {desc}", "step_mix": None if mix is None else {"refresh": mix[0], "cached": mix[1]}},
            "cpu_baseline": {"value": v, "unit": "steps/s", "cores": vals[-1]["cores"], "kind": "oracle", "sample": vals[-1]["sample"]},
            "e2e": {"value": v, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out), flush=True)
@@ -379,11 +401,33 @@ def job_value(world, steps, dev_us):
 
 
 # ---------------------------------------------------------------------------------------------------------
+def at_block_boundary(run):
+    """True when the step that is due opens a block for the workload's first request (its K/V cache is not valid)."""
+    st = run.eng.info(run.ids[0])
+    return st["n_masked"] == 0 or not st["cache_valid"]
+
+
+def timed_steps(run, K, clk_index):
+    """K steps, device time summed from the library's per-step CUDA events; returns the per-step records."""
+    recs = []
+    with ClockSampler(clk_index) as clk:
+        import torch
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(K):
+            us, cm, nr, nc, work = run.step()
+            recs.append({"us": us, "commits": cm, "n_refresh": nr, "n_cached": nc, "work": work,
+                         "kind": "mixed" if (nr and nc) else ("refresh" if nr else "cached")})
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+    return recs, wall, clk.summary()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=128)
-    ap.add_argument("--warmup", type=int, default=16)
+    ap.add_argument("--steps", type=int, default=64)
+    ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--workload", default="C2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -391,6 +435,8 @@ def main():
     ap.add_argument("--micro", default=None, choices=["lmhead"], help="isolated micro-benchmark instead of the step benchmark")
     ap.add_argument("--cost-table", action="store_true", help="print dlm_profile_step_costs for the workload's architecture")
     ap.add_argument("--two-call", action="store_true", help="mixed iterations as dlm_refresh_step + dlm_cached_step instead of one dlm_mixed_step")
+    ap.add_argument("--tau", type=float, default=None, help="override every request's confidence threshold")
+    ap.add_argument("--tau-sweep", action="store_true", help="add a sweep over the paper's candidate thresholds (P:123; BASELINE.json configs[4]: 0.5-0.95)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -411,64 +457,77 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import paper_2606_29094_b200 as pkg
     arch, seed, specs, desc = get_workload(args.workload)
+    if args.tau is not None:
+        for sp in specs:
+            sp.threshold = float(args.tau)
     peaks = load_peaks()
     K, W = max(1, args.steps), max(3, args.warmup)
 
     run = Runner(pkg, arch, seed, specs, mixed_launch=not args.two_call)
     for _ in range(W):
         run.step()
+    # advance (untimed) to a block boundary: the timed region then opens with a block's recompute step and holds both step
+    # kinds in the workload's own proportion.  Ragged batches (C3, C5) have a request at a boundary in almost every step.
+    aligned = 0
+    while len(specs) == 1 and not at_block_boundary(run) and aligned < 2 * specs[0].block_len:
+        run.step()
+        aligned += 1
     torch.cuda.synchronize()
     if dist:
         dist.barrier()
     run.h2d = run.d2h = 0
     launches0 = run.eng.launch_count()
-    dev_us, commits, per_kind = 0.0, 0, {"refresh": [], "cached": [], "mixed": []}
-    work_by_kind = {}
-    with ClockSampler(local) as clk:
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(K):
-            us, cm, nr, nc, work = run.step()
-            dev_us += us
-            commits += cm
-            kind = "mixed" if (nr and nc) else ("refresh" if nr else "cached")
-            per_kind[kind].append(us)
-            work_by_kind.setdefault(kind, work)
-        torch.cuda.synchronize()
-        wall = time.perf_counter() - t0
+    recs, wall, clocks = timed_steps(run, K, local)
     launches = run.eng.launch_count() - launches0
+    dev_us = sum(r["us"] for r in recs)
+    commits = sum(r["commits"] for r in recs)
     if dist:
         dev_us, wall, commits, launches = reduce_over_ranks(dist, "cuda", dev_us, wall, commits, launches)
     n_req = len(specs)
     value = job_value(world, K, dev_us)
+    mix = {"refresh_request_steps": sum(r["n_refresh"] for r in recs), "cached_request_steps": sum(r["n_cached"] for r in recs),
+           "refresh": sum(r["kind"] == "refresh" for r in recs), "cached": sum(r["kind"] == "cached" for r in recs),
+           "mixed": sum(r["kind"] == "mixed" for r in recs)}
     out = {"metric": "denoise_steps_per_s", "value": value, "unit": "steps/s", "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": dev_us / K * 1e-3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
            "data": "synthetic",
            "config": {"workload": f"{args.workload}: {desc}", "requests_per_gpu": n_req, "parallelism": f"replicas x{world}, no collective",
+                      "step_mix": mix, "untimed_alignment_steps": aligned, "tau": args.tau,
                       "l2": "every step streams all weights (15 GB >> 126 MB L2): inputs larger than L2, no flush",
                       "timing": "value: sum over steps of CUDA-event time around each step's kernels (library stream); e2e: wall clock of the same calls"},
            "committed_tokens_per_s": commits / (dev_us * 1e-6), "request_steps_per_s": value * n_req,
            "e2e": {"value": world * K / wall, "unit": "steps/s", "h2d_bytes_per_step": run.h2d // K, "d2h_bytes_per_step": run.d2h // K,
                    "committed_tokens_per_s": commits / wall},
-           "gpu_launches": int(launches), "clocks": clk.summary()}
-    # ---- per step kind: measured vs the step's roofline (north_star: >= 60 %) ----
+           "gpu_launches": int(launches), "clocks": clocks}
+    # ---- per step kind: measured vs the step's roofline (north_star: >= 60 %); work summed step by step ----
     steps_rf = {}
-    for kind, us in per_kind.items():
-        if not us:
+    for kind in ("refresh", "cached", "mixed"):
+        rs = [r for r in recs if r["kind"] == kind]
+        if not rs:
             continue
-        t_roof, bound = roofline_ms(work_by_kind[kind], peaks)
-        steps_rf[kind] = {"n": len(us), "ms": float(np.mean(us)) * 1e-3, "ms_min": float(np.min(us)) * 1e-3, "roofline_ms": t_roof, "bound": bound,
-                          "frac": t_roof / (float(np.mean(us)) * 1e-3), "gflop": work_by_kind[kind]["flops"] * 1e-9,
-                          "gbytes": work_by_kind[kind]["bytes"] * 1e-9}
+        roofs = [roofline_ms(r["work"], peaks) for r in rs]
+        t_meas, t_roof = sum(r["us"] for r in rs) * 1e-3, sum(x[0] for x in roofs)
+        bounds = sorted({x[1] for x in roofs})
+        steps_rf[kind] = {"n": len(rs), "ms": t_meas / len(rs), "ms_min": min(r["us"] for r in rs) * 1e-3, "roofline_ms": t_roof / len(rs),
+                          "bound": bounds[0] if len(bounds) == 1 else "mixed", "frac": t_roof / t_meas,
+                          "gflop": sum(r["work"]["flops"] for r in rs) / len(rs) * 1e-9, "gbytes": sum(r["work"]["bytes"] for r in rs) / len(rs) * 1e-9}
+    if "refresh" in steps_rf and "cached" in steps_rf and n_req == 1:
+        Bk = specs[0].block_len                    # the block cycle of P:582: one recompute step + B - 1 cache steps
+        t_cyc = steps_rf["refresh"]["ms"] + (Bk - 1) * steps_rf["cached"]["ms"]
+        r_cyc = steps_rf["refresh"]["roofline_ms"] + (Bk - 1) * steps_rf["cached"]["roofline_ms"]
+        steps_rf["block_cycle"] = {"steps": Bk, "ms": t_cyc / Bk, "steps_per_s": 1e3 * Bk / t_cyc, "roofline_ms": r_cyc / Bk, "frac": r_cyc / t_cyc}
     out["step_roofline"] = steps_rf
+    out["roofline_frac_all_steps"] = sum(roofline_ms(r["work"], peaks)[0] for r in recs) / (sum(r["us"] for r in recs) * 1e-3)
     out["peaks"] = peaks
 
-    # ---- dominant kernel: the tcgen05 GEMM inside cached steps, per-launch CUDA events ----
+    # ---- dominant kernel class, timed inside the production launch by the in-kernel trace ----
     if rank == 0 and not args.no_kernel_pass:
-        out["roofline"], out["kernels"] = kernel_pass(run, pkg, arch, peaks)
+        out["roofline"], out["kernels"] = trace_pass(run, pkg, arch, peaks)
+    if rank == 0 and args.tau_sweep:
+        out["tau_sweep"] = tau_sweep(pkg, arch, seed, specs, not args.two_call)
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         try:
-            out["cpu_baseline"] = cpu_baseline(arch, seed, specs)
+            out["cpu_baseline"] = cpu_baseline(arch, seed, specs, mix=(mix["refresh_request_steps"], mix["cached_request_steps"]))
         except Exception as e:      # the oracle must never take the GPU line down
             out["cpu_baseline"] = {"value": None, "unit": "steps/s", "cores": os.cpu_count(), "kind": "oracle", "sample": f"failed: {e!r}"}
     run.close()
@@ -479,57 +538,94 @@ def main():
         dist.destroy_process_group()
 
 
-def kernel_pass(run, pkg, arch, peaks, n_steps=24):
-    """Second pass with an event pair around every launch (DLM_OPT_KERNEL_TIMING): per-kernel-class time inside
-    cached steps.  The GEMM classes are one kernel (gemm_tc_kernel) with different epilogues; they stream the
-    weights, so their roofline is HBM for small batches and tensor for large ones."""
+def tau_sweep(pkg, arch, seed, specs, mixed_launch, taus=(0.5, 0.6, 0.7, 0.8, 0.9, 0.95), steps=12, warm=3):
+    """Throughput against the confidence threshold (the paper's knob: P:88-99, candidate set P:123): the same workload
+    with every request at threshold tau.  Lower thresholds commit more tokens per step, so requests finish in fewer steps."""
+    import copy
+    rows = []
+    for tau in taus:
+        sp = copy.deepcopy(specs)
+        for x in sp:
+            x.threshold = float(tau)
+        run = Runner(pkg, arch, seed, sp, mixed_launch=mixed_launch)
+        for _ in range(warm):
+            run.step()
+        us = cm = 0.0
+        for _ in range(steps):
+            u, c, _, _, _ = run.step()
+            us += u
+            cm += c
+        run.close()
+        rows.append({"tau": tau, "steps_per_s": steps / (us * 1e-6), "committed_tokens_per_s": cm / (us * 1e-6), "commits_per_step": cm / steps})
+    return rows
+
+
+def trace_pass(run, pkg, arch, peaks, n_steps=12):
+    """A few more steps of the same run with DLM_OPT_TRACE: every kernel stamps %globaltimer inside the production launch
+    (CUDA graph + programmatic dependent launch; overhead < 1 %).  A launch holds the step's critical path from the moment
+    its griddepcontrol.wait returns (the launch before it has completed) until the next launch's wait returns, so the
+    per-class times add up to the step's duration -- which event pairs around overlapping kernels cannot give.  Only steps
+    of the workload's dominant kind are kept (cached for one request, mixed / cached for batches)."""
     eng = run.eng
-    eng.set_option(pkg.OPT_KERNEL_TIMING, 1)
-    eng.kernel_times(reset=True)
-    n_cached, works, kt = 0, None, {}
+    eng.set_option(pkg.OPT_TRACE, 1)
+    kept, cls, work_sum, span = 0, {}, None, 0.0
     guard = 0
-    while n_cached < n_steps and guard < 8 * n_steps:
+    want = None
+    while kept < n_steps and guard < 8 * n_steps:
         guard += 1
         us, cm, nr, nc, work = run.step()
-        step_kt = eng.kernel_times(reset=True)
-        if nr:                                   # keep only pure cached steps in the accumulators
+        tr = eng.step_trace()
+        kind = "mixed" if (nr and nc) else ("refresh" if nr else "cached")
+        if len(run.specs) == 1 and kind != "cached":
             continue
-        n_cached += 1
-        works = work
-        for k, (n, t) in step_kt.items():
-            a = kt.get(k, (0, 0.0))
-            kt[k] = (a[0] + n, a[1] + t)
-    eng.set_option(pkg.OPT_KERNEL_TIMING, 0)
-    if not n_cached:
+        if want is None:
+            want = kind
+        if kind != want or not tr:
+            continue
+        kept += 1
+        for i, (k, b, w, e) in enumerate(tr):
+            nxt = tr[i + 1][2] if i + 1 < len(tr) else e
+            a = cls.setdefault(k, [0, 0.0])
+            a[0] += 1
+            a[1] += max(0.0, nxt - w)
+        span += tr[-1][3] - tr[0][2]
+        work_sum = work if work_sum is None else {k: work_sum[k] + v for k, v in work.items()}
+    eng.set_option(pkg.OPT_TRACE, 0)
+    if not kept:
         return None, None
-    tot = sum(us for _, us in kt.values())
-    kernels = {k: {"launches_per_step": n / n_cached, "us_per_step": us / n_cached, "share": us / tot} for k, (n, us) in kt.items()}
-    gemm = [k for k in kt if k.startswith("gemm_") or k == "lmhead"]
-    g_launch = sum(kt[k][0] for k in gemm)
-    g_us = sum(kt[k][1] for k in gemm)
+    tot = sum(t for _, t in cls.values())
+    kernels = {k: {"launches_per_step": n / kept, "us_per_step": t / kept, "share": t / tot} for k, (n, t) in cls.items()}
+    w = {k: v / kept for k, v in work_sum.items()}
+    # attention over cached K/V and the combine + unmask pass: achieved HBM rate against the measured peak (north_star (c), (e))
+    if "attention" in kernels:
+        kernels["attention"].update({"kv_read_gbytes": w["kv_read_bytes"] * 1e-9, "hbm_gbs": w["kv_read_bytes"] / (kernels["attention"]["us_per_step"] * 1e-6) * 1e-9,
+                                     "hbm_frac": w["kv_read_bytes"] / (kernels["attention"]["us_per_step"] * 1e-6) * 1e-9 / peaks["hbm_gbs"]})
+    if "combine_unmask" in kernels:
+        rows = sum(s.block_len for s in run.specs)
+        tile = 256 if rows > 128 else 128
+        part_bytes = rows * ((arch.vocab + tile - 1) // tile) * 16
+        kernels["combine_unmask"].update({"partials_bytes": part_bytes, "hbm_gbs": part_bytes / (kernels["combine_unmask"]["us_per_step"] * 1e-6) * 1e-9})
+    gemm = [k for k in kernels if k.startswith("gemm_") or k == "lmhead"]
+    g_launch = sum(kernels[k]["launches_per_step"] for k in gemm)
+    g_us = sum(kernels[k]["us_per_step"] for k in gemm)
     T = sum(s.block_len for s in run.specs)
-    w_bytes = works["weight_bytes"]
-    flops = works["flops_linear"]
-    t_b = w_bytes / (peaks["hbm_gbs"] * 1e9)
-    t_f = flops / (peaks["bf16_tflops_sustained"] * 1e12)
-    per_launch_s = g_us * 1e-6 / g_launch
+    t_b = w["weight_bytes"] / (peaks["hbm_gbs"] * 1e9)
+    t_f = w["flops_linear"] / (peaks["bf16_tflops_sustained"] * 1e12)
     if t_b >= t_f:
-        ach = w_bytes / (g_launch / n_cached) / per_launch_s * 1e-9
-        rf = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"]}
+        ach = w["weight_bytes"] / (g_us * 1e-6) * 1e-9
+        rf = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+              "algorithmic_bytes_per_launch": w["weight_bytes"] / g_launch}
     else:
-        ach = flops / (g_launch / n_cached) / per_launch_s * 1e-12
-        rf = {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"]}
-    # dram__bytes_read + dram__bytes_write per launch, from the committed ncu --set full capture of this workload
-    # (profiles/r01_ncu_kernels.md: 15.39 GB over the 129 GEMM launches of a C2 cached step); other workloads: not captured
-    traffic = 119.3e6 if (T == 32 and arch.n_layers == 32 and arch.d_model == 4096) else None
-    big = T > 128
-    rf.update({"traffic": traffic, "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_kernels.md)",
-               "algorithmic_bytes_per_launch": w_bytes / (g_launch / n_cached),
-               "kernel": ("gemm_pair_kernel (CTA-pair tcgen05 GEMM: QKV+RoPE, O, gate/up+SwiGLU, down, LM head)" if big else
-                          "gemm_skinny_kernel (QKV, O, gate/up+SwiGLU, down) + gemm_tc_kernel<LM head>: the weight-streaming GEMMs") + " inside cached steps",
-               "launches_per_step": g_launch / n_cached, "avg_launch_us": per_launch_s * 1e6, "share_of_step": g_us / tot,
-               "algorithmic": f"weights streamed once per step ({w_bytes * 1e-9:.2f} GB bf16) / GEMM launches; tokens per step T={T}",
-               "peak_source": peaks["source"], "steps_sampled": n_cached})
+        ach = w["flops_linear"] / (g_us * 1e-6) * 1e-12
+        rf = {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"],
+              "algorithmic_flops_per_launch": w["flops_linear"] / g_launch}
+    rf.update({"traffic": None, "traffic_note": "dram bytes are not measured by this run; the ncu --set full capture of the same command is under profiles/",
+               "kernel": ("gemm_pair_kernel (CTA-pair tcgen05 GEMM: QKV+RoPE, O, gate/up+SwiGLU, down, LM head)" if T > 128 else
+                          "gemm_skinny_kernel (QKV, O, gate/up+SwiGLU, down) + gemm_tc_kernel<LM head>: the weight-streaming GEMMs") + f" inside {want} steps",
+               "launches_per_step": g_launch, "avg_launch_us": g_us / g_launch, "share_of_step": g_us / (tot / kept),
+               "step_us_traced": tot / kept, "timing": "in-kernel %globaltimer stamps under CUDA-graph replay + PDL (DLM_OPT_TRACE); class times sum to the step",
+               "algorithmic": f"weights streamed once per step ({w['weight_bytes'] * 1e-9:.2f} GB bf16) over the GEMM launches; tokens per step T={T}",
+               "peak_source": peaks["source"], "steps_sampled": kept})
     return rf, kernels
 
 
