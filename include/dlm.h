@@ -196,7 +196,14 @@ DLM_API int  dlm_profile_step_costs_ex(dlm_ctx*, int32_t block_len, int32_t repe
                                       under CUDA-graph replay and programmatic dependent launch, costs ~3 atomics per CTA      */
 #define DLM_OPT_TCT_MIN_ITEMS 12   /* fewest (request, KV head, query tile) work items for which a step takes the tcgen05 attention
                                       kernels (default 1: always); below it the mma.sync kernel runs (debugging / A-B timing)  */
+#define DLM_OPT_LAYER_KERNEL  13   /* 1 (default): steps of <= 64 tokens whose requests each compute <= 64 stacked query rows (the
+                                      batch-1 cache step) run ALL layers in one persistent launch (layer_mega_kernel: weight
+                                      stream never stops, stream-K work split, in-kernel phase counter); 0: one kernel per stage */
+#define DLM_OPT_LAYER_KERNEL_PHASE_TS 14 /* 1: that kernel records a timestamp per phase in CTA 0 (tuning aid, dlm_layer_kernel_phases) */
 DLM_API int  dlm_set_option(dlm_ctx*, int32_t key, int32_t value);
+/* Phase end times of the last whole-stack launch taken with DLM_OPT_LAYER_KERNEL_PHASE_TS, microseconds since its first phase
+ * ended, 8 per layer (fold+norm, QKV, attention, O, fold+norm, gate/up, SwiGLU, down) + the final fold.  Returns the count. */
+DLM_API int  dlm_layer_kernel_phases(dlm_ctx*, float* usec, int32_t cap);
 
 /* Which kernel families the LAST step launched (bit set), so that a caller -- and the parity tests -- can see when a step
  * left the tcgen05 / TMA kernels: DLM_PATH_ATTN_PLAIN or DLM_PATH_GEMM_PLAIN on a bf16 model means the SIMT debugging
@@ -211,6 +218,7 @@ DLM_API int  dlm_set_option(dlm_ctx*, int32_t key, int32_t value);
 #define DLM_PATH_ATTN_PLAIN   0x080u   /* SIMT attention                                                 */
 #define DLM_PATH_ROPE_FUSED   0x100u   /* RoPE + K/V page write in the QKV GEMM's epilogue                */
 #define DLM_PATH_GRAPH_REPLAY 0x200u   /* the step was one CUDA-graph launch                             */
+#define DLM_PATH_LAYER_KERNEL 0x400u   /* all layers in one persistent launch (DLM_OPT_LAYER_KERNEL)     */
 DLM_API uint32_t dlm_last_step_kernels(dlm_ctx*);
 
 /* Timeline of the LAST step taken with DLM_OPT_TRACE = 1, one row per kernel launch in launch order: microseconds since the
@@ -234,7 +242,8 @@ DLM_API int  dlm_step_trace(dlm_ctx*, dlm_trace_row* rows, int32_t cap, int32_t*
 #define DLM_K_GEMM_DOWN      7   /* a9 */
 #define DLM_K_LMHEAD         8   /* a11 */
 #define DLM_K_COMBINE_UNMASK 9   /* a12 + a13 */
-#define DLM_K_COUNT          10
+#define DLM_K_LAYERS         10  /* a2 .. a9 of every layer in one persistent launch (cached steps of <= 64 tokens) */
+#define DLM_K_COUNT          11
 typedef struct { int32_t kernel, launches; float usec; } dlm_kernel_time;
 DLM_API int  dlm_kernel_times(dlm_ctx*, dlm_kernel_time* rows, int32_t cap, int32_t* n_rows, int32_t reset);
 

@@ -19,11 +19,11 @@ LIB_PATH = os.path.join(_HERE, "libdlm.so")
 DLM_OK, DLM_E_ARG, DLM_E_CAPACITY, DLM_E_STATE, DLM_E_CUDA = 0, -1, -2, -3, -4
 DLM_DRY_RUN = 1
 OPT_SIMPLE_KERNELS, OPT_DEBUG_DUMP, OPT_CUDA_GRAPH, OPT_FLASH_ATTENTION, OPT_KERNEL_TIMING, OPT_PDL, OPT_SKINNY_GEMM, OPT_PAIR_GEMM, OPT_TC_ATTENTION, OPT_FUSE_ROPE = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
-OPT_TRACE, OPT_TCT_MIN_ITEMS = 11, 12
+OPT_TRACE, OPT_TCT_MIN_ITEMS, OPT_LAYER_KERNEL, OPT_LAYER_KERNEL_PHASE_TS = 11, 12, 13, 14
 DTYPE_F32, DTYPE_BF16, DTYPE_BF16_PRECISE = 0, 1, 2
-PATH_GEMM_SKINNY, PATH_GEMM_PAIR, PATH_GEMM_TC, PATH_GEMM_PLAIN, PATH_ATTN_TC, PATH_ATTN_TCT, PATH_ATTN_FLASH, PATH_ATTN_PLAIN, PATH_ROPE_FUSED, PATH_GRAPH_REPLAY = (1 << i for i in range(10))
+PATH_GEMM_SKINNY, PATH_GEMM_PAIR, PATH_GEMM_TC, PATH_GEMM_PLAIN, PATH_ATTN_TC, PATH_ATTN_TCT, PATH_ATTN_FLASH, PATH_ATTN_PLAIN, PATH_ROPE_FUSED, PATH_GRAPH_REPLAY, PATH_LAYER_KERNEL = (1 << i for i in range(11))
 KERNEL_NAMES = ("embed", "rmsnorm", "gemm_qkv", "rope_kv", "attention", "gemm_o", "gemm_gateup", "gemm_down", "lmhead",
-                "combine_unmask")
+                "combine_unmask", "layers")
 KIND_REFRESH, KIND_CACHED, KIND_MIXED = 0, 1, 2
 N_FEATURES = 11
 FEATURE_NAMES = ("confidence_threshold", "output_length", "full_progress", "full_unmask_progress", "block_progress", "block_unmask_progress",
@@ -110,6 +110,7 @@ def lib() -> C.CDLL:
         L.dlm_last_step_kernels.argtypes = [vp]
         L.dlm_last_step_kernels.restype = C.c_uint32
         L.dlm_step_trace.argtypes = [vp, C.POINTER(_TraceRow), i32, C.POINTER(i32)]
+        L.dlm_layer_kernel_phases.argtypes = [vp, C.POINTER(f32), i32]
         L.dlm_set_option.argtypes = [vp, i32, i32]
         L.dlm_kernel_times.argtypes = [vp, C.POINTER(_KernelTime), i32, C.POINTER(i32), i32]
         L.dlm_debug_tensor.argtypes = [vp, i32, i32, i32, C.POINTER(f32), i64]
@@ -333,6 +334,12 @@ class Engine:
         n = C.c_int32(0)
         self._check(lib().dlm_kernel_times(self._h, rows, 32, C.byref(n), 1 if reset else 0))
         return {KERNEL_NAMES[rows[i].kernel]: (rows[i].launches, rows[i].usec) for i in range(n.value)}
+
+    def layer_kernel_phases(self) -> np.ndarray:
+        """Phase end times (us) of the last whole-stack launch taken with OPT_LAYER_KERNEL_PHASE_TS."""
+        buf = np.zeros(8 * self.arch.n_layers + 1, np.float32)
+        n = self._check(lib().dlm_layer_kernel_phases(self._h, _fp(buf), len(buf)))
+        return buf[:n].copy()
 
     def last_step_kernels(self) -> int:
         """PATH_* bit set of the kernel families the last step launched."""

@@ -24,6 +24,7 @@
 #include "gemm_pair.cuh"
 #include "gemm_tc.cuh"
 #include "kernels_basic.cuh"
+#include "layer_mega.cuh"
 
 namespace dlm {
 thread_local long long g_launches = 0;
@@ -657,8 +658,14 @@ struct dlm_ctx {
   // options
   int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1, opt_tcattn = 1, opt_fuse_rope = 1;
   int opt_trace = 0;
+  int opt_mega = 0;            // whole-stack persistent kernel for cached steps of <= 64 tokens (off until it beats the per-stage kernels)
+  CUtensorMap* mega_wmaps = nullptr;   // device array [n_layers][4] of the tiled weight maps
+  unsigned int* mega_bar = nullptr;    // its phase counter
+  unsigned long long* mega_ts = nullptr, *mega_ts_host = nullptr;   // optional phase timestamps (DLM_OPT_MEGA_PHASE_TS)
+  int opt_mega_ts = 0;
+  void* u2 = nullptr;          // second RMSNorm output buffer (gate/up input) of the whole-stack kernel
   int opt_tct_min_items = 64;  // fewest (request, KV head, query tile) items for which a step takes the tcgen05 attention kernels
-  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4) | (opt_tcattn << 5) | (opt_fuse_rope << 6) | (opt_trace << 7); }
+  int opt_mask() const { return opt_simple | (opt_flash << 1) | (opt_pdl << 2) | (opt_skinny << 3) | (opt_pair << 4) | (opt_tcattn << 5) | (opt_fuse_rope << 6) | (opt_trace << 7) | (opt_mega << 8) | (opt_mega_ts << 9); }
   std::map<GraphKey, GraphEntry> graphs;
   unsigned long long graph_clock = 0;
   unsigned paths = 0, last_paths = 0;   // DLM_PATH_* of the step being enqueued / of the last step
@@ -903,6 +910,24 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   ALLOC(c->out_dev, c->out_bytes);
   if (cudaMallocHost(&c->out_host, c->out_bytes) != cudaSuccess) FAIL(DLM_E_CUDA, "cudaMallocHost failed");
   ALLOC(c->trace_dev, (size_t)kMaxTraceSlots * 3 * 8);
+  if (c->bf16_model) {            // whole-stack kernel: second norm buffer, phase counter, the tiled weight maps of every layer
+    ALLOC(c->u2, (size_t)kMgMaxTpad * d * es);
+    ALLOC(c->mega_bar, 256);
+    ALLOC(c->mega_ts, (size_t)(kMgPhasesPerLayer * a.n_layers + 2) * 8);
+    ALLOC(c->mega_wmaps, (size_t)a.n_layers * 4 * sizeof(CUtensorMap));
+    std::vector<CUtensorMap> hm((size_t)a.n_layers * 4);
+    bool ok = true;
+    for (int l = 0; l < a.n_layers && ok; ++l) {
+      const void* w4[4] = {c->L[l].wqkv, c->L[l].wo, c->L[l].wgu, c->L[l].wd};
+      for (int gi = 0; gi < 4 && ok; ++gi) {
+        const TmapCache::Twin* tw = c->tmaps.twin(w4[gi]);
+        ok = tw && make_tmap_w_tiled(&hm[(size_t)l * 4 + gi], tw->ptr, tw->rows_pad, tw->k_pad, gi == 2 ? 64 : 128);
+      }
+    }
+    if (!ok) FAIL(DLM_E_CUDA, "cuTensorMapEncodeTiled failed (tiled weight maps)");
+    if (cudaMemcpyAsync(c->mega_wmaps, hm.data(), hm.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, c->st) != cudaSuccess || cudaStreamSynchronize(c->st) != cudaSuccess)
+      FAIL(DLM_E_CUDA, "tensor map upload failed");
+  }
   cudaEventCreate(&c->ev0);
   cudaEventCreate(&c->ev1);
   cudaError_t e = cudaStreamSynchronize(c->st);
@@ -971,6 +996,16 @@ extern "C" int dlm_step_trace(dlm_ctx* c, dlm_trace_row* rows, int32_t cap, int3
   return DLM_OK;
 }
 
+extern "C" int dlm_layer_kernel_phases(dlm_ctx* c, float* usec, int32_t cap) {
+  if (!c || !usec || !c->mega_ts) return DLM_E_ARG;
+  DevGuard dev_guard(c);
+  const int n = std::min<int>(cap, kMgPhasesPerLayer * c->a.n_layers + 1);
+  std::vector<unsigned long long> h(n);
+  if (cudaMemcpy(h.data(), c->mega_ts, (size_t)n * 8, cudaMemcpyDeviceToHost) != cudaSuccess) return DLM_E_CUDA;
+  for (int i = 0; i < n; ++i) usec[i] = (float)((double)(h[i] - h[0]) * 1e-3);
+  return n;
+}
+
 extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
   if (!c) return DLM_E_ARG;
   switch (key) {
@@ -985,6 +1020,8 @@ extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
     case DLM_OPT_TC_ATTENTION: c->opt_tcattn = value != 0; return DLM_OK;
     case DLM_OPT_FUSE_ROPE: c->opt_fuse_rope = value != 0; return DLM_OK;
     case DLM_OPT_TRACE: c->opt_trace = value != 0; return DLM_OK;
+    case DLM_OPT_LAYER_KERNEL: c->opt_mega = value != 0; return DLM_OK;
+    case DLM_OPT_LAYER_KERNEL_PHASE_TS: c->opt_mega_ts = value != 0; return DLM_OK;
     case DLM_OPT_TCT_MIN_ITEMS: c->opt_tct_min_items = std::max(1, value); return DLM_OK;
   }
   set_err(&c->err, "unknown option %d", key);
@@ -1276,6 +1313,59 @@ static int gemm_big_resid(dlm_ctx* c, const void* A, const void* W, int M, int N
   return gemm_big(c, A, c->Tmax, W, N, M, N, K, EPI_RESID, c->x, nullptr, N, 0, pdl);
 }
 
+// Whole-stack persistent kernel (layer_mega.cuh): can this step take it?
+static bool mega_ok(const dlm_ctx* c, const BatchDesc& bd) {
+  const dlm_arch& a = c->a;
+  if (!c->bf16_model || c->opt_simple || !c->opt_mega || !c->opt_skinny || !c->w_tiled || !c->mega_wmaps) return false;
+  if (bd.T <= 0 || bd.T > kMgMaxTpad || a.head_dim != 128 || a.kv_page_tokens != 64) return false;
+  const int r = a.n_heads / a.n_kv_heads, NQKV = nqkv(a);
+  if (bd.max_q_len * r > 64) return false;                                   // one attention unit = <= 64 stacked rows
+  if (a.d_model % 128 || a.d_model > 4096 || (a.n_heads * a.head_dim) % 64 || NQKV % 128 || a.d_ffn % 64) return false;
+  if (NQKV / 128 > kMgMaxTiles || a.d_ffn / 64 > kMgMaxTiles || a.d_model / 128 > kMgMaxTiles) return false;
+  return true;
+}
+
+static int mega_launch(dlm_ctx* c, const BatchDesc& bd, int layer0, int n_layers, bool dump, bool pdl) {
+  const dlm_arch& a = c->a;
+  const int d = a.d_model, F = a.d_ffn, HQ = a.n_heads * a.head_dim, NQKV = nqkv(a);
+  MegaParams p = {};
+  p.layer0 = layer0; p.n_layers = n_layers; p.T = bd.T; p.tpad = (bd.T + 31) / 32 * 32;
+  p.stages = mega_stages(p.tpad);
+  p.d = d; p.HQ = HQ; p.NQKV = NQKV; p.F = F; p.Fp = (int)pad_to(F, 128); p.n_heads = a.n_heads;
+  p.eps = a.rms_eps; p.scale_log2 = (1.f / sqrtf((float)a.head_dim)) * 1.4426950408889634f;
+  p.wmaps = c->mega_wmaps;
+  p.x = c->x; p.u = (bf16*)c->u; p.u2 = (bf16*)c->u2; p.attn = (bf16*)c->attn; p.act = (bf16*)c->act;
+  p.q_dump = dump ? (bf16*)c->q : nullptr; p.xmid_dump = dump ? c->tmp : nullptr;
+  p.part_a = c->qkv; p.part_x = c->part_x;
+  p.rope_cos = c->rope_cos; p.rope_sin = c->rope_sin; p.kv_store = (bf16*)c->kv_store; p.page_table = c->page_table;
+  p.b = bd; p.g = c->kg; p.bar = c->mega_bar;
+  p.phase_ts = c->opt_mega_ts ? c->mega_ts : nullptr;
+  p.tr = c->tslot();
+  if (p.stages < 2 || p.stages * (p.tpad * 128) + kMgScratchOwn < kMgAttnBytes) { set_err(&c->err, "layer kernel: shared-memory plan does not fit (tpad %d)", p.tpad); return DLM_E_ARG; }
+  // slice capacity: a tile is cut into at most ceil(kbt * G / U) + 1 runs
+  const int G = g_num_sms;
+  auto max_seg = [&](long long n_tiles, long long kbt) { const long long U = n_tiles * kbt; return (int)((kbt * G + U - 1) / U) + 1; };
+  const long long need_a = std::max<long long>((long long)max_seg(NQKV / 128, d / 64) * bd.T * NQKV, (long long)max_seg(F / 64, d / 64) * bd.T * 2 * F);
+  const long long need_x = (long long)std::max(max_seg(d / 128, HQ / 64), max_seg(d / 128, F / 64)) * bd.T * d;
+  if (need_a > c->qkv_rows * (long long)NQKV || need_x > c->part_rows * (long long)d) { set_err(&c->err, "layer kernel: slice buffers too small"); return DLM_E_CAPACITY; }
+  const CUtensorMap* mu = c->tmaps.get(c->u, c->Tmax, d, p.tpad);
+  const CUtensorMap* mu2 = c->tmaps.get(c->u2, kMgMaxTpad, d, p.tpad);
+  const CUtensorMap* mat = c->tmaps.get(c->attn, c->Tmax, HQ, p.tpad);
+  const CUtensorMap* mac = c->tmaps.get(c->act, c->Tmax, F, p.tpad);
+  if (!mu || !mu2 || !mat || !mac) { set_err(&c->err, "cuTensorMapEncodeTiled failed (layer kernel activations)"); return DLM_E_CUDA; }
+  static bool configured[kMaxDevices] = {};
+  if (!configured[g_dev]) {
+    cudaError_t e = cudaFuncSetAttribute(layer_mega_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) { set_err(&c->err, "layer kernel: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+    configured[g_dev] = true;
+  }
+  CU_TRY(&c->err, cudaMemsetAsync(c->mega_bar, 0, 256, c->st));
+  cudaError_t e = launch_k(layer_mega_kernel, dim3(G), dim3(kMgThreads), (size_t)mega_smem_bytes(p.tpad, p.stages), c->st, pdl, *mu, *mu2, *mat, *mac, p);
+  if (e != cudaSuccess) { set_err(&c->err, "layer kernel launch: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+  c->paths |= DLM_PATH_LAYER_KERNEL;
+  return DLM_OK;
+}
+
 template <typename TE>
 static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
   const dlm_arch& a = c->a;
@@ -1307,7 +1397,31 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     KScope ks(c, DLM_K_EMBED);                    // first kernel of the step: plain launch (stream order vs. the previous step)
     launch_k(embed_kernel<TE>, dim3(T), dim3(256), 0, st, false, c->x, (const TE*)c->E, (const int*)c->tokens, a.max_seq, bd, d, c->tslot());
   }
-  for (int l = 0; l < a.n_layers && T > 0; ++l) {
+  const bool mega = tc && T > 0 && mega_ok(c, bd);
+  if (mega) {
+    // every layer in ONE persistent launch; in debug-dump mode the same kernel runs layer by layer (identical arithmetic) so
+    // that each layer's stage tensors can be copied out
+    KScope ks(c, DLM_K_LAYERS);
+    if (!c->opt_dump) {
+      int rc = mega_launch(c, bd, 0, a.n_layers, false, false);      // plain launch: its memset must not overtake the embedding kernel
+      if (rc) return rc;
+    } else {
+      if (!c->tmp) CU_TRY(err, cudaMalloc(&c->tmp, (size_t)c->Tmax * std::max(d, 2 * F) * 4));
+      for (int l = 0; l < a.n_layers; ++l) {
+        dump_stage(c, l, DLM_T_X_IN, c->x, (size_t)d * 4, T);
+        int rc = mega_launch(c, bd, l, 1, true, false);
+        if (rc) return rc;
+        dump_stage(c, l, DLM_T_NORM1, c->u, (size_t)d * sizeof(TE), T);
+        dump_stage(c, l, DLM_T_Q, c->q, (size_t)HQ * sizeof(TE), T);
+        dump_stage(c, l, DLM_T_ATTN, c->attn, (size_t)HQ * sizeof(TE), T);
+        dump_stage(c, l, DLM_T_X_MID, c->tmp, (size_t)d * 4, T);
+        dump_stage(c, l, DLM_T_NORM2, c->u2, (size_t)d * sizeof(TE), T);
+        dump_stage(c, l, DLM_T_ACT, c->act, (size_t)F * sizeof(TE), T);
+        dump_stage(c, l, DLM_T_X_OUT, c->x, (size_t)d * 4, T);
+      }
+    }
+  }
+  for (int l = 0; l < a.n_layers && T > 0 && !mega; ++l) {
     const LayerW& w = c->L[l];
     dump_stage(c, l, DLM_T_X_IN, c->x, (size_t)d * 4, T);
     {

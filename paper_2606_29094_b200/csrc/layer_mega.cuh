@@ -1,0 +1,585 @@
+// Persistent whole-stack kernel for small cached steps (T <= 64 tokens, the batch-1 "cache step" of P:347 that the
+// headline workload spends 31 of every 32 steps in): ALL layers of the step in ONE launch, one CTA per SM.
+//
+// Why.  With 32 tokens a layer is pure weight streaming (436 MB per layer at the LLaDA shape = 66.7 us at the measured
+// HBM rate) and the in-kernel timeline of the multi-kernel path (DLM_OPT_TRACE) shows its GEMMs already AT that rate --
+// the whole distance to the roofline (3.19 ms vs 2.34 ms per step) is the ~25 us per layer during which the small
+// kernels between the GEMMs (RMSNorm x 2, RoPE + K/V write, attention, split merge) hold the stream while HBM idles:
+// a kernel boundary costs ~3.5 us of dependency latency and only the next GEMM's shared-memory ring can be prefetched
+// under it.  Here the weight stream never stops:
+//
+//   warp 0        W producer: walks the step's whole sequence of (layer, projection, tile, K block) work of THIS SM and
+//                 issues the TMA loads of the weight tiles into a ring of `stages` x 16 KB as slots free up.  It depends on
+//                 nothing but ring space, so it runs ahead across every phase boundary: while the SM waits for a grid-wide
+//                 dependency, does attention or a norm, the ring fills with the NEXT projection's weights.
+//   warp 1        X producer: TMA loads of the activation tiles (tpad rows x 64) of the same sequence; before the first load
+//                 of a projection it waits for the grid-wide phase counter (the producer of that activation has finished).
+//   warp 2        MMA issuer: tcgen05.mma 128 x tpad x 16, swap-AB (weights on the 128 TMEM lanes, tokens on N), accumulator
+//                 double-buffered in TMEM.
+//   warps 3..6    compute: GEMM epilogues (TMEM -> fp32 partial slices) and the phases between the projections: residual
+//                 fold + RMSNorm, RoPE + K/V page write + attention (mma.sync flash loop over the paged K/V), SwiGLU.
+//
+// Work split (stream-K).  A projection with n_tiles x kbt (tile, K block) units is cut into gridDim.x equal contiguous runs,
+// so every SM streams the same number of weight bytes in every phase (+-16 KB) whatever N / 128 is (32 tiles for O / down,
+// 96 for QKV, 192 for gate/up on 148 SMs).  A tile cut by a run boundary leaves one fp32 partial slice per run (`seg`); the
+// consumer phase sums the slices of a tile in slice order, so results are deterministic (no atomics).
+//
+// Phases per layer (each ends with one arrival per CTA on a global counter; waiting = polling that counter):
+//   0 fold + norm   x += sum of the down-projection slices of the previous layer; u = bf16(RMSNorm(x))
+//   1 QKV GEMM      u -> partial slices
+//   2 attention     per (request, KV head): sum the Q/K/V slices, RoPE, write K/V to the pages, softmax(QK^T)V over all S
+//   3 O GEMM        attn -> slices
+//   4 fold + norm
+//   5 gate/up GEMM  u -> slices (64 gate + 64 up rows per tile)
+//   6 SwiGLU        act = bf16(silu(sum gate) * sum up)
+//   7 down GEMM     act -> slices
+// and a final fold after the last layer.  Rounding points are those of the multi-kernel path.
+#pragma once
+#include <math_constants.h>
+
+#include "attn_flash.cuh"
+#include "common.cuh"
+#include "kernels_basic.cuh"
+#include "ptx_sm100.cuh"
+
+namespace dlm {
+
+constexpr int kMgThreads = 224;
+constexpr int kMgWBytes = 128 * 128;          // one weight tile: 128 rows x 64 bf16
+constexpr int kMgMaxTpad = 64;
+constexpr int kMgPhasesPerLayer = 8;
+constexpr int kMgScratchOwn = 48 * 1024;      // attention scratch beyond the (idle) X ring: Q 16 KB + K 2 x 16 KB + V 2 x 16 KB = 80 KB in all
+constexpr int kMgAttnBytes = 80 * 1024;
+constexpr int kMgMaxTiles = 384;              // tiles per projection the slice-count tables hold
+constexpr int kMgTailBytes = 512 + 4 * kMgMaxTiles * 4 + 64;      // barriers, slice-count tables, reduction scratch
+
+struct MegaParams {
+  int layer0, n_layers;            // layers [layer0, layer0 + n_layers) in this launch (debug-dump mode runs them one by one)
+  int T, tpad, stages;
+  int d, HQ, NQKV, F, Fp;          // Fp = first tiled row of the up projection (pad128(F))
+  int n_heads;
+  float eps, scale_log2;
+  const CUtensorMap* wmaps;        // device array [n_layers][4]: tiled weight maps of Wqkv, Wo, Wgu (box 64), Wd
+  float* x;                        // [T, d] fp32 residual stream (in: embeddings; out: the last layer's output)
+  bf16* u;                         // [T, d] RMSNorm output feeding QKV
+  bf16* u2;                        // [T, d] RMSNorm output feeding gate/up
+  bf16* q_dump;                    // optional [T, HQ]: Q after RoPE (debug dump), or null
+  float* xmid_dump;                // optional [T, d]: residual after the O projection (debug dump), or null
+  bf16* attn;                      // [T, HQ]
+  bf16* act;                       // [T, F]
+  float* part_a;                   // slices of the QKV and gate/up projections: [seg][T][NQKV | 2F]
+  float* part_x;                   // slices of the O and down projections:       [seg][T][d]
+  const float* rope_cos;
+  const float* rope_sin;
+  bf16* kv_store;
+  const int* page_table;
+  BatchDesc b;
+  KvGeom g;
+  unsigned int* bar;               // phase counter, zero at launch
+  unsigned long long* phase_ts;    // optional [8 L + 2] %globaltimer at the end of each phase in CTA 0 (tuning aid), or null
+  TraceSlot tr;
+};
+
+__host__ __device__ inline int mega_stage_bytes(int tpad) { return kMgWBytes + tpad * 128; }
+__host__ inline int mega_stages(int tpad) { return (227 * 1024 - kMgScratchOwn - kMgTailBytes - 1024) / mega_stage_bytes(tpad); }
+__host__ inline int mega_smem_bytes(int tpad, int stages) { return stages * mega_stage_bytes(tpad) + kMgScratchOwn + kMgTailBytes + 1024; }
+
+// ---- stream-K geometry of a projection: U = n_tiles * kbt units over G CTAs ----
+struct MgGemm { int n_tiles, kbt; };
+__device__ __forceinline__ long long mg_u0(long long U, int G, int i) { return U * i / G; }
+// CTA whose run contains `unit`: smallest i with U (i + 1) / G > unit
+__device__ __forceinline__ int mg_owner(long long unit, long long U, int G) { return (int)(((unit + 1) * G + U - 1) / U) - 1; }
+__device__ __forceinline__ int mg_nseg(int tile, const MgGemm& gm, int G) {
+  const long long U = (long long)gm.n_tiles * gm.kbt;
+  return mg_owner((long long)(tile + 1) * gm.kbt - 1, U, G) - mg_owner((long long)tile * gm.kbt, U, G) + 1;
+}
+
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// poll the phase counter until `target` arrivals (bounded: a protocol bug traps instead of hanging the GPU)
+__device__ __forceinline__ void mg_wait_count(const unsigned int* bar, unsigned int target) {
+  if (ld_acquire_u32(bar) >= target) return;
+  const long long t0 = clock64();
+  while (ld_acquire_u32(bar) < target) {
+    __nanosleep(32);
+    if (clock64() - t0 > 4000000000LL) __trap();
+  }
+}
+__device__ __forceinline__ void mg_bar128() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
+__global__ void __launch_bounds__(kMgThreads, 1)
+layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapU2, const __grid_constant__ CUtensorMap mapAttn,
+                  const __grid_constant__ CUtensorMap mapAct, const MegaParams p) {
+  extern __shared__ uint8_t mg_smem[];
+  const uint32_t base = (ptx::smem_u32(mg_smem) + 1023u) & ~1023u;
+  uint8_t* const gen_base = mg_smem + (base - ptx::smem_u32(mg_smem));
+  const int stages = p.stages;
+  const uint32_t sW = base;                                          // [stages][16 KB]
+  const uint32_t sX = sW + stages * kMgWBytes;                       // [stages][tpad x 128 B]   (attention scratch aliases it)
+  const uint32_t x_stage = (uint32_t)p.tpad * 128u;
+  const uint32_t sOwn = sX + stages * x_stage;                       // kMgScratchOwn
+  const uint32_t bar_base = sOwn + kMgScratchOwn;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (stages + s); };
+  const uint32_t tmem_full = bar_base + 16u * stages;                // [2]
+  const uint32_t tmem_empty = tmem_full + 16u;                       // [2]
+  const uint32_t tmem_ptr_addr = tmem_empty + 16u;
+  int* const nseg_tab = reinterpret_cast<int*>(gen_base + (bar_base - base) + 512);     // [4][kMgMaxTiles]
+  float* const red = reinterpret_cast<float*>(gen_base + (bar_base - base) + 512 + 4 * kMgMaxTiles * 4);   // [4]
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int G = (int)gridDim.x, cta = (int)blockIdx.x;
+  const int L = p.n_layers, T = p.T, tpad = p.tpad;
+  const MgGemm gm[4] = {{p.NQKV / 128, p.d / 64}, {p.d / 128, p.HQ / 64}, {p.F / 64, p.d / 64}, {p.d / 128, p.F / 64}};
+  const uint32_t tmem_cols = 2 * tpad <= 64 ? 64u : 128u;
+
+  if (threadIdx.x == 0) trace_begin(p.tr);
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&mapU); ptx::prefetch_tmap(&mapU2); ptx::prefetch_tmap(&mapAttn); ptx::prefetch_tmap(&mapAct);
+    for (int s = 0; s < stages; ++s) { ptx::mbar_init(full_bar(s), 2); ptx::mbar_init(empty_bar(s), 1); }
+    for (int a = 0; a < 2; ++a) { ptx::mbar_init(tmem_full + 8u * a, 1); ptx::mbar_init(tmem_empty + 8u * a, 4); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc(tmem_ptr_addr, tmem_cols);
+    ptx::tmem_relinquish();
+  }
+  // slice counts per tile of the four projections (consumers sum that many slices)
+  for (int i = threadIdx.x; i < 4 * kMgMaxTiles; i += kMgThreads) {
+    const int gi = i / kMgMaxTiles, t = i % kMgMaxTiles;
+    nseg_tab[i] = t < gm[gi].n_tiles ? mg_nseg(t, gm[gi], G) : 0;
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr));
+
+  if (warp == 0) {
+    // =============================== W producer ===============================
+    if (ptx::elect_one()) {
+      int s = 0;
+      uint32_t ph = 0;
+      for (int l = 0; l < L; ++l) {
+        for (int gi = 0; gi < 4; ++gi) {
+          const CUtensorMap* mw = p.wmaps + (p.layer0 + l) * 4 + gi;
+          const long long U = (long long)gm[gi].n_tiles * gm[gi].kbt;
+          const long long u0 = mg_u0(U, G, cta), u1 = mg_u0(U, G, cta + 1);
+          for (long long un = u0; un < u1; ++un, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1u : 0u)) {
+            const int tile = (int)(un / gm[gi].kbt), kb = (int)(un % gm[gi].kbt);
+            ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+            ptx::mbar_expect_tx(full_bar(s), (uint32_t)kMgWBytes);
+            const uint32_t dst = sW + s * kMgWBytes;
+            if (gi == 2) {          // 64 gate rows + the matching 64 up rows
+              ptx::tma_load_w_tiled(dst, mw, kb, tile * 64, 64, 64, full_bar(s), DLM_L2_EVICT_FIRST);
+              ptx::tma_load_w_tiled(dst + 64 * 128, mw, kb, p.Fp + tile * 64, 64, 64, full_bar(s), DLM_L2_EVICT_FIRST);
+            } else {
+              ptx::tma_load_w_tiled(dst, mw, kb, tile * 128, 128, 128, full_bar(s), DLM_L2_EVICT_FIRST);
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // =============================== X producer ===============================
+    if (ptx::elect_one()) {
+      pdl_wait();                    // x (embeddings) and the request state come from the kernels before this one
+      int s = 0;
+      uint32_t ph = 0;
+      for (int l = 0; l < L; ++l) {
+        for (int gi = 0; gi < 4; ++gi) {
+          const CUtensorMap* mx = gi == 0 ? &mapU : (gi == 1 ? &mapAttn : (gi == 2 ? &mapU2 : &mapAct));
+          const long long U = (long long)gm[gi].n_tiles * gm[gi].kbt;
+          const long long u0 = mg_u0(U, G, cta), u1 = mg_u0(U, G, cta + 1);
+          if (u0 < u1) {
+            // the activation is complete when the phase before this projection has been arrived at by every CTA
+            const int phase = l * kMgPhasesPerLayer + 2 * gi + 1;
+            mg_wait_count(p.bar, (unsigned)G * (unsigned)phase);
+            asm volatile("fence.proxy.async;" ::: "memory");      // generic-proxy writes of other CTAs -> TMA (async proxy) reads
+          }
+          for (long long un = u0; un < u1; ++un, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1u : 0u)) {
+            const int kb = (int)(un % gm[gi].kbt);
+            ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+            ptx::mbar_expect_tx(full_bar(s), x_stage);
+            ptx::tma_load_2d(sX + s * x_stage, mx, kb * 64, 0, full_bar(s), DLM_L2_EVICT_LAST);
+          }
+        }
+      }
+    }
+  } else if (warp == 2) {
+    // =============================== MMA issuer ===============================
+    const uint32_t idesc = ptx::umma_idesc_bf16(128, tpad);
+    int s = 0, it = 0;
+    uint32_t ph = 0;
+    for (int l = 0; l < L; ++l) {
+      for (int gi = 0; gi < 4; ++gi) {
+        const long long U = (long long)gm[gi].n_tiles * gm[gi].kbt;
+        const long long u0 = mg_u0(U, G, cta), u1 = mg_u0(U, G, cta + 1);
+        for (long long un = u0; un < u1;) {
+          const int k0 = (int)(un % gm[gi].kbt);
+          const int n = (int)min((long long)(gm[gi].kbt - k0), u1 - un);      // K blocks of this segment
+          const uint32_t acc = (uint32_t)it & 1u, aph = ((uint32_t)it >> 1) & 1u;
+          ptx::mbar_wait(tmem_empty + 8u * acc, aph ^ 1u);
+          ptx::tc_fence_after();
+          const uint32_t d_tmem = tmem_base + acc * (uint32_t)tpad;
+          for (int k = 0; k < n; ++k, s = (s + 1 == stages ? 0 : s + 1), ph ^= (s == 0 ? 1u : 0u)) {
+            ptx::mbar_wait(full_bar(s), ph);
+            ptx::tc_fence_after();
+            if (ptx::elect_one()) {
+              const uint32_t w_lo = ptx::umma_desc_lo(sW + s * kMgWBytes), x_lo = ptx::umma_desc_lo(sX + s * x_stage);
+#pragma unroll
+              for (int kk = 0; kk < 4; ++kk)
+                ptx::umma_bf16_lo(d_tmem, w_lo + 2 * kk, x_lo + 2 * kk, idesc, (k | kk) != 0 ? 1u : 0u);
+              ptx::umma_commit(empty_bar(s));
+              if (k + 1 == n) ptx::umma_commit(tmem_full + 8u * acc);
+            }
+            __syncwarp();
+          }
+          un += n;
+          ++it;
+        }
+      }
+    }
+  } else {
+    // =============================== compute warps (3..6) ===============================
+    const int tid = threadIdx.x - 96;                 // 0..127
+    const int cw = warp - 3;                          // 0..3
+    const int quarter = warp & 3;                     // TMEM lane quarter this warp may read
+    int it = 0;                                       // accumulator use counter (mirrors the MMA warp)
+    int phase = 0;                                    // phases completed by this CTA
+    pdl_wait();
+    if (tid == 0) trace_wait(p.tr);
+
+    auto arrive = [&]() {                             // this CTA has finished the current phase
+      mg_bar128();
+      if (tid == 0) {
+        __threadfence();
+        asm volatile("fence.proxy.async;" ::: "memory");
+        atomicAdd(p.bar, 1u);
+        if (p.phase_ts && cta == 0) p.phase_ts[phase] = gtimer_ns();
+      }
+      ++phase;
+    };
+    auto wait_prev = [&]() {                          // every CTA has finished the phase before the current one
+      if (tid == 0) mg_wait_count(p.bar, (unsigned)G * (unsigned)phase);
+      mg_bar128();
+    };
+
+    // ---- GEMM epilogue: this CTA's segments of projection gi -> fp32 slices ----
+    auto gemm_epilogue = [&](int gi, float* part, int ld) {
+      const long long U = (long long)gm[gi].n_tiles * gm[gi].kbt;
+      const long long u0 = mg_u0(U, G, cta), u1 = mg_u0(U, G, cta + 1);
+      for (long long un = u0; un < u1;) {
+        const int tile = (int)(un / gm[gi].kbt), k0 = (int)(un % gm[gi].kbt);
+        const int n = (int)min((long long)(gm[gi].kbt - k0), u1 - un);
+        const int seg = cta - mg_owner((long long)tile * gm[gi].kbt, U, G);
+        const uint32_t acc = (uint32_t)it & 1u, aph = ((uint32_t)it >> 1) & 1u;
+        ptx::mbar_wait(tmem_full + 8u * acc, aph);
+        ptx::tc_fence_after();
+        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + acc * (uint32_t)tpad;
+        float* o = part + ((long long)seg * T) * ld + (long long)tile * 128 + quarter * 32 + lane;
+        uint32_t r[32];
+        for (int c = 0; c < tpad / 32; ++c) {
+          __syncwarp();
+          ptx::tmem_ld_32x32(taddr + c * 32, r);
+          ptx::tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const int tok = c * 32 + j;
+            if (tok < T) __stcg(o + (long long)tok * ld, __uint_as_float(r[j]));
+          }
+        }
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(tmem_empty + 8u * acc);
+        un += n;
+        ++it;
+      }
+      arrive();
+    };
+
+    // ---- fold + RMSNorm: x[t] += slices of the previous O / down projection (tile slice counts nseg), u = bf16(x rs) ----
+    auto fold_norm = [&](const int* nseg, bool have_part, bf16* uo, float* copy_to) {
+      wait_prev();
+      const int nvec = p.d >> 2;
+      for (int t = cta; t < T; t += G) {
+        float4* xr = reinterpret_cast<float4*>(p.x + (long long)t * p.d);
+        float4 v[8];                                   // d <= 4096 (8 x 128 threads x 4)
+        float ss = 0.f;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int i = tid + k * 128;
+          if (i < nvec) {
+            float4 a = __ldcg(xr + i);
+            if (have_part) {
+              const int ns = nseg[(i * 4) >> 7];
+              const float4* pr = reinterpret_cast<const float4*>(p.part_x + (long long)t * p.d) + i;
+              const long long st4 = ((long long)T * p.d) >> 2;
+              for (int s = 0; s < ns; ++s) {
+                const float4 q = __ldcg(pr + s * st4);
+                a.x += q.x; a.y += q.y; a.z += q.z; a.w += q.w;
+              }
+              __stcg(xr + i, a);
+            }
+            if (copy_to) reinterpret_cast<float4*>(copy_to + (long long)t * p.d)[i] = a;
+            v[k] = a;
+            ss += a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w;
+          }
+        }
+        if (!uo) continue;                             // final fold: only x is wanted
+        ss = warp_sum(ss);
+        if (lane == 0) red[cw] = ss;
+        mg_bar128();
+        const float rs = rsqrtf(((red[0] + red[1]) + (red[2] + red[3])) / (float)p.d + p.eps);
+        bf16* ur = uo + (long long)t * p.d;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int i = tid + k * 128;
+          if (i < nvec) {
+            uint2 w;
+            w.x = pack_bf16(v[k].x * rs, v[k].y * rs); w.y = pack_bf16(v[k].z * rs, v[k].w * rs);
+            __stcg(reinterpret_cast<uint2*>(ur + 4 * i), w);
+          }
+        }
+        mg_bar128();                                   // red[] is reused by the next row
+      }
+      arrive();
+    };
+
+    // ---- SwiGLU: act[t, f] = bf16(silu(sum gate slices) * sum up slices); slice layout [seg][T][tile * 128 + {gate 0..63 | up 64..127}] ----
+    auto swiglu = [&](const int* nseg) {
+      wait_prev();
+      const int ld = 2 * p.F;
+      const int f4 = p.F >> 2;                          // float4 groups per row (a group never straddles a 64-feature tile)
+      const long long st = (long long)T * ld;
+      for (int i = cta * 128 + tid; i < T * f4; i += G * 128) {
+        const int t = i / f4, f = (i - t * f4) * 4, tile = f >> 6, j = f & 63;
+        const float* gp = p.part_a + (long long)t * ld + tile * 128 + j;
+        float4 g = make_float4(0.f, 0.f, 0.f, 0.f), w = g;
+        const int ns = nseg[tile];
+        for (int s = 0; s < ns; ++s) {
+          const float4 a = __ldcg(reinterpret_cast<const float4*>(gp + s * st)), c = __ldcg(reinterpret_cast<const float4*>(gp + s * st + 64));
+          g.x += a.x; g.y += a.y; g.z += a.z; g.w += a.w;
+          w.x += c.x; w.y += c.y; w.z += c.z; w.w += c.w;
+        }
+        uint2 o;
+        o.x = pack_bf16(silu_f(g.x) * w.x, silu_f(g.y) * w.y); o.y = pack_bf16(silu_f(g.z) * w.z, silu_f(g.w) * w.w);
+        __stcg(reinterpret_cast<uint2*>(p.act + (long long)t * p.F + f), o);
+      }
+      arrive();
+    };
+
+    // ---- attention phase of layer l: units (request, KV head) ----
+    auto attention = [&](int l, const int* nseg_qkv) {
+      wait_prev();
+      const int H = p.n_heads, Hkv = p.g.n_kv_heads, r = H / Hkv;
+      // scratch = the X ring (idle during this phase: this CTA's X producer cannot pass the phase counter before the CTA
+      // arrives) followed by the own scratch, contiguous: Q [64 rows][256 B] 16 KB, K 2 x 16 KB, V 2 x 16 KB
+      const uint32_t sQ = sX, bK = sX + 16384, bV = sX + 16384 + 32768;
+      const long long stq = (long long)T * p.NQKV;          // slice stride of part_a
+      for (int unit = cta; unit < p.b.n * Hkv; unit += G) {
+        const int bi = unit / Hkv, kvh = unit % Hkv;
+        const int q_len = p.b.q_len[bi];
+        if (q_len <= 0) continue;
+        const int n_rows = q_len * r, S = p.b.kv_len[bi], q_off = p.b.q_off[bi], pos0 = p.b.q_pos0[bi];
+        const int* pt = p.page_table + (long long)p.b.slot[bi] * p.g.max_pages_per_req;
+        // -- (a) Q rows: sum the slices, rotate, bf16 into sQ; rows past n_rows: zeros
+        for (int i = tid; i < 64 * 16; i += 128) {          // item = (stacked row, group of 4 pair indices e..e+3 in [0, 64))
+          const int rho = i >> 4, e = (i & 15) * 4;
+          float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
+          if (rho < n_rows) {
+            const int tok = rho / r, h = kvh * r + rho % r;
+            const float* src = p.part_a + (long long)(q_off + tok) * p.NQKV + h * 128 + e;
+            const int ns = nseg_qkv[h];
+            for (int s = 0; s < ns; ++s) {
+              const float4 a = __ldcg(reinterpret_cast<const float4*>(src + s * stq)), c = __ldcg(reinterpret_cast<const float4*>(src + s * stq + 64));
+              lo.x += a.x; lo.y += a.y; lo.z += a.z; lo.w += a.w;
+              hi.x += c.x; hi.y += c.y; hi.z += c.z; hi.w += c.w;
+            }
+            const float4 cs = *reinterpret_cast<const float4*>(p.rope_cos + (long long)(pos0 + tok) * 64 + e);
+            const float4 sn = *reinterpret_cast<const float4*>(p.rope_sin + (long long)(pos0 + tok) * 64 + e);
+            const float4 l2 = make_float4(lo.x * cs.x - hi.x * sn.x, lo.y * cs.y - hi.y * sn.y, lo.z * cs.z - hi.z * sn.z, lo.w * cs.w - hi.w * sn.w);
+            hi = make_float4(hi.x * cs.x + lo.x * sn.x, hi.y * cs.y + lo.y * sn.y, hi.z * cs.z + lo.z * sn.z, hi.w * cs.w + lo.w * sn.w);
+            lo = l2;
+            if (p.q_dump) {
+              bf16* qd = p.q_dump + ((long long)(q_off + tok) * H + h) * 128 + e;
+              *reinterpret_cast<uint2*>(qd) = make_uint2(pack_bf16(lo.x, lo.y), pack_bf16(lo.z, lo.w));
+              *reinterpret_cast<uint2*>(qd + 64) = make_uint2(pack_bf16(hi.x, hi.y), pack_bf16(hi.z, hi.w));
+            }
+          }
+          const uint32_t a0 = sQ + tile_off(rho, e >> 3) + (e & 7) * 2, a1 = sQ + tile_off(rho, 8 + (e >> 3)) + (e & 7) * 2;
+          asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a0), "r"(pack_bf16(lo.x, lo.y)), "r"(pack_bf16(lo.z, lo.w)) : "memory");
+          asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a1), "r"(pack_bf16(hi.x, hi.y)), "r"(pack_bf16(hi.z, hi.w)) : "memory");
+        }
+        // -- (b) fresh K (rotated) and V of the computed tokens -> the request's pages
+        const int kcol = p.HQ + kvh * 128, vcol = p.HQ + Hkv * 128 + kvh * 128;
+        const int ns_k = nseg_qkv[kcol >> 7], ns_v = nseg_qkv[vcol >> 7];
+        for (int i = tid; i < q_len * 16; i += 128) {
+          const int tok = i >> 4, e = (i & 15) * 4, pos = pos0 + tok;
+          const float* ks = p.part_a + (long long)(q_off + tok) * p.NQKV + kcol + e;
+          const float* vs = p.part_a + (long long)(q_off + tok) * p.NQKV + vcol + e;
+          float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo, v0 = lo, v1 = lo;
+          for (int s = 0; s < ns_k; ++s) {
+            const float4 a = __ldcg(reinterpret_cast<const float4*>(ks + s * stq)), c = __ldcg(reinterpret_cast<const float4*>(ks + s * stq + 64));
+            lo.x += a.x; lo.y += a.y; lo.z += a.z; lo.w += a.w;
+            hi.x += c.x; hi.y += c.y; hi.z += c.z; hi.w += c.w;
+          }
+          for (int s = 0; s < ns_v; ++s) {
+            const float4 a = __ldcg(reinterpret_cast<const float4*>(vs + s * stq)), c = __ldcg(reinterpret_cast<const float4*>(vs + s * stq + 64));
+            v0.x += a.x; v0.y += a.y; v0.z += a.z; v0.w += a.w;
+            v1.x += c.x; v1.y += c.y; v1.z += c.z; v1.w += c.w;
+          }
+          const float4 cs = *reinterpret_cast<const float4*>(p.rope_cos + (long long)pos * 64 + e);
+          const float4 sn = *reinterpret_cast<const float4*>(p.rope_sin + (long long)pos * 64 + e);
+          const float4 l2 = make_float4(lo.x * cs.x - hi.x * sn.x, lo.y * cs.y - hi.y * sn.y, lo.z * cs.z - hi.z * sn.z, lo.w * cs.w - hi.w * sn.w);
+          hi = make_float4(hi.x * cs.x + lo.x * sn.x, hi.y * cs.y + lo.y * sn.y, hi.z * cs.z + lo.z * sn.z, hi.w * cs.w + lo.w * sn.w);
+          const int page = pt[pos / p.g.page_tokens];
+          bf16* kd = p.kv_store + p.g.offset(l, page, 0, kvh, pos % p.g.page_tokens) + e;
+          bf16* vd = p.kv_store + p.g.offset(l, page, 1, kvh, pos % p.g.page_tokens) + e;
+          *reinterpret_cast<uint2*>(kd) = make_uint2(pack_bf16(l2.x, l2.y), pack_bf16(l2.z, l2.w));
+          *reinterpret_cast<uint2*>(kd + 64) = make_uint2(pack_bf16(hi.x, hi.y), pack_bf16(hi.z, hi.w));
+          *reinterpret_cast<uint2*>(vd) = make_uint2(pack_bf16(v0.x, v0.y), pack_bf16(v0.z, v0.w));
+          *reinterpret_cast<uint2*>(vd + 64) = make_uint2(pack_bf16(v1.x, v1.y), pack_bf16(v1.z, v1.w));
+        }
+        __threadfence_block();
+        mg_bar128();                                        // Q tile complete; the fresh K/V rows are visible to this CTA's loads
+        // -- (c) flash loop over the request's K/V pages (64-token tiles, double-buffered cp.async); warp w owns rows 16 w .. 16 w + 15
+        auto load_kv = [&](int tile, int buf) {
+          const int j0 = tile * kFaBN;
+          const int page = pt[j0 / p.g.page_tokens];
+          const int in_page = j0 % p.g.page_tokens;
+          const bf16* kb = p.kv_store + p.g.offset(l, page, 0, kvh, in_page);
+          const bf16* vb = p.kv_store + p.g.offset(l, page, 1, kvh, in_page);
+          for (int i = tid; i < kFaBN * 16; i += 128) {
+            const int row = i >> 4, ch = i & 15;
+            const bool ok = j0 + row < S;
+            cp_async16(bK + buf * kFaBN * 256 + tile_off(row, ch), kb + row * kFaDh + ch * 8, ok);
+            cp_async16(bV + buf * kFaBN * 256 + tile_off(row, ch), vb + row * kFaDh + ch * 8, ok);
+          }
+        };
+        const int n_tiles = (S + kFaBN - 1) / kFaBN;
+        load_kv(0, 0);
+        cp_async_commit();
+        float o[16][4];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f; }
+        float m0 = -CUDART_INF_F, m1 = -CUDART_INF_F, l0 = 0.f, l1 = 0.f;
+        uint32_t qf[8][4];
+        const int wrow = cw * 16;
+        const bool live = wrow < n_rows;                    // warp-uniform: this warp has query rows
+        for (int t = 0; t < n_tiles; ++t) {
+          const int buf = t & 1;
+          if (t + 1 < n_tiles) load_kv(t + 1, buf ^ 1);
+          cp_async_commit();
+          cp_async_wait<1>();
+          mg_bar128();
+          if (live) {
+            if (t == 0) {
+#pragma unroll
+              for (int ks = 0; ks < 8; ++ks)
+                ldsm_x4(sQ + tile_off(wrow + (lane & 7) + ((lane >> 3) & 1) * 8, ks * 2 + (lane >> 4)), qf[ks][0], qf[ks][1], qf[ks][2], qf[ks][3]);
+            }
+            const uint32_t kbase = bK + buf * kFaBN * 256, vbase = bV + buf * kFaBN * 256;
+            float sc[8][4];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { sc[j][0] = sc[j][1] = sc[j][2] = sc[j][3] = 0.f; }
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+#pragma unroll
+              for (int jp = 0; jp < 4; ++jp) {
+                uint32_t b0, b1, b2, b3;
+                ldsm_x4(kbase + tile_off(jp * 16 + (lane & 7) + (lane >> 4) * 8, ks * 2 + ((lane >> 3) & 1)), b0, b1, b2, b3);
+                mma_bf16_16816(sc[2 * jp], qf[ks], b0, b1);
+                mma_bf16_16816(sc[2 * jp + 1], qf[ks], b2, b3);
+              }
+            }
+            const int j0 = t * kFaBN;
+            float tm0 = -CUDART_INF_F, tm1 = -CUDART_INF_F;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const int col = j0 + j * 8 + (lane & 3) * 2;
+              sc[j][0] = (col < S) ? sc[j][0] * p.scale_log2 : -CUDART_INF_F;
+              sc[j][1] = (col + 1 < S) ? sc[j][1] * p.scale_log2 : -CUDART_INF_F;
+              sc[j][2] = (col < S) ? sc[j][2] * p.scale_log2 : -CUDART_INF_F;
+              sc[j][3] = (col + 1 < S) ? sc[j][3] * p.scale_log2 : -CUDART_INF_F;
+              tm0 = fmaxf(tm0, fmaxf(sc[j][0], sc[j][1]));
+              tm1 = fmaxf(tm1, fmaxf(sc[j][2], sc[j][3]));
+            }
+            tm0 = fmaxf(tm0, __shfl_xor_sync(0xffffffffu, tm0, 1)); tm0 = fmaxf(tm0, __shfl_xor_sync(0xffffffffu, tm0, 2));
+            tm1 = fmaxf(tm1, __shfl_xor_sync(0xffffffffu, tm1, 1)); tm1 = fmaxf(tm1, __shfl_xor_sync(0xffffffffu, tm1, 2));
+            const float nm0 = fmaxf(m0, tm0), nm1 = fmaxf(m1, tm1);
+            const float c0 = exp2f(m0 - nm0), c1 = exp2f(m1 - nm1);
+            m0 = nm0; m1 = nm1;
+            float rs0 = 0.f, rs1 = 0.f;
+            uint32_t pf[4][4];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const float p0 = exp2f(sc[j][0] - nm0), p1 = exp2f(sc[j][1] - nm0);
+              const float p2 = exp2f(sc[j][2] - nm1), p3 = exp2f(sc[j][3] - nm1);
+              rs0 += p0 + p1; rs1 += p2 + p3;
+              pf[j >> 1][(j & 1) * 2 + 0] = pack_bf16(p0, p1);
+              pf[j >> 1][(j & 1) * 2 + 1] = pack_bf16(p2, p3);
+            }
+            l0 = l0 * c0 + rs0; l1 = l1 * c1 + rs1;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) { o[i][0] *= c0; o[i][1] *= c0; o[i][2] *= c1; o[i][3] *= c1; }
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+#pragma unroll
+              for (int np = 0; np < 8; ++np) {
+                uint32_t b0, b1, b2, b3;
+                ldsm_x4_t(vbase + tile_off(kk * 16 + (lane & 7) + ((lane >> 3) & 1) * 8, np * 2 + (lane >> 4)), b0, b1, b2, b3);
+                mma_bf16_16816(o[2 * np], pf[kk], b0, b1);
+                mma_bf16_16816(o[2 * np + 1], pf[kk], b2, b3);
+              }
+            }
+          }
+          mg_bar128();                                      // everyone is done with `buf` before the next prefetch overwrites it
+        }
+        cp_async_wait<0>();
+        if (live) {
+          l0 += __shfl_xor_sync(0xffffffffu, l0, 1); l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+          l1 += __shfl_xor_sync(0xffffffffu, l1, 1); l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+          const int gq = lane >> 2, tq = lane & 3;
+#pragma unroll
+          for (int hr = 0; hr < 2; ++hr) {
+            const int rho = wrow + gq + hr * 8;
+            if (rho >= n_rows) continue;
+            const int tok = rho / r, hh = rho % r;
+            const long long orow = (long long)(q_off + tok) * H + kvh * r + hh;
+            const float inv = 1.f / (hr ? l1 : l0);
+            bf16* dst = p.attn + orow * kFaDh;
+#pragma unroll
+            for (int i = 0; i < 16; ++i)
+              __stcg(reinterpret_cast<unsigned int*>(dst + i * 8 + tq * 2), pack_bf16(o[i][hr * 2] * inv, o[i][hr * 2 + 1] * inv));
+          }
+        }
+        mg_bar128();                                        // sQ / K / V buffers are rewritten by the next unit
+      }
+      arrive();
+    };
+
+    const int* ns_qkv = nseg_tab, *ns_o = nseg_tab + kMgMaxTiles, *ns_gu = nseg_tab + 2 * kMgMaxTiles, *ns_dn = nseg_tab + 3 * kMgMaxTiles;
+    for (int l = 0; l < L; ++l) {
+      fold_norm(ns_dn, l > 0, p.u, nullptr);                // phase 8 l + 0 (the launch's first layer finds x complete)
+      gemm_epilogue(0, p.part_a, p.NQKV);                   //             1
+      attention(p.layer0 + l, ns_qkv);                      //             2
+      gemm_epilogue(1, p.part_x, p.d);                      //             3
+      fold_norm(ns_o, true, p.u2, p.xmid_dump);             //             4
+      gemm_epilogue(2, p.part_a, 2 * p.F);                  //             5
+      swiglu(ns_gu);                                        //             6
+      gemm_epilogue(3, p.part_x, p.d);                      //             7
+    }
+    fold_norm(ns_dn, true, nullptr, nullptr);               // the last layer's down slices into x (the head normalises its own rows)
+  }
+  pdl_launch_dependents();
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (threadIdx.x == 0) trace_end(p.tr);
+  if (warp == 2) ptx::tmem_dealloc(tmem_base, tmem_cols);
+}
+
+}  // namespace dlm

@@ -444,7 +444,7 @@ def test_launch_modes_agree_bitwise():
         for a, b in zip(outs["production"], outs[mode]):
             assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2]) and a[3] == b[3], mode
     for a, b in zip(outs["production"], outs["no_skinny"]):     # different K summation order: close, not identical
-        assert np.allclose(a[0], b[0], rtol=0, atol=5e-2) and np.allclose(a[1], b[1], rtol=0, atol=2e-2)
+        assert np.allclose(a[0], b[0], rtol=0, atol=1e-1) and np.allclose(a[1], b[1], rtol=0, atol=3e-2)      # lse ~24: 4e-3 relative, the bf16 floor between two GEMM paths
 
 
 def test_c5_reduced_depth_gqa_teacher_forced():
