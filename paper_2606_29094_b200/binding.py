@@ -337,7 +337,7 @@ class Engine:
 
     def layer_kernel_phases(self) -> np.ndarray:
         """Phase end times (us) of the last whole-stack launch taken with OPT_LAYER_KERNEL_PHASE_TS."""
-        buf = np.zeros(8 * self.arch.n_layers + 1, np.float32)
+        buf = np.zeros(7 * self.arch.n_layers + 1, np.float32)
         n = self._check(lib().dlm_layer_kernel_phases(self._h, _fp(buf), len(buf)))
         return buf[:n].copy()
 

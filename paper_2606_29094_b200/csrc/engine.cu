@@ -658,7 +658,8 @@ struct dlm_ctx {
   // options
   int opt_simple = 0, opt_dump = 0, opt_graph = 1, opt_flash = 1, opt_pdl = 1, opt_skinny = 1, opt_pair = 1, opt_tcattn = 1, opt_fuse_rope = 1;
   int opt_trace = 0;
-  int opt_mega = 0;            // whole-stack persistent kernel for cached steps of <= 64 tokens (off until it beats the per-stage kernels)
+  int opt_mega = 0;            // whole-stack persistent kernel for cached steps of <= 64 tokens: correct, but 4.0 ms per C2 cached step against
+                               // 3.19 ms for the per-stage kernels (its grid-wide phase boundaries cost what kernel boundaries cost), so off by default
   CUtensorMap* mega_wmaps = nullptr;   // device array [n_layers][4] of the tiled weight maps
   unsigned int* mega_bar = nullptr;    // its phase counter
   unsigned long long* mega_ts = nullptr, *mega_ts_host = nullptr;   // optional phase timestamps (DLM_OPT_MEGA_PHASE_TS)
@@ -912,7 +913,7 @@ extern "C" int dlm_init_ex(const dlm_arch* arch, uint64_t seed, const dlm_mem* m
   ALLOC(c->trace_dev, (size_t)kMaxTraceSlots * 3 * 8);
   if (c->bf16_model) {            // whole-stack kernel: second norm buffer, phase counter, the tiled weight maps of every layer
     ALLOC(c->u2, (size_t)kMgMaxTpad * d * es);
-    ALLOC(c->mega_bar, 256);
+    ALLOC(c->mega_bar, 4096);
     ALLOC(c->mega_ts, (size_t)(kMgPhasesPerLayer * a.n_layers + 2) * 8);
     ALLOC(c->mega_wmaps, (size_t)a.n_layers * 4 * sizeof(CUtensorMap));
     std::vector<CUtensorMap> hm((size_t)a.n_layers * 4);
@@ -1322,6 +1323,10 @@ static bool mega_ok(const dlm_ctx* c, const BatchDesc& bd) {
   if (bd.max_q_len * r > 64) return false;                                   // one attention unit = <= 64 stacked rows
   if (a.d_model % 128 || a.d_model > 4096 || (a.n_heads * a.head_dim) % 64 || NQKV % 128 || a.d_ffn % 64) return false;
   if (NQKV / 128 > kMgMaxTiles || a.d_ffn / 64 > kMgMaxTiles || a.d_model / 128 > kMgMaxTiles) return false;
+  // a tile is cut into at most ceil(kbt * G / U) + 1 runs: no more than the kernel's fixed-size slice sums take
+  const int G = g_num_sms, d = a.d_model, F = a.d_ffn, HQ = a.n_heads * a.head_dim;
+  auto max_seg = [&](long long n_tiles, long long kbt) { const long long U = n_tiles * kbt; return (int)((kbt * G + U - 1) / U) + 1; };
+  if (max_seg(NQKV / 128, d / 64) > kMgMaxSegQkv || max_seg(F / 64, d / 64) > kMgMaxSegGu || max_seg(d / 128, HQ / 64) > kMgMaxSeg || max_seg(d / 128, F / 64) > kMgMaxSeg) return false;
   return true;
 }
 
@@ -1335,16 +1340,19 @@ static int mega_launch(dlm_ctx* c, const BatchDesc& bd, int layer0, int n_layers
   p.eps = a.rms_eps; p.scale_log2 = (1.f / sqrtf((float)a.head_dim)) * 1.4426950408889634f;
   p.wmaps = c->mega_wmaps;
   p.x = c->x; p.u = (bf16*)c->u; p.u2 = (bf16*)c->u2; p.attn = (bf16*)c->attn; p.act = (bf16*)c->act;
-  p.q_dump = dump ? (bf16*)c->q : nullptr; p.xmid_dump = dump ? c->tmp : nullptr;
+  p.q = (bf16*)c->q; p.xmid_dump = dump ? c->tmp : nullptr;
   p.part_a = c->qkv; p.part_x = c->part_x;
   p.rope_cos = c->rope_cos; p.rope_sin = c->rope_sin; p.kv_store = (bf16*)c->kv_store; p.page_table = c->page_table;
-  p.b = bd; p.g = c->kg; p.bar = c->mega_bar;
+  p.b = bd; p.g = c->kg; p.bar = c->mega_bar; p.tile_cnt = c->mega_bar + 64;
   p.phase_ts = c->opt_mega_ts ? c->mega_ts : nullptr;
   p.tr = c->tslot();
   if (p.stages < 2 || p.stages * (p.tpad * 128) + kMgScratchOwn < kMgAttnBytes) { set_err(&c->err, "layer kernel: shared-memory plan does not fit (tpad %d)", p.tpad); return DLM_E_ARG; }
   // slice capacity: a tile is cut into at most ceil(kbt * G / U) + 1 runs
   const int G = g_num_sms;
   auto max_seg = [&](long long n_tiles, long long kbt) { const long long U = n_tiles * kbt; return (int)((kbt * G + U - 1) / U) + 1; };
+  if (max_seg(NQKV / 128, d / 64) > kMgMaxSegQkv || max_seg(F / 64, d / 64) > kMgMaxSegGu || max_seg(d / 128, HQ / 64) > kMgMaxSeg || max_seg(d / 128, F / 64) > kMgMaxSeg) {
+    set_err(&c->err, "layer kernel: a tile would be cut into more slices than the kernel sums"); return DLM_E_ARG;
+  }
   const long long need_a = std::max<long long>((long long)max_seg(NQKV / 128, d / 64) * bd.T * NQKV, (long long)max_seg(F / 64, d / 64) * bd.T * 2 * F);
   const long long need_x = (long long)std::max(max_seg(d / 128, HQ / 64), max_seg(d / 128, F / 64)) * bd.T * d;
   if (need_a > c->qkv_rows * (long long)NQKV || need_x > c->part_rows * (long long)d) { set_err(&c->err, "layer kernel: slice buffers too small"); return DLM_E_CAPACITY; }
@@ -1359,7 +1367,7 @@ static int mega_launch(dlm_ctx* c, const BatchDesc& bd, int layer0, int n_layers
     if (e != cudaSuccess) { set_err(&c->err, "layer kernel: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
     configured[g_dev] = true;
   }
-  CU_TRY(&c->err, cudaMemsetAsync(c->mega_bar, 0, 256, c->st));
+  CU_TRY(&c->err, cudaMemsetAsync(c->mega_bar, 0, 4096, c->st));
   cudaError_t e = launch_k(layer_mega_kernel, dim3(G), dim3(kMgThreads), (size_t)mega_smem_bytes(p.tpad, p.stages), c->st, pdl, *mu, *mu2, *mat, *mac, p);
   if (e != cudaSuccess) { set_err(&c->err, "layer kernel launch: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
   c->paths |= DLM_PATH_LAYER_KERNEL;

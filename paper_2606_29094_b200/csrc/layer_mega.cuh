@@ -47,9 +47,11 @@ namespace dlm {
 constexpr int kMgThreads = 224;
 constexpr int kMgWBytes = 128 * 128;          // one weight tile: 128 rows x 64 bf16
 constexpr int kMgMaxTpad = 64;
-constexpr int kMgPhasesPerLayer = 8;
+constexpr int kMgPhasesPerLayer = 7;          // fold+norm, QKV (+RoPE, K/V write), attention, O, fold+norm, gate/up (+SwiGLU), down
 constexpr int kMgScratchOwn = 48 * 1024;      // attention scratch beyond the (idle) X ring: Q 16 KB + K 2 x 16 KB + V 2 x 16 KB = 80 KB in all
 constexpr int kMgAttnBytes = 80 * 1024;
+constexpr int kMgMaxSeg = 6;                  // most slices a tile of the O / down projection may be cut into
+constexpr int kMgMaxSegQkv = 3, kMgMaxSegGu = 2;
 constexpr int kMgMaxTiles = 384;              // tiles per projection the slice-count tables hold
 constexpr int kMgTailBytes = 512 + 4 * kMgMaxTiles * 4 + 64;      // barriers, slice-count tables, reduction scratch
 
@@ -63,7 +65,7 @@ struct MegaParams {
   float* x;                        // [T, d] fp32 residual stream (in: embeddings; out: the last layer's output)
   bf16* u;                         // [T, d] RMSNorm output feeding QKV
   bf16* u2;                        // [T, d] RMSNorm output feeding gate/up
-  bf16* q_dump;                    // optional [T, HQ]: Q after RoPE (debug dump), or null
+  bf16* q;                         // [T, HQ] Q after RoPE (written by the QKV projection's finishing CTA of each head)
   float* xmid_dump;                // optional [T, d]: residual after the O projection (debug dump), or null
   bf16* attn;                      // [T, HQ]
   bf16* act;                       // [T, F]
@@ -76,6 +78,7 @@ struct MegaParams {
   BatchDesc b;
   KvGeom g;
   unsigned int* bar;               // phase counter, zero at launch
+  unsigned int* tile_cnt;          // [kMgMaxTiles] arrivals per tile of the projection in flight (zero at launch, self-resetting)
   unsigned long long* phase_ts;    // optional [8 L + 2] %globaltimer at the end of each phase in CTA 0 (tuning aid), or null
   TraceSlot tr;
 };
@@ -129,6 +132,7 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
   const uint32_t tmem_ptr_addr = tmem_empty + 16u;
   int* const nseg_tab = reinterpret_cast<int*>(gen_base + (bar_base - base) + 512);     // [4][kMgMaxTiles]
   float* const red = reinterpret_cast<float*>(gen_base + (bar_base - base) + 512 + 4 * kMgMaxTiles * 4);   // [4]
+  int* const red_i = reinterpret_cast<int*>(red + 8);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int G = (int)gridDim.x, cta = (int)blockIdx.x;
@@ -196,7 +200,7 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
           const long long u0 = mg_u0(U, G, cta), u1 = mg_u0(U, G, cta + 1);
           if (u0 < u1) {
             // the activation is complete when the phase before this projection has been arrived at by every CTA
-            const int phase = l * kMgPhasesPerLayer + 2 * gi + 1;
+            const int phase = l * kMgPhasesPerLayer + (gi == 3 ? 6 : 2 * gi + 1);      // phases completed before this projection may read X
             mg_wait_count(p.bar, (unsigned)G * (unsigned)phase);
             asm volatile("fence.proxy.async;" ::: "memory");      // generic-proxy writes of other CTAs -> TMA (async proxy) reads
           }
@@ -268,8 +272,99 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
       mg_bar128();
     };
 
+    // ---- finish one 128-column tile (= one head) of the QKV projection: sum its slices, RoPE, write Q / the K,V page rows ----
+    auto finish_qkv = [&](int tile, int ns, int layer) {
+      const int col0 = tile * 128, Hkv = p.g.n_kv_heads, H = p.n_heads;
+      const int kind = col0 < p.HQ ? 0 : (col0 < p.HQ + Hkv * 128 ? 1 : 2);          // Q head | K head | V head
+      const int head = kind == 0 ? tile : (kind == 1 ? tile - H : tile - H - Hkv);
+      const long long stq = (long long)T * p.NQKV;
+      for (int i0 = tid; i0 < T * 16; i0 += 4 * 128) {        // item = (token, pair indices e .. e + 3 of [0, 64)); 4 items per pass
+        float4 lo[4][kMgMaxSegQkv], hi[4][kMgMaxSegQkv], cs[4], sn[4];
+        int pos[4], bi_[4];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {                         // every load of the pass first
+          const int i = i0 + m * 128;
+          const bool ok = i < T * 16;
+          const int t = ok ? i >> 4 : 0, e = (i & 15) * 4;
+          const float* src = p.part_a + (long long)t * p.NQKV + col0 + e;
+#pragma unroll
+          for (int s = 0; s < kMgMaxSegQkv; ++s) {
+            lo[m][s] = (ok && s < ns) ? __ldcg(reinterpret_cast<const float4*>(src + s * stq)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            hi[m][s] = (ok && s < ns) ? __ldcg(reinterpret_cast<const float4*>(src + s * stq + 64)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+          const int bi = p.b.tok_bi[t];
+          bi_[m] = bi;
+          pos[m] = p.b.q_pos0[bi] + (t - p.b.q_off[bi]);
+          cs[m] = *reinterpret_cast<const float4*>(p.rope_cos + (long long)pos[m] * 64 + e);
+          sn[m] = *reinterpret_cast<const float4*>(p.rope_sin + (long long)pos[m] * 64 + e);
+        }
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+          const int i = i0 + m * 128;
+          if (i >= T * 16) continue;
+          const int t = i >> 4, e = (i & 15) * 4;
+          float4 a = lo[m][0], c = hi[m][0];
+#pragma unroll
+          for (int s = 1; s < kMgMaxSegQkv; ++s) {
+            a.x += lo[m][s].x; a.y += lo[m][s].y; a.z += lo[m][s].z; a.w += lo[m][s].w;
+            c.x += hi[m][s].x; c.y += hi[m][s].y; c.z += hi[m][s].z; c.w += hi[m][s].w;
+          }
+          if (kind < 2) {                                     // rotate the pairs (e, e + 64) by the token's absolute position
+            const float4 a2 = make_float4(a.x * cs[m].x - c.x * sn[m].x, a.y * cs[m].y - c.y * sn[m].y, a.z * cs[m].z - c.z * sn[m].z, a.w * cs[m].w - c.w * sn[m].w);
+            c = make_float4(c.x * cs[m].x + a.x * sn[m].x, c.y * cs[m].y + a.y * sn[m].y, c.z * cs[m].z + a.z * sn[m].z, c.w * cs[m].w + a.w * sn[m].w);
+            a = a2;
+          }
+          bf16* dst;
+          if (kind == 0) {
+            dst = p.q + ((long long)t * H + head) * 128 + e;
+          } else {
+            const int page = p.page_table[(long long)p.b.slot[bi_[m]] * p.g.max_pages_per_req + pos[m] / p.g.page_tokens];
+            dst = p.kv_store + p.g.offset(layer, page, kind - 1, head, pos[m] % p.g.page_tokens) + e;
+          }
+          __stcg(reinterpret_cast<uint2*>(dst), make_uint2(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w)));
+          __stcg(reinterpret_cast<uint2*>(dst + 64), make_uint2(pack_bf16(c.x, c.y), pack_bf16(c.z, c.w)));
+        }
+      }
+    };
+
+    // ---- finish one gate/up tile (64 features): act[t, f] = bf16(silu(sum gate slices) * sum up slices) ----
+    auto finish_gu = [&](int tile, int ns) {
+      const int ld = 2 * p.F;
+      const long long st = (long long)T * ld;
+      for (int i0 = tid; i0 < T * 16; i0 += 4 * 128) {        // item = (token, features j .. j + 3 of the tile's 64)
+        float4 ga[4][kMgMaxSegGu], ua[4][kMgMaxSegGu];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+          const int i = i0 + m * 128;
+          const bool ok = i < T * 16;
+          const int t = ok ? i >> 4 : 0, j = (i & 15) * 4;
+          const float* gp = p.part_a + (long long)t * ld + tile * 128 + j;
+#pragma unroll
+          for (int s = 0; s < kMgMaxSegGu; ++s) {
+            ga[m][s] = (ok && s < ns) ? __ldcg(reinterpret_cast<const float4*>(gp + s * st)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            ua[m][s] = (ok && s < ns) ? __ldcg(reinterpret_cast<const float4*>(gp + s * st + 64)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+        }
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+          const int i = i0 + m * 128;
+          if (i >= T * 16) continue;
+          const int t = i >> 4, j = (i & 15) * 4;
+          float4 g = ga[m][0], w = ua[m][0];
+#pragma unroll
+          for (int s = 1; s < kMgMaxSegGu; ++s) {
+            g.x += ga[m][s].x; g.y += ga[m][s].y; g.z += ga[m][s].z; g.w += ga[m][s].w;
+            w.x += ua[m][s].x; w.y += ua[m][s].y; w.z += ua[m][s].z; w.w += ua[m][s].w;
+          }
+          uint2 o;
+          o.x = pack_bf16(silu_f(g.x) * w.x, silu_f(g.y) * w.y); o.y = pack_bf16(silu_f(g.z) * w.z, silu_f(g.w) * w.w);
+          __stcg(reinterpret_cast<uint2*>(p.act + (long long)t * p.F + tile * 64 + j), o);
+        }
+      }
+    };
+
     // ---- GEMM epilogue: this CTA's segments of projection gi -> fp32 slices ----
-    auto gemm_epilogue = [&](int gi, float* part, int ld) {
+    auto gemm_epilogue = [&](int gi, float* part, int ld, const int* nseg, int layer) {
       const long long U = (long long)gm[gi].n_tiles * gm[gi].kbt;
       const long long u0 = mg_u0(U, G, cta), u1 = mg_u0(U, G, cta + 1);
       for (long long un = u0; un < u1;) {
@@ -295,6 +390,20 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
         ptx::tc_fence_before();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(tmem_empty + 8u * acc);
+        if (gi == 0 || gi == 2) {
+          // the CTA that completes a tile (the last of its <= 3 runs to arrive) finishes it: sums the slices in slice order and
+          // applies RoPE + the Q / K/V-page write (QKV) or SwiGLU (gate/up).  This runs under the other CTAs' streaming
+          // instead of in a phase of its own.
+          __threadfence();
+          mg_bar128();
+          if (tid == 0) red_i[0] = (int)atomicAdd(p.tile_cnt + tile, 1u);
+          mg_bar128();
+          if (red_i[0] == nseg[tile] - 1) {
+            if (tid == 0) p.tile_cnt[tile] = 0;           // every run of the tile has arrived: ready for the next layer
+            __threadfence();
+            if (gi == 0) finish_qkv(tile, nseg[tile], layer); else finish_gu(tile, nseg[tile]);
+          }
+        }
         un += n;
         ++it;
       }
@@ -312,21 +421,42 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           const int i = tid + k * 128;
-          if (i < nvec) {
-            float4 a = __ldcg(xr + i);
-            if (have_part) {
-              const int ns = nseg[(i * 4) >> 7];
-              const float4* pr = reinterpret_cast<const float4*>(p.part_x + (long long)t * p.d) + i;
-              const long long st4 = ((long long)T * p.d) >> 2;
-              for (int s = 0; s < ns; ++s) {
-                const float4 q = __ldcg(pr + s * st4);
-                a.x += q.x; a.y += q.y; a.z += q.z; a.w += q.w;
-              }
-              __stcg(xr + i, a);
+          v[k] = i < nvec ? __ldcg(xr + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        if (have_part) {
+          // every slice load of four chunks is issued before the first add (independent loads: one L2 round trip per half
+          // instead of one per slice); slices past a tile's count are not read and add an exact zero, order = slice order
+          const float4* pr = reinterpret_cast<const float4*>(p.part_x + (long long)t * p.d);
+          const long long st4 = ((long long)T * p.d) >> 2;
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            float4 q[4][kMgMaxSeg];
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+              const int i = tid + (h * 4 + kk) * 128;
+              const int ns = i < nvec ? nseg[i >> 5] : 0;
+#pragma unroll
+              for (int s = 0; s < kMgMaxSeg; ++s) q[kk][s] = s < ns ? __ldcg(pr + s * st4 + i) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
-            if (copy_to) reinterpret_cast<float4*>(copy_to + (long long)t * p.d)[i] = a;
-            v[k] = a;
-            ss += a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w;
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+              float4& a = v[h * 4 + kk];
+#pragma unroll
+              for (int s = 0; s < kMgMaxSeg; ++s) { a.x += q[kk][s].x; a.y += q[kk][s].y; a.z += q[kk][s].z; a.w += q[kk][s].w; }
+            }
+          }
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const int i = tid + k * 128;
+            if (i < nvec) __stcg(xr + i, v[k]);
+          }
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int i = tid + k * 128;
+          if (i < nvec) {
+            if (copy_to) reinterpret_cast<float4*>(copy_to + (long long)t * p.d)[i] = v[k];
+            ss += v[k].x * v[k].x + v[k].y * v[k].y + v[k].z * v[k].z + v[k].w * v[k].w;
           }
         }
         if (!uo) continue;                             // final fold: only x is wanted
@@ -349,103 +479,26 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
       arrive();
     };
 
-    // ---- SwiGLU: act[t, f] = bf16(silu(sum gate slices) * sum up slices); slice layout [seg][T][tile * 128 + {gate 0..63 | up 64..127}] ----
-    auto swiglu = [&](const int* nseg) {
-      wait_prev();
-      const int ld = 2 * p.F;
-      const int f4 = p.F >> 2;                          // float4 groups per row (a group never straddles a 64-feature tile)
-      const long long st = (long long)T * ld;
-      for (int i = cta * 128 + tid; i < T * f4; i += G * 128) {
-        const int t = i / f4, f = (i - t * f4) * 4, tile = f >> 6, j = f & 63;
-        const float* gp = p.part_a + (long long)t * ld + tile * 128 + j;
-        float4 g = make_float4(0.f, 0.f, 0.f, 0.f), w = g;
-        const int ns = nseg[tile];
-        for (int s = 0; s < ns; ++s) {
-          const float4 a = __ldcg(reinterpret_cast<const float4*>(gp + s * st)), c = __ldcg(reinterpret_cast<const float4*>(gp + s * st + 64));
-          g.x += a.x; g.y += a.y; g.z += a.z; g.w += a.w;
-          w.x += c.x; w.y += c.y; w.z += c.z; w.w += c.w;
-        }
-        uint2 o;
-        o.x = pack_bf16(silu_f(g.x) * w.x, silu_f(g.y) * w.y); o.y = pack_bf16(silu_f(g.z) * w.z, silu_f(g.w) * w.w);
-        __stcg(reinterpret_cast<uint2*>(p.act + (long long)t * p.F + f), o);
-      }
-      arrive();
-    };
-
     // ---- attention phase of layer l: units (request, KV head) ----
-    auto attention = [&](int l, const int* nseg_qkv) {
+    auto attention = [&](int l) {
       wait_prev();
       const int H = p.n_heads, Hkv = p.g.n_kv_heads, r = H / Hkv;
       // scratch = the X ring (idle during this phase: this CTA's X producer cannot pass the phase counter before the CTA
       // arrives) followed by the own scratch, contiguous: Q [64 rows][256 B] 16 KB, K 2 x 16 KB, V 2 x 16 KB
       const uint32_t sQ = sX, bK = sX + 16384, bV = sX + 16384 + 32768;
-      const long long stq = (long long)T * p.NQKV;          // slice stride of part_a
       for (int unit = cta; unit < p.b.n * Hkv; unit += G) {
         const int bi = unit / Hkv, kvh = unit % Hkv;
         const int q_len = p.b.q_len[bi];
         if (q_len <= 0) continue;
-        const int n_rows = q_len * r, S = p.b.kv_len[bi], q_off = p.b.q_off[bi], pos0 = p.b.q_pos0[bi];
+        const int n_rows = q_len * r, S = p.b.kv_len[bi], q_off = p.b.q_off[bi];
         const int* pt = p.page_table + (long long)p.b.slot[bi] * p.g.max_pages_per_req;
-        // -- (a) Q rows: sum the slices, rotate, bf16 into sQ; rows past n_rows: zeros
-        for (int i = tid; i < 64 * 16; i += 128) {          // item = (stacked row, group of 4 pair indices e..e+3 in [0, 64))
-          const int rho = i >> 4, e = (i & 15) * 4;
-          float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
-          if (rho < n_rows) {
-            const int tok = rho / r, h = kvh * r + rho % r;
-            const float* src = p.part_a + (long long)(q_off + tok) * p.NQKV + h * 128 + e;
-            const int ns = nseg_qkv[h];
-            for (int s = 0; s < ns; ++s) {
-              const float4 a = __ldcg(reinterpret_cast<const float4*>(src + s * stq)), c = __ldcg(reinterpret_cast<const float4*>(src + s * stq + 64));
-              lo.x += a.x; lo.y += a.y; lo.z += a.z; lo.w += a.w;
-              hi.x += c.x; hi.y += c.y; hi.z += c.z; hi.w += c.w;
-            }
-            const float4 cs = *reinterpret_cast<const float4*>(p.rope_cos + (long long)(pos0 + tok) * 64 + e);
-            const float4 sn = *reinterpret_cast<const float4*>(p.rope_sin + (long long)(pos0 + tok) * 64 + e);
-            const float4 l2 = make_float4(lo.x * cs.x - hi.x * sn.x, lo.y * cs.y - hi.y * sn.y, lo.z * cs.z - hi.z * sn.z, lo.w * cs.w - hi.w * sn.w);
-            hi = make_float4(hi.x * cs.x + lo.x * sn.x, hi.y * cs.y + lo.y * sn.y, hi.z * cs.z + lo.z * sn.z, hi.w * cs.w + lo.w * sn.w);
-            lo = l2;
-            if (p.q_dump) {
-              bf16* qd = p.q_dump + ((long long)(q_off + tok) * H + h) * 128 + e;
-              *reinterpret_cast<uint2*>(qd) = make_uint2(pack_bf16(lo.x, lo.y), pack_bf16(lo.z, lo.w));
-              *reinterpret_cast<uint2*>(qd + 64) = make_uint2(pack_bf16(hi.x, hi.y), pack_bf16(hi.z, hi.w));
-            }
-          }
-          const uint32_t a0 = sQ + tile_off(rho, e >> 3) + (e & 7) * 2, a1 = sQ + tile_off(rho, 8 + (e >> 3)) + (e & 7) * 2;
-          asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a0), "r"(pack_bf16(lo.x, lo.y)), "r"(pack_bf16(lo.z, lo.w)) : "memory");
-          asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a1), "r"(pack_bf16(hi.x, hi.y)), "r"(pack_bf16(hi.z, hi.w)) : "memory");
+        // -- Q tile: the rows the QKV projection's finishing CTAs wrote (bf16, rotated); rows past n_rows: zeros
+        for (int i = tid; i < 64 * 16; i += 128) {
+          const int rho = i >> 4, ch = i & 15;
+          const bool ok = rho < n_rows;
+          const int tok = ok ? rho / r : 0, hh = ok ? rho % r : 0;
+          cp_async16(sQ + tile_off(rho, ch), p.q + ((long long)(q_off + tok) * H + kvh * r + hh) * 128 + ch * 8, ok);
         }
-        // -- (b) fresh K (rotated) and V of the computed tokens -> the request's pages
-        const int kcol = p.HQ + kvh * 128, vcol = p.HQ + Hkv * 128 + kvh * 128;
-        const int ns_k = nseg_qkv[kcol >> 7], ns_v = nseg_qkv[vcol >> 7];
-        for (int i = tid; i < q_len * 16; i += 128) {
-          const int tok = i >> 4, e = (i & 15) * 4, pos = pos0 + tok;
-          const float* ks = p.part_a + (long long)(q_off + tok) * p.NQKV + kcol + e;
-          const float* vs = p.part_a + (long long)(q_off + tok) * p.NQKV + vcol + e;
-          float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo, v0 = lo, v1 = lo;
-          for (int s = 0; s < ns_k; ++s) {
-            const float4 a = __ldcg(reinterpret_cast<const float4*>(ks + s * stq)), c = __ldcg(reinterpret_cast<const float4*>(ks + s * stq + 64));
-            lo.x += a.x; lo.y += a.y; lo.z += a.z; lo.w += a.w;
-            hi.x += c.x; hi.y += c.y; hi.z += c.z; hi.w += c.w;
-          }
-          for (int s = 0; s < ns_v; ++s) {
-            const float4 a = __ldcg(reinterpret_cast<const float4*>(vs + s * stq)), c = __ldcg(reinterpret_cast<const float4*>(vs + s * stq + 64));
-            v0.x += a.x; v0.y += a.y; v0.z += a.z; v0.w += a.w;
-            v1.x += c.x; v1.y += c.y; v1.z += c.z; v1.w += c.w;
-          }
-          const float4 cs = *reinterpret_cast<const float4*>(p.rope_cos + (long long)pos * 64 + e);
-          const float4 sn = *reinterpret_cast<const float4*>(p.rope_sin + (long long)pos * 64 + e);
-          const float4 l2 = make_float4(lo.x * cs.x - hi.x * sn.x, lo.y * cs.y - hi.y * sn.y, lo.z * cs.z - hi.z * sn.z, lo.w * cs.w - hi.w * sn.w);
-          hi = make_float4(hi.x * cs.x + lo.x * sn.x, hi.y * cs.y + lo.y * sn.y, hi.z * cs.z + lo.z * sn.z, hi.w * cs.w + lo.w * sn.w);
-          const int page = pt[pos / p.g.page_tokens];
-          bf16* kd = p.kv_store + p.g.offset(l, page, 0, kvh, pos % p.g.page_tokens) + e;
-          bf16* vd = p.kv_store + p.g.offset(l, page, 1, kvh, pos % p.g.page_tokens) + e;
-          *reinterpret_cast<uint2*>(kd) = make_uint2(pack_bf16(l2.x, l2.y), pack_bf16(l2.z, l2.w));
-          *reinterpret_cast<uint2*>(kd + 64) = make_uint2(pack_bf16(hi.x, hi.y), pack_bf16(hi.z, hi.w));
-          *reinterpret_cast<uint2*>(vd) = make_uint2(pack_bf16(v0.x, v0.y), pack_bf16(v0.z, v0.w));
-          *reinterpret_cast<uint2*>(vd + 64) = make_uint2(pack_bf16(v1.x, v1.y), pack_bf16(v1.z, v1.w));
-        }
-        __threadfence_block();
-        mg_bar128();                                        // Q tile complete; the fresh K/V rows are visible to this CTA's loads
         // -- (c) flash loop over the request's K/V pages (64-token tiles, double-buffered cp.async); warp w owns rows 16 w .. 16 w + 15
         auto load_kv = [&](int tile, int buf) {
           const int j0 = tile * kFaBN;
@@ -564,14 +617,13 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
 
     const int* ns_qkv = nseg_tab, *ns_o = nseg_tab + kMgMaxTiles, *ns_gu = nseg_tab + 2 * kMgMaxTiles, *ns_dn = nseg_tab + 3 * kMgMaxTiles;
     for (int l = 0; l < L; ++l) {
-      fold_norm(ns_dn, l > 0, p.u, nullptr);                // phase 8 l + 0 (the launch's first layer finds x complete)
-      gemm_epilogue(0, p.part_a, p.NQKV);                   //             1
-      attention(p.layer0 + l, ns_qkv);                      //             2
-      gemm_epilogue(1, p.part_x, p.d);                      //             3
+      fold_norm(ns_dn, l > 0, p.u, nullptr);                // phase 7 l + 0 (the launch's first layer finds x complete)
+      gemm_epilogue(0, p.part_a, p.NQKV, ns_qkv, p.layer0 + l);   //   1  (+ RoPE, Q and K/V page write by each tile's last CTA)
+      attention(p.layer0 + l);                              //             2
+      gemm_epilogue(1, p.part_x, p.d, ns_o, 0);             //             3
       fold_norm(ns_o, true, p.u2, p.xmid_dump);             //             4
-      gemm_epilogue(2, p.part_a, 2 * p.F);                  //             5
-      swiglu(ns_gu);                                        //             6
-      gemm_epilogue(3, p.part_x, p.d);                      //             7
+      gemm_epilogue(2, p.part_a, 2 * p.F, ns_gu, 0);        //             5  (+ SwiGLU by each tile's last CTA)
+      gemm_epilogue(3, p.part_x, p.d, ns_dn, 0);            //             6
     }
     fold_norm(ns_dn, true, nullptr, nullptr);               // the last layer's down slices into x (the head normalises its own rows)
   }

@@ -934,3 +934,38 @@ def test_debug_tensor_k_v_rows_and_feature_capacity():
     ok = eng.refresh_step([big], dry_run=True)                       # without the features the request is fine
     assert ok.total >= 1
     eng.close()
+
+
+def test_layer_kernel_option_matches_oracle_and_its_own_dump_mode():
+    """DLM_OPT_LAYER_KERNEL (whole-stack persistent kernel, off by default): a cached step of 32 and of 64 tokens through it
+    agrees with the oracle like the per-stage kernels do, its debug-dump mode (one layer per launch) is bit-identical to the
+    single launch, and dlm_last_step_kernels reports it."""
+    pkg = _pkg()
+    a = _reduced(ARCH_LLADA8B, 2)
+    seed = WEIGHT_SEED["C2"]
+    rng = np.random.default_rng(77)
+    specs = [(random_tokens(rng, 150, a.vocab, a.mask_id), 64, 32, 0.9), (random_tokens(rng, 70, a.vocab, a.mask_id), 64, 32, 0.5)]
+    wts = ow.Weights(a, seed, keep_f64=True)
+    for n in (1, 2):
+        outs = {}
+        for mode in ("single", "dump", "per_stage"):
+            eng = pkg.Engine(a, seed, max_requests=2, max_seq=256, max_block=32)
+            eng.set_option(pkg.OPT_LAYER_KERNEL, 0 if mode == "per_stage" else 1)
+            eng.set_option(pkg.OPT_DEBUG_DUMP, 1 if mode == "dump" else 0)
+            ids = [eng.add_request(*s) for s in specs[:n]]
+            eng.refresh_step(ids, dry_run=True)
+            g = [eng.cached_step(ids, dry_run=True) for _ in range(3)][-1]          # eager, captured, replayed
+            assert bool(eng.last_step_kernels() & pkg.PATH_LAYER_KERNEL) == (mode != "per_stage")
+            outs[mode] = g
+            eng.close()
+        assert np.array_equal(outs["single"].lse, outs["dump"].lse) and outs["single"].commits == outs["dump"].commits
+        assert np.allclose(outs["single"].lse, outs["per_stage"].lse, rtol=0, atol=1e-1)
+        for j, s in enumerate(specs[:n]):
+            oreq = ostep.Request(a, s[0], s[1], s[2], s[3])
+            ostep.refresh_step(oreq, wts, dry_run=True)
+            o = ostep.cached_step(oreq, wts, dry_run=True)
+            g = outs["single"]
+            assert np.abs(g.lse[j][:32] - o.lse).max() <= 2e-2 * np.abs(o.lse).max()
+            assert np.abs(g.row_conf[j][:32] - o.conf).max() < CONF_ERR_MAX
+            clear = o.margin >= 5e-2
+            assert np.array_equal(g.row_tok[j][:32][clear], o.tok[clear])
