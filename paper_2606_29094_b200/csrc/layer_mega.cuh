@@ -41,6 +41,7 @@
 #include "common.cuh"
 #include "kernels_basic.cuh"
 #include "ptx_sm100.cuh"
+#include "qkv_finish.cuh"
 
 namespace dlm {
 
@@ -272,60 +273,12 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
       mg_bar128();
     };
 
-    // ---- finish one 128-column tile (= one head) of the QKV projection: sum its slices, RoPE, write Q / the K,V page rows ----
-    auto finish_qkv = [&](int tile, int ns, int layer) {
-      const int col0 = tile * 128, Hkv = p.g.n_kv_heads, H = p.n_heads;
-      const int kind = col0 < p.HQ ? 0 : (col0 < p.HQ + Hkv * 128 ? 1 : 2);          // Q head | K head | V head
-      const int head = kind == 0 ? tile : (kind == 1 ? tile - H : tile - H - Hkv);
-      const long long stq = (long long)T * p.NQKV;
-      for (int i0 = tid; i0 < T * 16; i0 += 4 * 128) {        // item = (token, pair indices e .. e + 3 of [0, 64)); 4 items per pass
-        float4 lo[4][kMgMaxSegQkv], hi[4][kMgMaxSegQkv], cs[4], sn[4];
-        int pos[4], bi_[4];
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {                         // every load of the pass first
-          const int i = i0 + m * 128;
-          const bool ok = i < T * 16;
-          const int t = ok ? i >> 4 : 0, e = (i & 15) * 4;
-          const float* src = p.part_a + (long long)t * p.NQKV + col0 + e;
-#pragma unroll
-          for (int s = 0; s < kMgMaxSegQkv; ++s) {
-            lo[m][s] = (ok && s < ns) ? __ldcg(reinterpret_cast<const float4*>(src + s * stq)) : make_float4(0.f, 0.f, 0.f, 0.f);
-            hi[m][s] = (ok && s < ns) ? __ldcg(reinterpret_cast<const float4*>(src + s * stq + 64)) : make_float4(0.f, 0.f, 0.f, 0.f);
-          }
-          const int bi = p.b.tok_bi[t];
-          bi_[m] = bi;
-          pos[m] = p.b.q_pos0[bi] + (t - p.b.q_off[bi]);
-          cs[m] = *reinterpret_cast<const float4*>(p.rope_cos + (long long)pos[m] * 64 + e);
-          sn[m] = *reinterpret_cast<const float4*>(p.rope_sin + (long long)pos[m] * 64 + e);
-        }
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {
-          const int i = i0 + m * 128;
-          if (i >= T * 16) continue;
-          const int t = i >> 4, e = (i & 15) * 4;
-          float4 a = lo[m][0], c = hi[m][0];
-#pragma unroll
-          for (int s = 1; s < kMgMaxSegQkv; ++s) {
-            a.x += lo[m][s].x; a.y += lo[m][s].y; a.z += lo[m][s].z; a.w += lo[m][s].w;
-            c.x += hi[m][s].x; c.y += hi[m][s].y; c.z += hi[m][s].z; c.w += hi[m][s].w;
-          }
-          if (kind < 2) {                                     // rotate the pairs (e, e + 64) by the token's absolute position
-            const float4 a2 = make_float4(a.x * cs[m].x - c.x * sn[m].x, a.y * cs[m].y - c.y * sn[m].y, a.z * cs[m].z - c.z * sn[m].z, a.w * cs[m].w - c.w * sn[m].w);
-            c = make_float4(c.x * cs[m].x + a.x * sn[m].x, c.y * cs[m].y + a.y * sn[m].y, c.z * cs[m].z + a.z * sn[m].z, c.w * cs[m].w + a.w * sn[m].w);
-            a = a2;
-          }
-          bf16* dst;
-          if (kind == 0) {
-            dst = p.q + ((long long)t * H + head) * 128 + e;
-          } else {
-            const int page = p.page_table[(long long)p.b.slot[bi_[m]] * p.g.max_pages_per_req + pos[m] / p.g.page_tokens];
-            dst = p.kv_store + p.g.offset(layer, page, kind - 1, head, pos[m] % p.g.page_tokens) + e;
-          }
-          __stcg(reinterpret_cast<uint2*>(dst), make_uint2(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w)));
-          __stcg(reinterpret_cast<uint2*>(dst + 64), make_uint2(pack_bf16(c.x, c.y), pack_bf16(c.z, c.w)));
-        }
-      }
-    };
+    // ---- finish one 128-column tile (= one head) of the QKV projection: qkv_finish.cuh ----
+    QkvFinish qf_;
+    qf_.part = p.part_a; qf_.slice_stride = (long long)T * p.NQKV; qf_.ld = p.NQKV; qf_.T = T; qf_.HQ = p.HQ; qf_.n_heads = p.n_heads;
+    qf_.q = p.q; qf_.kv_store = p.kv_store; qf_.rope_cos = p.rope_cos; qf_.rope_sin = p.rope_sin; qf_.page_table = p.page_table;
+    qf_.b = p.b; qf_.g = p.g; qf_.tile_cnt = p.tile_cnt;
+    auto finish_qkv = [&](int tile, int ns, int layer) { qkv_finish_tile<kMgMaxSegQkv>(qf_, tile, ns, layer, tid); };
 
     // ---- finish one gate/up tile (64 features): act[t, f] = bf16(silu(sum gate slices) * sum up slices) ----
     auto finish_gu = [&](int tile, int ns) {
