@@ -436,6 +436,8 @@ def main():
     ap.add_argument("--cost-table", action="store_true", help="print dlm_profile_step_costs for the workload's architecture")
     ap.add_argument("--two-call", action="store_true", help="mixed iterations as dlm_refresh_step + dlm_cached_step instead of one dlm_mixed_step")
     ap.add_argument("--tau", type=float, default=None, help="override every request's confidence threshold")
+    ap.add_argument("--trace-rows", type=int, default=0, help="add the first N launches of one traced step (begin / wait / end in us) to the JSON line")
+    ap.add_argument("--layer-kernel", action="store_true", help="run cached steps of <= 64 tokens through the whole-stack persistent kernel (DLM_OPT_LAYER_KERNEL) and report its phase times")
     ap.add_argument("--tau-sweep", action="store_true", help="add a sweep over the paper's candidate thresholds (P:123; BASELINE.json configs[4]: 0.5-0.95)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -464,6 +466,8 @@ def main():
     K, W = max(1, args.steps), max(3, args.warmup)
 
     run = Runner(pkg, arch, seed, specs, mixed_launch=not args.two_call)
+    if args.layer_kernel:
+        run.eng.set_option(pkg.OPT_LAYER_KERNEL, 1)
     for _ in range(W):
         run.step()
     # advance (untimed) to a block boundary: the timed region then opens with a block's recompute step and holds both step
@@ -523,6 +527,11 @@ def main():
     # ---- dominant kernel class, timed inside the production launch by the in-kernel trace ----
     if rank == 0 and not args.no_kernel_pass:
         out["roofline"], out["kernels"] = trace_pass(run, pkg, arch, peaks)
+    if rank == 0 and args.trace_rows > 0:
+        out["trace_rows"] = trace_rows(run, pkg, args.trace_rows)
+    if rank == 0 and args.layer_kernel:
+        out["layer_kernel_phases_us"] = layer_kernel_phases(run, pkg, arch)
+        out["config"]["layer_kernel"] = True
     if rank == 0 and args.tau_sweep:
         out["tau_sweep"] = tau_sweep(pkg, arch, seed, specs, not args.two_call)
     if rank == 0 and not args.no_cpu_baseline and world == 1:
@@ -558,6 +567,39 @@ def tau_sweep(pkg, arch, seed, specs, mixed_launch, taus=(0.5, 0.6, 0.7, 0.8, 0.
         run.close()
         rows.append({"tau": tau, "steps_per_s": steps / (us * 1e-6), "committed_tokens_per_s": cm / (us * 1e-6), "commits_per_step": cm / steps})
     return rows
+
+
+def trace_rows(run, pkg, n):
+    """The first n launches of one traced step of the workload's dominant kind: [class, begin_us, wait_us, end_us]."""
+    eng = run.eng
+    eng.set_option(pkg.OPT_TRACE, 1)
+    rows = []
+    for _ in range(40):
+        us, cm, nr, nc, work = run.step()
+        if len(run.specs) == 1 and nr:
+            continue
+        rows = eng.step_trace()
+        if rows:
+            break
+    eng.set_option(pkg.OPT_TRACE, 0)
+    return [[k, round(b, 2), round(w, 2), round(e, 2)] for k, b, w, e in rows[:n]]
+
+
+def layer_kernel_phases(run, pkg, arch):
+    """Mean duration (us) of each of the whole-stack kernel's 7 phases per layer in CTA 0 (first and last layer left out)."""
+    eng = run.eng
+    eng.set_option(pkg.OPT_LAYER_KERNEL_PHASE_TS, 1)
+    ph = None
+    for _ in range(40):
+        us, cm, nr, nc, work = run.step()
+        if not nr and eng.last_step_kernels() & pkg.PATH_LAYER_KERNEL:
+            ph = eng.layer_kernel_phases()
+    eng.set_option(pkg.OPT_LAYER_KERNEL_PHASE_TS, 0)
+    if ph is None or len(ph) < 7 * arch.n_layers + 1:
+        return None
+    d = np.diff(ph)[: 7 * arch.n_layers].reshape(arch.n_layers, 7)[1:-1]
+    names = ("qkv_gemm+rope", "attention", "o_gemm", "fold+norm", "gateup_gemm+swiglu", "down_gemm", "fold+norm(next layer)")
+    return {n: round(float(d[:, j].mean()), 2) for j, n in enumerate(names)} | {"layer_total": round(float(d.sum(1).mean()), 2)}
 
 
 def trace_pass(run, pkg, arch, peaks, n_steps=12):

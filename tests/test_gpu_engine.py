@@ -30,6 +30,10 @@ def _gpu_hidden_block_rows(pkg, eng, rid, arch, o, refresh):
     return x[o.block_lo:o.block_lo + len(o.conf)] if refresh else x
 
 
+# P-C stage S5 (gate/up + SwiGLU): beyond the one bf16 rounding of the output, the error of the fp32 tensor-memory accumulation
+# over K = 4096: measured 7.6e-6 (32 rows) .. 1.8e-5 (512 rows) absolute at max |act| 18 .. 21.5, i.e. <= 8.3e-7 of max |act|;
+# bound = ~2x that.  (Not silu_f's fast exponential: the fp32-output GEMM alone shows 1.6e-6 .. 5.2e-6 of max |out|.)
+S5_EXTRA = 2e-6
 CONF_ERR_MAX = 5e-2      # bound on |conf_gpu - conf_oracle| of the bf16 path (measured 5e-3 .. 1.6e-2, SURVEY 8(c) "Precision floor")
 
 
@@ -514,7 +518,7 @@ def test_stagewise_from_gpu_inputs():
             xm_o = x_in + attn @ wts.get(ow.layer_tid(l, ow.SUB_O)).T
             assert np.abs(xm_o - x_mid).max() <= 1e-4 * max(1.0, np.abs(xm_o).max())
             act_o = omodel.silu(u2 @ wts.get(ow.layer_tid(l, ow.SUB_G)).T) * (u2 @ wts.get(ow.layer_tid(l, ow.SUB_U)).T)
-            assert bf(act_o, act, 2e-4)       # fp32 tensor-core accumulation over K = 4096, then one bf16 rounding
+            assert bf(act_o, act, S5_EXTRA * np.abs(act_o).max())
             xo_o = x_mid + act @ wts.get(ow.layer_tid(l, ow.SUB_D)).T
             assert np.abs(xo_o - x_out).max() <= 1e-4 * max(1.0, np.abs(xo_o).max())
     # S7: LM head from the GPU's final-normed rows
@@ -621,7 +625,7 @@ def test_c2_full_size_sampled_stages_and_properties():
         xm_o = x_in[rows] + attn[rows] @ wts.get(ow.layer_tid(l, ow.SUB_O)).T
         assert np.abs(xm_o - x_mid[rows]).max() <= 1e-4 * max(1.0, np.abs(xm_o).max())
         act_o = omodel.silu(u2[rows] @ wts.get(ow.layer_tid(l, ow.SUB_G)).T) * (u2[rows] @ wts.get(ow.layer_tid(l, ow.SUB_U)).T)
-        assert bf(act_o, act[rows], 3e-4)
+        assert bf(act_o, act[rows], S5_EXTRA * np.abs(act_o).max())
         xo_o = x_mid[rows] + act[rows] @ wts.get(ow.layer_tid(l, ow.SUB_D)).T
         assert np.abs(xo_o - x_out[rows]).max() <= 1e-4 * max(1.0, np.abs(xo_o).max())
     # LM head over the FULL vocabulary for the block rows, from the GPU's final-normed rows
@@ -654,7 +658,7 @@ def test_c2_full_size_sampled_stages_and_properties():
         xm_o = x_in + attn @ wts.get(ow.layer_tid(l, ow.SUB_O)).T
         assert np.abs(xm_o - x_mid).max() <= 1e-4 * max(1.0, np.abs(xm_o).max())
         act_o = omodel.silu(u2 @ wts.get(ow.layer_tid(l, ow.SUB_G)).T) * (u2 @ wts.get(ow.layer_tid(l, ow.SUB_U)).T)
-        assert bf(act_o, act, 3e-4)
+        assert bf(act_o, act, S5_EXTRA * np.abs(act_o).max())
         xo_o = x_mid + act @ wts.get(ow.layer_tid(l, ow.SUB_D)).T
         assert np.abs(xo_o - x_out).max() <= 1e-4 * max(1.0, np.abs(xo_o).max())
     eng.set_option(pkg.OPT_DEBUG_DUMP, 0)

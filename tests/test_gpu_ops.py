@@ -9,6 +9,10 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 
+# fp32 accumulation in tensor memory over K <= 12 288: measured max |error| 1.5e-6 .. 5.2e-6 of max |out| on B200
+# (K = 4096 / 12 288, 32 and 512 rows); the bound is twice the largest value measured.
+GEMM_TOL = 1e-5
+
 def _bf16(x):
     return torch.from_numpy(x).to(torch.bfloat16)
 
@@ -34,7 +38,7 @@ def test_gemm_tc_store_and_residual(M, N, K, bn):
     A, a = _mk(rng, M, K)
     W, w = _mk(rng, N, K, 0.05)
     want = a @ w.T
-    tol = 2e-5 * np.sqrt(K) * np.abs(a).max() * np.abs(w).max() + 1e-6
+    tol = GEMM_TOL * np.abs(want).max() + 1e-6
     got = pkg.op_gemm_bf16(A, W, pkg.EPI_F32, bn)
     torch.cuda.synchronize()
     assert np.abs(_f64(got) - want).max() <= tol
@@ -78,7 +82,7 @@ def test_gemm_pair_store_and_residual(M, N, K, bn):
     A, a = _mk(rng, M, K)
     W, w = _mk(rng, N, K, 0.05)
     want = a @ w.T
-    tol = 2e-5 * np.sqrt(K) * np.abs(a).max() * np.abs(w).max() + 1e-6
+    tol = GEMM_TOL * np.abs(want).max() + 1e-6
     got = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_F32, bn)
     torch.cuda.synchronize()
     assert np.abs(_f64(got) - want).max() <= tol
@@ -101,7 +105,7 @@ def test_gemm_pair_split_k(M, N, K, splits):
     A, a = _mk(rng, M, K)
     W, w = _mk(rng, N, K, 0.05)
     want = a @ w.T
-    tol = 2e-5 * np.sqrt(K) * np.abs(a).max() * np.abs(w).max() + 1e-6
+    tol = GEMM_TOL * np.abs(want).max() + 1e-6
     got, ns = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_F32, 0 if splits == 0 else 256, splits=splits, return_splits=True)
     torch.cuda.synchronize()
     assert 1 <= ns <= 4 and (splits == 0 or ns <= splits)
@@ -135,7 +139,7 @@ def test_gemm_skinny_partial(T, N, K, splits):
     X, x = _mk(rng, T, K)
     W, w = _mk(rng, N, K, 0.05)
     want = x @ w.T
-    tol = 2e-5 * np.sqrt(K) * np.abs(x).max() * np.abs(w).max() + 1e-6
+    tol = GEMM_TOL * np.abs(want).max() + 1e-6
     got, ns = pkg.op_gemm_skinny_bf16(X, W, pkg.EPI_F32, splits)
     torch.cuda.synchronize()
     assert 1 <= ns <= 16 and (splits in (0,) or ns <= splits)
