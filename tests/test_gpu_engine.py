@@ -973,3 +973,40 @@ def test_layer_kernel_option_matches_oracle_and_its_own_dump_mode():
             assert np.abs(g.row_conf[j][:32] - o.conf).max() < CONF_ERR_MAX
             clear = o.margin >= 5e-2
             assert np.array_equal(g.row_tok[j][:32][clear], o.tok[clear])
+
+
+@pytest.mark.parametrize("bf16_model", [False, True])
+def test_finished_and_single_row_requests_in_a_batch(bf16_model):
+    """Degenerate batch members: a FINISHED request (computes nothing, commits 0) and a request with one-token blocks share a
+    batch with an ordinary request; the ordinary request's result is what it gets alone, in every step kind, and a batch made
+    only of finished requests is legal and empty."""
+    pkg = _pkg()
+    a = ARCH_C1.replace(weight_dtype=1) if bf16_model else ARCH_C1
+    rng = np.random.default_rng(19)
+    eng = pkg.Engine(a, WEIGHT_SEED["C1"], max_requests=3, max_seq=128, max_block=32)
+    done = eng.add_request(random_tokens(rng, 20, a.vocab, a.mask_id), 32, 32, 0.0)
+    eng.refresh_step([done])                                   # tau = 0: the whole (only) block in one step
+    assert eng.info(done)["n_masked"] == 0
+    one = eng.add_request(random_tokens(rng, 7, a.vocab, a.mask_id), 3, 1, 0.9)       # blocks of a single position
+    live = eng.add_request(random_tokens(rng, 50, a.vocab, a.mask_id), 64, 32, 0.9)
+    solo_r = eng.refresh_step([live], dry_run=True)
+    solo_c = eng.cached_step([live], dry_run=True)
+    eng.refresh_step([one], dry_run=True)
+    for order in ([done, live, one], [one, done, live]):
+        j = order.index(live)
+        for kind, solo in (("refresh", solo_r), ("cached", solo_c), ("mixed", solo_c)):
+            g = getattr(eng, kind + "_step")(order, dry_run=True)
+            assert g.n_committed[order.index(done)] == 0 and g.n_committed[order.index(one)] == 1
+            if bf16_model:          # the batch's token count changes the GEMM tiling: fp32 summation order only
+                assert np.allclose(g.lse[j], solo.lse[0], rtol=2e-3, atol=2e-3)
+            else:
+                assert g.commits[j] == solo.commits[0] and np.allclose(g.lse[j], solo.lse[0], rtol=1e-5, atol=1e-5)
+    g = eng.mixed_step([done])
+    assert g.total == 0 and g.n_masked_left[0] == 0
+    steps = 0
+    while eng.info(one)["n_masked"]:                           # one-position blocks: refresh, commit, next block
+        g = eng.mixed_step([one])
+        assert g.n_committed[0] == 1
+        steps += 1
+    assert steps == 3
+    eng.close()
