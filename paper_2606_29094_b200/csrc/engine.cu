@@ -1345,6 +1345,14 @@ static int mega_launch(dlm_ctx* c, const BatchDesc& bd, int layer0, int n_layers
   p.rope_cos = c->rope_cos; p.rope_sin = c->rope_sin; p.kv_store = (bf16*)c->kv_store; p.page_table = c->page_table;
   p.b = bd; p.g = c->kg; p.bar = c->mega_bar; p.tile_cnt = c->mega_bar + 64;
   p.phase_ts = c->opt_mega_ts ? c->mega_ts : nullptr;
+  // attention phase: K/V ranges per (request, KV head) so that about one unit lands on every SM; merged by the last to arrive
+  {
+    const int units = bd.n * a.n_kv_heads, kv_tiles = (bd.max_kv_len + 63) / 64;
+    int nsp = std::max(1, std::min(std::min(kMgMaxAttSplits, g_num_sms / std::max(1, units)), kv_tiles));
+    while (nsp > 1 && (size_t)nsp * bd.T * a.n_heads * (128 + 2) * 4 > c->attn_ws_bytes) --nsp;
+    p.att_splits = nsp;
+    p.ws_o = c->attn_ws; p.ws_ml = c->attn_ws + (size_t)nsp * bd.T * a.n_heads * 128;
+  }
   p.tr = c->tslot();
   if (p.stages < 2 || p.stages * (p.tpad * 128) + kMgScratchOwn < kMgAttnBytes) { set_err(&c->err, "layer kernel: shared-memory plan does not fit (tpad %d)", p.tpad); return DLM_E_ARG; }
   // slice capacity: a tile is cut into at most ceil(kbt * G / U) + 1 runs

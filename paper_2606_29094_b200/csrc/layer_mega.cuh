@@ -53,6 +53,7 @@ constexpr int kMgScratchOwn = 48 * 1024;      // attention scratch beyond the (i
 constexpr int kMgAttnBytes = 80 * 1024;
 constexpr int kMgMaxSeg = 6;                  // most slices a tile of the O / down projection may be cut into
 constexpr int kMgMaxSegQkv = 3, kMgMaxSegGu = 2;
+constexpr int kMgMaxAttSplits = 4;            // K/V ranges per (request, KV head) in the attention phase
 constexpr int kMgMaxTiles = 384;              // tiles per projection the slice-count tables hold
 constexpr int kMgTailBytes = 512 + 4 * kMgMaxTiles * 4 + 64;      // barriers, slice-count tables, reduction scratch
 
@@ -80,6 +81,9 @@ struct MegaParams {
   KvGeom g;
   unsigned int* bar;               // phase counter, zero at launch
   unsigned int* tile_cnt;          // [kMgMaxTiles] arrivals per tile of the projection in flight (zero at launch, self-resetting)
+  int att_splits;                  // K/V splits per (request, KV head) in the attention phase (1: no merge)
+  float* ws_o;                     // [att_splits][T * H][128] unnormalised partial outputs
+  float* ws_ml;                    // [att_splits][T * H][2]   (running max in log2 units, running sum)
   unsigned long long* phase_ts;    // optional [8 L + 2] %globaltimer at the end of each phase in CTA 0 (tuning aid), or null
   TraceSlot tr;
 };
@@ -439,8 +443,10 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
       // scratch = the X ring (idle during this phase: this CTA's X producer cannot pass the phase counter before the CTA
       // arrives) followed by the own scratch, contiguous: Q [64 rows][256 B] 16 KB, K 2 x 16 KB, V 2 x 16 KB
       const uint32_t sQ = sX, bK = sX + 16384, bV = sX + 16384 + 32768;
-      for (int unit = cta; unit < p.b.n * Hkv; unit += G) {
-        const int bi = unit / Hkv, kvh = unit % Hkv;
+      const int nsp = p.att_splits;
+      const long long TH = (long long)T * H;
+      for (int unit = cta; unit < p.b.n * Hkv * nsp; unit += G) {
+        const int sp = unit % nsp, bi = (unit / nsp) / Hkv, kvh = (unit / nsp) % Hkv;
         const int q_len = p.b.q_len[bi];
         if (q_len <= 0) continue;
         const int n_rows = q_len * r, S = p.b.kv_len[bi], q_off = p.b.q_off[bi];
@@ -466,8 +472,10 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
             cp_async16(bV + buf * kFaBN * 256 + tile_off(row, ch), vb + row * kFaDh + ch * 8, ok);
           }
         };
-        const int n_tiles = (S + kFaBN - 1) / kFaBN;
-        load_kv(0, 0);
+        const int n_tiles_all = (S + kFaBN - 1) / kFaBN;
+        const int per_sp = (n_tiles_all + nsp - 1) / nsp;
+        const int t_begin = sp * per_sp, t_end = min(n_tiles_all, t_begin + per_sp);     // this unit's K/V tiles (may be empty)
+        if (t_begin < t_end) load_kv(t_begin, 0);
         cp_async_commit();
         float o[16][4];
 #pragma unroll
@@ -476,14 +484,14 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
         uint32_t qf[8][4];
         const int wrow = cw * 16;
         const bool live = wrow < n_rows;                    // warp-uniform: this warp has query rows
-        for (int t = 0; t < n_tiles; ++t) {
-          const int buf = t & 1;
-          if (t + 1 < n_tiles) load_kv(t + 1, buf ^ 1);
+        for (int t = t_begin; t < t_end; ++t) {
+          const int buf = (t - t_begin) & 1;
+          if (t + 1 < t_end) load_kv(t + 1, buf ^ 1);
           cp_async_commit();
           cp_async_wait<1>();
           mg_bar128();
           if (live) {
-            if (t == 0) {
+            if (t == t_begin) {
 #pragma unroll
               for (int ks = 0; ks < 8; ++ks)
                 ldsm_x4(sQ + tile_off(wrow + (lane & 7) + ((lane >> 3) & 1) * 8, ks * 2 + (lane >> 4)), qf[ks][0], qf[ks][1], qf[ks][2], qf[ks][3]);
@@ -556,11 +564,72 @@ layer_mega_kernel(const __grid_constant__ CUtensorMap mapU, const __grid_constan
             if (rho >= n_rows) continue;
             const int tok = rho / r, hh = rho % r;
             const long long orow = (long long)(q_off + tok) * H + kvh * r + hh;
-            const float inv = 1.f / (hr ? l1 : l0);
-            bf16* dst = p.attn + orow * kFaDh;
+            if (nsp == 1) {
+              const float inv = 1.f / (hr ? l1 : l0);
+              bf16* dst = p.attn + orow * kFaDh;
 #pragma unroll
-            for (int i = 0; i < 16; ++i)
-              __stcg(reinterpret_cast<unsigned int*>(dst + i * 8 + tq * 2), pack_bf16(o[i][hr * 2] * inv, o[i][hr * 2 + 1] * inv));
+              for (int i = 0; i < 16; ++i)
+                __stcg(reinterpret_cast<unsigned int*>(dst + i * 8 + tq * 2), pack_bf16(o[i][hr * 2] * inv, o[i][hr * 2 + 1] * inv));
+            } else {                                          // unnormalised partial of this K/V range
+              float* dst = p.ws_o + ((long long)sp * TH + orow) * kFaDh;
+#pragma unroll
+              for (int i = 0; i < 16; ++i)
+                __stcg(reinterpret_cast<float2*>(dst + i * 8 + tq * 2), make_float2(o[i][hr * 2], o[i][hr * 2 + 1]));
+              if (tq == 0) {
+                const bool any = t_begin < t_end;
+                __stcg(reinterpret_cast<float2*>(p.ws_ml + ((long long)sp * TH + orow) * 2), make_float2(any ? (hr ? m1 : m0) : -CUDART_INF_F, any ? (hr ? l1 : l0) : 0.f));
+              }
+            }
+          }
+        }
+        if (nsp > 1) {
+          // the last of the (request, KV head)'s K/V ranges to arrive merges them: out = sum_s o_s 2^(m_s - m) / sum_s l_s 2^(m_s - m),
+          // ranges in index order (deterministic)
+          unsigned int* cnt = p.tile_cnt + kMgMaxTiles + (bi * Hkv + kvh);
+          mg_bar128();
+          if (tid == 0) { __threadfence(); red_i[0] = (int)atomicAdd(cnt, 1u); }
+          mg_bar128();
+          if (red_i[0] == nsp - 1) {
+            if (tid == 0) *cnt = 0;
+            __threadfence();
+            for (int i0 = tid; i0 < n_rows * 32; i0 += 2 * 128) {       // item = (stacked row, 4 output dims); 2 items per pass
+              float4 po[2][kMgMaxAttSplits];
+              float2 ml[2][kMgMaxAttSplits];
+#pragma unroll
+              for (int mm = 0; mm < 2; ++mm) {
+                const int i = i0 + mm * 128;
+                const bool ok = i < n_rows * 32;
+                const int rho = ok ? i >> 5 : 0, e = (i & 31) * 4;
+                const long long orow = (long long)(q_off + rho / r) * H + kvh * r + rho % r;
+#pragma unroll
+                for (int s2 = 0; s2 < kMgMaxAttSplits; ++s2) {
+                  const bool ld = ok && s2 < nsp;
+                  ml[mm][s2] = ld ? __ldcg(reinterpret_cast<const float2*>(p.ws_ml + ((long long)s2 * TH + orow) * 2)) : make_float2(-CUDART_INF_F, 0.f);
+                  po[mm][s2] = ld ? __ldcg(reinterpret_cast<const float4*>(p.ws_o + ((long long)s2 * TH + orow) * kFaDh + e)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+              }
+#pragma unroll
+              for (int mm = 0; mm < 2; ++mm) {
+                const int i = i0 + mm * 128;
+                if (i >= n_rows * 32) continue;
+                const int rho = i >> 5, e = (i & 31) * 4;
+                const long long orow = (long long)(q_off + rho / r) * H + kvh * r + rho % r;
+                float mx = -CUDART_INF_F;
+#pragma unroll
+                for (int s2 = 0; s2 < kMgMaxAttSplits; ++s2) mx = fmaxf(mx, ml[mm][s2].x);
+                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                float lsum = 0.f;
+#pragma unroll
+                for (int s2 = 0; s2 < kMgMaxAttSplits; ++s2) {
+                  if (ml[mm][s2].x == -CUDART_INF_F) continue;
+                  const float w = exp2f(ml[mm][s2].x - mx);
+                  lsum += ml[mm][s2].y * w;
+                  acc.x += po[mm][s2].x * w; acc.y += po[mm][s2].y * w; acc.z += po[mm][s2].z * w; acc.w += po[mm][s2].w * w;
+                }
+                const float inv = 1.f / lsum;
+                __stcg(reinterpret_cast<uint2*>(p.attn + orow * kFaDh + e), make_uint2(pack_bf16(acc.x * inv, acc.y * inv), pack_bf16(acc.z * inv, acc.w * inv)));
+              }
+            }
           }
         }
         mg_bar128();                                        // sQ / K / V buffers are rewritten by the next unit
