@@ -134,12 +134,20 @@ __global__ void __launch_bounds__(1024) rmsnorm_kernel(TA* __restrict__ u, float
         const long long ps4 = part_stride >> 2;
         // eight slice loads in flight at a time (the kernel is one dependent L2 round trip after the other); slices are still
         // added in slice order, a slice past n_part is not read and adds an exact zero
-        for (int s0 = 0; s0 < n_part; s0 += 8) {
-          float4 q[8];
+        if (n_part > 4) {          // weight-streaming regime (8-9 slices, one chunk per thread)
+          for (int s0 = 0; s0 < n_part; s0 += 8) {
+            float4 q[8];
 #pragma unroll
-          for (int s = 0; s < 8; ++s) q[s] = s0 + s < n_part ? __ldcg(pr + (s0 + s) * ps4) : make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int s = 0; s < 8; ++s) q[s] = s0 + s < n_part ? __ldcg(pr + (s0 + s) * ps4) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-          for (int s = 0; s < 8; ++s) { a.x += q[s].x; a.y += q[s].y; a.z += q[s].z; a.w += q[s].w; }
+            for (int s = 0; s < 8; ++s) { a.x += q[s].x; a.y += q[s].y; a.z += q[s].z; a.w += q[s].w; }
+          }
+        } else {                   // CTA-pair regime (<= 4 slices, up to 4 chunks per thread): keep the register footprint small
+#pragma unroll 4
+          for (int s = 0; s < n_part; ++s) {
+            const float4 q = __ldcg(pr + s * ps4);
+            a.x += q.x; a.y += q.y; a.z += q.z; a.w += q.w;
+          }
         }
         xr[i] = a;
       }
