@@ -18,7 +18,7 @@ import subprocess
 import sys
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-SELECT = "teacher_forced or free_running or precise or batch_shape"
+SELECT = "teacher_forced or free_running or precise or batch_shape or full_depth"
 
 
 def main():

@@ -1010,3 +1010,56 @@ def test_finished_and_single_row_requests_in_a_batch(bf16_model):
         steps += 1
     assert steps == 3
     eng.close()
+
+
+def test_c2_full_depth_refresh_and_cached_step_vs_oracle():
+    """north_star's tolerance at the REAL size: BASELINE.json configs[1] with all 32 layers, d 4096, vocabulary 126 464 -- one
+    refresh step (512 tokens, CTA-pair GEMMs, tcgen05 attention) and one cached step (32 tokens, weight-streaming GEMMs on the
+    tiled copy) from the workload's initial state, against the fp64 oracle run at full depth: hidden state of the block rows
+    (last layer's residual output) and log-sum-exp within 2e-2 relative, tokens equal where the oracle's top-2 margin is clear,
+    commits judged by compare_commits.  The confidence error of 32 bf16 layers is measured against the control's (the fp64
+    oracle with bf16 rounding at the same points): the GPU may not be worse than twice the control."""
+    pkg = _pkg()
+    from oracle import control
+    from synth_inputs import workload_c2
+    arch, seed = ARCH_LLADA8B, WEIGHT_SEED["C2"]
+    spec = workload_c2()[0]
+    S, Bk = len(spec.prompt) + spec.gen_len, spec.block_len
+    eng = pkg.Engine(arch, seed, max_requests=1, max_seq=S, max_block=Bk, max_batch_tokens=S)
+    eng.set_option(pkg.OPT_DEBUG_DUMP, 1)
+    rid = eng.add_request(spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
+    wts = ow.Weights(arch, seed)
+    oreq = ostep.Request(arch, spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
+    creq = ostep.Request(arch, spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
+    rnd = control.make_rounder(1e-6, 99)
+    lo, hi = oreq.block_range(0)
+    masked = oreq.tokens[lo:hi] == arch.mask_id
+    stats = dict(steps=0, exact=0, excluded=0, mismatch=0, unexplained=0, max_conf_err=0.0, max_hid=0.0, max_lse=0.0, median_gap=None,
+                 control=dict(exact=0, excluded=0, mismatch=0, max_conf_err=0.0))
+    for kind in ("refresh", "cached"):
+        g = eng.refresh_step([rid], dry_run=True) if kind == "refresh" else eng.cached_step([rid], dry_run=True)
+        o = ostep.refresh_step(oreq, wts, dry_run=True) if kind == "refresh" else ostep.cached_step(oreq, wts, dry_run=True)
+        hid = _gpu_hidden_block_rows(pkg, eng, rid, arch, o, kind == "refresh")
+        e_hid = float(compare.rel_rows(hid, o.hidden).max())
+        e_lse = float(np.abs(g.lse[0][:Bk] - o.lse).max() / np.abs(o.lse).max())
+        e_conf = float(np.abs(g.row_conf[0][:Bk] - o.conf).max())
+        c = control.step(creq, wts, kind == "refresh", rnd=rnd)
+        c_conf = float(np.abs(c.conf - o.conf).max())
+        c_hid = float(compare.rel_rows(c.hidden, o.hidden).max())
+        dc = compare.compare_commits(o, masked, spec.threshold, [(x.pos, x.tok, x.conf) for x in c.commits])
+        stats["control"]["exact"] += dc.exact; stats["control"]["excluded"] += dc.n_excluded; stats["control"]["mismatch"] += dc.n_mismatch
+        stats["control"]["max_conf_err"] = max(stats["control"]["max_conf_err"], c_conf)
+        stats["control_max_hid"] = max(stats.get("control_max_hid", 0.0), c_hid)
+        assert e_hid <= 2e-2 and e_lse <= 2e-2 and e_conf <= max(CONF_ERR_MAX, 2 * c_conf), (kind, e_hid, e_lse, e_conf, c_conf, c_hid)
+        clear = o.margin >= 2 * e_conf + 1e-3
+        assert np.array_equal(g.row_tok[0][:Bk][clear], o.tok[clear]), kind
+        d = compare.compare_commits(o, masked, spec.threshold, g.commits[0])
+        wide = compare.compare_commits(o, masked, spec.threshold, g.commits[0], band=2 * e_conf + compare.BAND)
+        assert wide.n_mismatch == 0, (kind, wide.detail)
+        stats["steps"] += 1; stats["exact"] += d.exact; stats["excluded"] += d.n_excluded; stats["mismatch"] += d.n_mismatch
+        stats["max_hid"], stats["max_lse"], stats["max_conf_err"] = max(stats["max_hid"], e_hid), max(stats["max_lse"], e_lse), max(stats["max_conf_err"], e_conf)
+        if np.isfinite(d.min_gap):
+            stats["median_gap"] = d.min_gap
+    _record("P-B_C2_full_depth_L32", stats)
+    print("C2 full depth", stats)
+    eng.close()
