@@ -195,8 +195,9 @@ DLM_API int  dlm_profile_step_costs_ex(dlm_ctx*, int32_t block_len, int32_t repe
 #define DLM_OPT_TRACE         11   /* 1: every kernel of the next steps stamps %globaltimer into its own record (dlm_step_trace); works
                                       under CUDA-graph replay and programmatic dependent launch, costs ~3 atomics per CTA      */
 #define DLM_OPT_TCT_MIN_ITEMS 12   /* fewest (request, KV head, query tile) work items for which a step takes the tcgen05 attention
-                                      kernels (default 1: always); below it the mma.sync kernel runs (debugging / A-B timing)  */
-#define DLM_OPT_LAYER_KERNEL  13   /* 1 (default 0: measured slower than the per-stage kernels): steps of <= 64 tokens whose requests each compute <= 64 stacked query rows (the
+                                      kernels (default 64); below it the mma.sync kernel runs.  1 = always tcgen05 (A/B timing)         */
+#define DLM_OPT_LAYER_KERNEL  13   /* default 0 (measured slower than the per-stage kernels).  1: steps of <= 64 tokens whose
+                                      requests each compute <= 64 stacked query rows (the
                                       batch-1 cache step) run ALL layers in one persistent launch (layer_mega_kernel: weight
                                       stream never stops, stream-K work split, in-kernel phase counter); 0: one kernel per stage */
 #define DLM_OPT_LAYER_KERNEL_PHASE_TS 14 /* 1: that kernel records a timestamp per phase in CTA 0 (tuning aid, dlm_layer_kernel_phases) */
