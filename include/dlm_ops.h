@@ -36,6 +36,11 @@ DLM_API int dlm_op_gemm_bf16(const void* A, const void* W, void* out, int32_t M,
 DLM_API int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, int32_t M, int32_t N, int32_t K, int32_t epilogue,
                           int32_t bn, int32_t splits, void* stream);
 
+/* The tile plan dlm_op_gemm_pair_bf16 / the engine take for a shape with bn = 0 (no split-K): *bn = width of the column blocks,
+ * and when the launch mixes two widths (gate/up projections of <= 1024 rows: the pairs' last tiles are narrower so that the
+ * last wave is full) *bn2 = the narrow width and *n_wide = how many leading column blocks are *bn wide; else *bn2 = 0. */
+DLM_API int dlm_op_gemm_pair_plan(int32_t M, int32_t N, int32_t K, int32_t epilogue, int32_t* bn, int32_t* bn2, int32_t* n_wide);
+
 /* Weight-streaming split-K tcgen05 GEMM for T <= 128 tokens (the cached step's a3/a6/a8/a9): swap-AB (weights on
  * the MMA's M side, tokens on N), every K split writes an fp32 slice and the slices are summed in a fixed order.
  * epilogue DLM_EPI_F32: out fp32 [T, N] = X . W^T; DLM_EPI_SWIGLU: out bf16 [T, N], W = [2N, K] (gate rows, up rows).

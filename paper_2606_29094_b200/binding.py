@@ -134,6 +134,7 @@ def lib() -> C.CDLL:
         L.dlm_op_gemm_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
         L.dlm_op_gemm_pair_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
         L.dlm_op_gemm_plain_bf16.argtypes = [vp, vp, vp, i32, i32, i32, vp]
+        L.dlm_op_gemm_pair_plan.argtypes = [i32, i32, i32, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
         L.dlm_op_gemm_skinny_bf16.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
         L.dlm_op_lmhead_scratch_bytes.argtypes = [i32, i32]
         L.dlm_op_lmhead_scratch_bytes.restype = i64
@@ -440,6 +441,13 @@ def op_gemm_pair_bf16(A, W, epilogue: int = EPI_F32, bn: int = 0, out=None, spli
     rc = lib().dlm_op_gemm_pair_bf16(A.data_ptr(), W.data_ptr(), out.data_ptr(), M, N, K, epilogue, bn, splits, _stream_ptr())
     _op_check(rc)
     return (out, rc) if return_splits else out
+
+
+def op_gemm_pair_plan(M: int, N: int, K: int, epilogue: int):
+    """(bn, bn2, n_wide) of the automatic tile plan (bn2 = 0: one width)."""
+    a, b, c = C.c_int32(), C.c_int32(), C.c_int32()
+    _op_check(lib().dlm_op_gemm_pair_plan(M, N, K, epilogue, C.byref(a), C.byref(b), C.byref(c)))
+    return a.value, b.value, c.value
 
 
 def op_gemm_skinny_bf16(X, W, epilogue: int = EPI_F32, splits: int = 0):

@@ -6,6 +6,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -269,6 +270,52 @@ static void plan_pair(int M, int N, int K, int epi, int max_splits, int* bn_out,
   }
 }
 
+// Mixed tile widths for launches with few row tiles (<= 16: one panel, column blocks dealt round-robin in order): the first
+// n_a column blocks are bn1 wide, the rest bn2 < bn1, so that the pairs' last tiles are narrower, cheaper ones instead of a
+// partly filled wave of wide tiles (512 tokens: 192 gate/up tiles of 256 on 74 pairs = 3 waves for 2.6 waves of work; measured
+// gate/up at 512 tokens 2590 -> 2468 us per C2 refresh step, 3006 -> 2611 us per C4 cached step).  Exact
+// makespan of the round-robin dealing under plan_pair's cost model; taken only when it beats the best uniform width by > 3 %.
+static bool plan_pair_mixed(int M, int N, int K, int epi, int bn_uniform, int* bn1_out, int* bn2_out, int* n_a_out, int* n_b_out) {
+  const int m_tiles = (M + 255) / 256, pairs = std::max(1, g_num_sms / 2), num_kb = (K + kBK - 1) / kBK;
+  // gate/up only: for the fused-RoPE QKV epilogue the 256-wide first tiles measured slower than three waves of 128-wide ones
+  // (C2 refresh: QKV 1485 -> 1534 us per step), its long epilogue is cheaper in small pieces
+  // and only up to 1024 rows: with more row tiles the tail wave is a small share (< 3 % by this model at 9 row tiles), and the
+  // search below is host time on the launch path of steps that are not replayed from a graph (memoised per shape)
+  if (m_tiles > 4 || epi != EPI_SWIGLU) return false;
+  struct Plan { bool ok; int b1, b2, na, nb; };
+  static thread_local std::map<std::tuple<int, int, int, int, int>, Plan> memo;
+  const auto key = std::make_tuple(M, N, K, bn_uniform, g_num_sms);
+  auto hit = memo.find(key);
+  if (hit != memo.end()) {
+    if (hit->second.ok) { *bn1_out = hit->second.b1; *bn2_out = hit->second.b2; *n_a_out = hit->second.na; *n_b_out = hit->second.nb; }
+    return hit->second.ok;
+  }
+  auto per = [&](int bn) { return epi == EPI_SWIGLU ? bn / 2 : bn; };
+  auto cost = [&](int bn) { return (long long)num_kb * (56 + (200 * bn) / 256) + 8LL * (128 + bn / 2); };
+  auto makespan = [&](int n_a, int bn1, int n_b, int bn2) {
+    std::vector<long long> load(pairs, 0);
+    const int tiles = m_tiles * (n_a + n_b);
+    for (int t = 0; t < tiles; ++t) load[t % pairs] += cost(t / m_tiles < n_a ? bn1 : bn2);
+    return *std::max_element(load.begin(), load.end());
+  };
+  const long long uni = makespan((N + per(bn_uniform) - 1) / per(bn_uniform), bn_uniform, 0, bn_uniform);
+  static const int w_glu[][2] = {{256, 192}, {256, 128}, {192, 128}, {256, 64}, {192, 64}, {128, 64}};
+  const int (*w)[2] = w_glu;
+  const int nw = 6;
+  long long best = uni;
+  for (int i = 0; i < nw; ++i) {
+    const int p1 = per(w[i][0]), p2 = per(w[i][1]);
+    for (int n_a = 1; n_a * p1 < N; ++n_a) {
+      const int n_b = (N - n_a * p1 + p2 - 1) / p2;
+      const long long c = makespan(n_a, w[i][0], n_b, w[i][1]);
+      if (c < best) { best = c; *bn1_out = w[i][0]; *bn2_out = w[i][1]; *n_a_out = n_a; *n_b_out = n_b; }
+    }
+  }
+  const bool ok = best * 100 < uni * 97;
+  memo[key] = Plan{ok, *bn1_out, *bn2_out, *n_a_out, *n_b_out};
+  return ok;
+}
+
 template <int EPI>
 static cudaError_t launch_gemm_pair_t(const CUtensorMap* ma, const CUtensorMap* mb, const CUtensorMap* mc, const GemmPairParams& p, cudaStream_t st, bool pdl) {
   static bool configured[kMaxDevices] = {};
@@ -303,6 +350,7 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
   if (epi != EPI_F32) max_splits = 1;
   int splits = 1;
   if (epi == EPI_ROPE && bn != 128 && bn != 256) bn = 0;         // whole 128-wide heads per tile: 256 or 128, planned
+  const bool auto_bn = bn <= 0;
   if (bn <= 0) plan_pair(M, N, K, epi, max_splits, &bn, &splits);
   else if (max_splits < 0) splits = -max_splits;                 // test hook: forced split count
   if (bn % 32 || bn < 64 || bn > 256 || (epi == EPI_SWIGLU && bn % 64)) { set_err(err, "gemm_pair: bad bn=%d", bn); return DLM_E_ARG; }
@@ -318,6 +366,14 @@ static int gemm_pair(TmapCache& tc, std::string* err, const void* A, long long a
   p.m_tiles = (M + 255) / 256;
   p.n_tiles_n = (N + per - 1) / per;
   p.panel = std::min(p.m_tiles, 16);
+  p.bn2 = 0; p.n_tiles_a = p.n_tiles_n;
+  if (auto_bn && p.splits == 1 && getenv("DLM_NO_MIXED_TILES") == nullptr) {
+    int b1 = bn, b2 = 0, na = 0, nb = 0;
+    if (plan_pair_mixed(M, N, K, epi, bn, &b1, &b2, &na, &nb)) {
+      bn = b1; p.bn = b1; p.bn2 = b2; p.n_tiles_a = na; p.n_tiles_n = na + nb;
+      p.stages = std::max(2, std::min(std::min((num_kb + kPairKbPerStage - 1) / kPairKbPerStage, 12), (224 * 1024 - kPairEpiStageBytes) / gemm_pair_stage_bytes(bn)));
+    }
+  }
   p.w_policy = DLM_L2_EVICT_NORMAL;
   p.a_policy = DLM_L2_EVICT_NORMAL;
   if (epi == EPI_LMHEAD && p.n_tiles_n != p.n_tiles) { set_err(err, "gemm_pair: lm-head tile count mismatch"); return DLM_E_ARG; }
@@ -2002,6 +2058,17 @@ extern "C" int dlm_op_gemm_pair_bf16(const void* A, const void* W, void* out, in
   cudaFree(part);
   if (!rc && e != cudaSuccess) { set_err(&g_init_error, "dlm_op_gemm_pair_bf16: %s", cudaGetErrorString(e)); rc = DLM_E_CUDA; }
   return rc < 0 ? rc : ns;
+}
+
+extern "C" int dlm_op_gemm_pair_plan(int32_t M, int32_t N, int32_t K, int32_t epi, int32_t* bn, int32_t* bn2, int32_t* n_wide) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!bn || !bn2 || !n_wide || M <= 0 || N <= 0 || K <= 0 || epi < 0 || epi > 3) { set_err(&g_init_error, "dlm_op_gemm_pair_plan: bad arguments"); return DLM_E_ARG; }
+  int b = 0, sp = 1, b1 = 0, b2 = 0, na = 0, nb = 0;
+  plan_pair(M, N, K, epi, 1, &b, &sp);
+  *bn = b; *bn2 = 0; *n_wide = 0;
+  if (plan_pair_mixed(M, N, K, epi, b, &b1, &b2, &na, &nb)) { *bn = b1; *bn2 = b2; *n_wide = na; }
+  return DLM_OK;
 }
 
 extern "C" int dlm_op_gemm_skinny_bf16(const void* X, const void* W, void* out, int32_t T, int32_t N, int32_t K, int32_t epi, int32_t splits, void* stream) {

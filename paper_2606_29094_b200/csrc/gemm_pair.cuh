@@ -42,6 +42,8 @@ struct RopeEpi {
 struct GemmPairParams {
   int M, N, K;        // N = output features (SwiGLU: F; a tile covers bn/2 of them)
   int bn;             // MMA N of the pair tile: multiple of 32 (SwiGLU: 64) in [64, 256]
+  int bn2, n_tiles_a; // mixed widths (bn2 > 0): the first n_tiles_a column blocks are bn wide, the rest bn2 < bn wide, so that the
+                      // last wave of a launch with few row tiles is a wave of narrower, cheaper tiles instead of a partly filled one
   int stages;
   int up_row0;        // SwiGLU: first row of the up projection inside W (= F)
   int m_tiles, n_tiles_n, panel;
@@ -156,6 +158,18 @@ __device__ __forceinline__ PairTile pair_tile(int t, int m_tiles, int n_tiles, i
   return r;
 }
 
+// width and first output column (SwiGLU: first feature) of column block n_blk
+struct PairCols { int bn, n0; };
+template <int EPI>
+__device__ __forceinline__ PairCols pair_cols(int n_blk, const GemmPairParams& p) {
+  PairCols c;
+  const int per1 = EPI == EPI_SWIGLU ? p.bn / 2 : p.bn;
+  if (p.bn2 <= 0 || n_blk < p.n_tiles_a) { c.bn = p.bn; c.n0 = n_blk * per1; return c; }
+  const int per2 = EPI == EPI_SWIGLU ? p.bn2 / 2 : p.bn2;
+  c.bn = p.bn2; c.n0 = p.n_tiles_a * per1 + (n_blk - p.n_tiles_a) * per2;
+  return c;
+}
+
 template <int EPI>
 __global__ void __launch_bounds__(kPairThreads, 1)
 gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CUtensorMap mapC,
@@ -207,9 +221,11 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
       const uint32_t half_rows = (uint32_t)BN / 2;
       const uint32_t w_bytes = half_rows * 128u;
       const uint32_t tx_kb = 2u * (kATileBytes + w_bytes);          // both CTAs' bytes of one K block
+      // the box is always BN / 2 rows (one tensor map); a narrower tile uses the first bn_t / 2 of them
       auto w_row_of = [&](const PairTile& tl) {
-        if (EPI == EPI_SWIGLU) return tl.n_blk * (int)half_rows + (leader ? 0 : p.up_row0);
-        return tl.n_blk * BN + (int)rank * (int)half_rows;
+        const PairCols pc = pair_cols<EPI>(tl.n_blk, p);
+        if (EPI == EPI_SWIGLU) return pc.n0 + (leader ? 0 : p.up_row0);
+        return pc.n0 + (int)rank * (pc.bn / 2);
       };
       auto load_w = [&](uint32_t sa, int kb_abs, int cnt, int w_row, uint32_t fb) {
         for (int h = 0; h < cnt; ++h)
@@ -265,10 +281,10 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
   } else if (warp == 1) {
     if (leader) {
       // ---------------- MMA issuer (leader CTA; the whole warp walks the loop, one elected lane issues) ----------------
-      const uint32_t idesc = ptx::umma_idesc_bf16(256, BN);
       int i = 0, s = 0;
       uint32_t ph = 0;
       for (int u = cluster; u < total_units; u += n_clusters, ++i) {
+        const uint32_t idesc = ptx::umma_idesc_bf16(256, pair_cols<EPI>(pair_tile(u % total_tiles, p.m_tiles, p.n_tiles_n, p.panel).n_blk, p).bn);
         const uint32_t as = (uint32_t)i & 1u, aph = ((uint32_t)i >> 1) & 1u;
         ptx::mbar_wait(tmem_empty_bar + 8u * as, aph ^ 1u);
         ptx::tc_fence_after();
@@ -309,6 +325,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
     int i = 0;
     for (int u = cluster; u < total_units; u += n_clusters, ++i) {
       const PairTile tl = pair_tile(u % total_tiles, p.m_tiles, p.n_tiles_n, p.panel);
+      const PairCols pc = pair_cols<EPI>(tl.n_blk, p);
+      const int BNt = pc.bn;                              // this tile's width (== BN unless the launch mixes two widths)
       const uint32_t as = (uint32_t)i & 1u, aph = ((uint32_t)i >> 1) & 1u;
       const int row = tl.m_blk * 256 + (int)rank * 128 + quarter * 32 + lane;
       const bool row_ok = row < p.M;
@@ -340,7 +358,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         // fp32 outputs leave through TMA: the chunk is staged (swizzled as the output map expects) and one lane issues a bulk
         // tensor store -- or, for the residual stream, a bulk REDUCE-ADD (x += acc happens in L2: no read of x by the SM, and
         // exactly one add per element, so the result is deterministic).  TMA clips rows >= M and columns >= N.
-        const int n0 = tl.n_blk * BN, nch = BN / 32;
+        const int n0 = pc.n0, nch = BNt / 32;
         for (int c = 0; c < nch; ++c) {
           const int b = c & 1;
           if (c >= 2) {                                                            // the bulk op that last read this buffer
@@ -361,7 +379,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         if (lane == 0) ptx::bulk_wait_read<0>();                                   // the stage is reused by the next tile
         __syncwarp();
       } else if (EPI == EPI_BF16) {
-        const int n0 = tl.n_blk * BN, nch = BN / 32;
+        const int n0 = pc.n0, nch = BNt / 32;
         const long long obase = (long long)(row_w0 + t_rr) * p.ldc + n0 + t_c4;   // transposed view, hoisted
         for (int c = 0; c < nch; ++c) {
           __syncwarp();
@@ -387,8 +405,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
           }
         }
       } else if (EPI == EPI_SWIGLU) {
-        const int half = BN / 2;
-        const int f0 = tl.n_blk * half;
+        const int half = BNt / 2;
+        const int f0 = pc.n0;
         uint32_t u2[32];
         for (int c = 0; c < half / 32; ++c) {
           __syncwarp();
@@ -425,8 +443,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant
         }
         uint32_t u2[32];
 #pragma unroll 1
-        for (int hh = 0; hh < (BN >> 7); ++hh) {
-          const int hg = tl.n_blk * (BN >> 7) + hh;             // global head index: Q heads, then K heads, then V heads
+        for (int hh = 0; hh < (BNt >> 7); ++hh) {
+          const int hg = (pc.n0 >> 7) + hh;             // global head index: Q heads, then K heads, then V heads
           const bool head_ok = hg < e.n_heads + 2 * e.g.n_kv_heads;
           const bool rotate = hg < e.n_heads + e.g.n_kv_heads;
           long long dst_own = 0;                                // element offset of this thread's row in its destination, -1: none

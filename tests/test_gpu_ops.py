@@ -126,6 +126,25 @@ def test_gemm_pair_swiglu(M, F, K, bn):
     assert np.all(np.abs(_f64(got) - want) <= np.abs(want) * 2 ** -8 + 2e-4)
 
 
+@pytest.mark.parametrize("M,F,K", [(512, 12288, 256), (1000, 12200, 128), (300, 11000, 192)])
+def test_gemm_pair_swiglu_mixed_tile_widths(M, F, K):
+    """Gate/up projections of <= 1024 rows with many column blocks: the automatic plan deals the first column blocks wide and the
+    rest narrow (two tile widths in one launch); results against fp64 on every element, ragged tails in the
+    rows and in the features (12 200 and 11 000 are multiples of neither width), and the plan really is mixed."""
+    import paper_2606_29094_b200 as pkg
+    bn, bn2, n_wide = pkg.op_gemm_pair_plan(M, F, K, pkg.EPI_SWIGLU)
+    assert bn2 in (64, 128, 192) and bn2 < bn and 0 < n_wide < (F + bn // 2 - 1) // (bn // 2), (bn, bn2, n_wide)
+    rng = np.random.default_rng(M + F + K)
+    A, a = _mk(rng, M, K)
+    W, w = _mk(rng, 2 * F, K, 0.1)
+    want = omodel.silu(a @ w[:F].T) * (a @ w[F:].T)
+    got = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_SWIGLU, 0)
+    uniform = pkg.op_gemm_pair_bf16(A, W, pkg.EPI_SWIGLU, 256)
+    torch.cuda.synchronize()
+    assert np.all(np.abs(_f64(got) - want) <= np.abs(want) * 2 ** -8 + 2e-4)
+    assert np.array_equal(_f64(got), _f64(uniform))            # same K order per element whatever the tile width: bit-identical
+
+
 SKINNY_SHAPES = [  # (T, N, K): tails in every dimension, one and several K blocks per split
     (32, 256, 128), (1, 128, 64), (32, 4096, 4096), (17, 384, 688), (64, 200, 512), (100, 1056, 200), (128, 768, 256), (33, 96, 4096)]
 
