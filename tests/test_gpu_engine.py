@@ -64,7 +64,7 @@ def _run_parity(arch, seed, spec, max_steps, teacher_forced, hid_tol, lse_tol, s
     eng.set_option(pkg.OPT_SIMPLE_KERNELS, 1 if simple else 0)
     eng.set_option(pkg.OPT_FLASH_ATTENTION, 1 if flash else 0)
     rid = eng.add_request(spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
-    wts = ow.Weights(oarch, seed)
+    wts = ow.Weights(oarch, seed, keep_f64=oarch.n_layers <= 4)      # shallow models: keep the float64 copies (the step loop reuses them)
     oreq = ostep.Request(oarch, spec.prompt, spec.gen_len, spec.block_len, spec.threshold)
     creq = ostep.Request(oarch, spec.prompt, spec.gen_len, spec.block_len, spec.threshold) if with_control else None
     rnd = control.make_rounder(1e-6, 1234) if with_control else None
@@ -412,11 +412,11 @@ def test_c2_reduced_depth_teacher_forced(simple, flash):
     arch = _reduced(ARCH_LLADA8B, 2)
     rng = np.random.default_rng(2002)
     spec = RequestSpec(random_tokens(rng, 96, arch.vocab, arch.mask_id), 64, 32, 0.9)
-    steps = 34 if (not simple and flash) else 5          # production kernels: one whole block (1 refresh + cached steps) and the next refresh
+    steps = 64 if (not simple and flash) else 5          # production kernels: both blocks of the generation, to completion
     s = _run_parity(arch, WEIGHT_SEED["C2"], spec, steps, teacher_forced=True, hid_tol=2e-2, lse_tol=2e-2, simple=simple, flash=flash, with_control=True,
                     record=f"P-B_C2_L2_simple{int(simple)}_flash{int(flash)}")
     print("P-B C2/L2", dict(simple=simple, flash=flash), s)
-    assert s["steps"] == steps and s["unexplained"] == 0
+    assert (s["steps"] == steps or (steps == 64 and 34 <= s["steps"] <= 64)) and s["unexplained"] == 0
 
 
 def test_launch_modes_agree_bitwise():
@@ -456,9 +456,9 @@ def test_c5_reduced_depth_gqa_teacher_forced():
     arch = _reduced(ARCH_QWEN7B, 2)
     rng = np.random.default_rng(2005)
     spec = RequestSpec(random_tokens(rng, 200, arch.vocab, arch.mask_id), 64, 32, 0.9)
-    s = _run_parity(arch, WEIGHT_SEED["C5"], spec, 12, teacher_forced=True, hid_tol=2e-2, lse_tol=2e-2, with_control=True, record="P-B_C5_L2_gqa")
+    s = _run_parity(arch, WEIGHT_SEED["C5"], spec, 34, teacher_forced=True, hid_tol=2e-2, lse_tol=2e-2, with_control=True, record="P-B_C5_L2_gqa")
     print("P-B C5/L2", s)
-    assert s["steps"] == 12 and s["unexplained"] == 0
+    assert s["steps"] == 34 and s["unexplained"] == 0
 
 
 def test_c2_reduced_depth_precise_mode_free_running():
@@ -468,10 +468,10 @@ def test_c2_reduced_depth_precise_mode_free_running():
     arch = _reduced(ARCH_LLADA8B, 2)
     rng = np.random.default_rng(2002)
     spec = RequestSpec(random_tokens(rng, 96, arch.vocab, arch.mask_id), 64, 32, 0.9)
-    s = _run_parity(arch.replace(weight_dtype=2), WEIGHT_SEED["C2"], spec, 34, teacher_forced=False, hid_tol=1e-4, lse_tol=1e-4,
+    s = _run_parity(arch.replace(weight_dtype=2), WEIGHT_SEED["C2"], spec, 64, teacher_forced=False, hid_tol=1e-4, lse_tol=1e-4,
                     oracle_arch=arch, record="P-D_C2_L2_precise_free_running")
     print("P-D C2/L2 precise", s)
-    assert s["mismatch"] == 0 and s["steps"] == 34
+    assert s["mismatch"] == 0 and 34 <= s["steps"] <= 64
 
 
 def test_stagewise_from_gpu_inputs():
