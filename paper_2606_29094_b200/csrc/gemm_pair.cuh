@@ -13,7 +13,8 @@
 //               residual add | SwiGLU | LM-head split-vocab statistics), then a remote arrive on the leader's
 //               tmem_empty barrier
 // Tiles are walked persistently (grid = one pair per TPC) in panels of `panel` m-tiles so that a wave shares its A
-// panel and a few W tiles through L2.
+// panel and a few W tiles through L2.  A launch may mix two tile widths (GemmPairParams::bn2): the leading column blocks
+// are BN wide, the rest narrower, so that with few row tiles the pairs' last tiles form a full wave of cheap tiles.
 // SwiGLU: the leader CTA stages gate rows, its peer the matching up rows, so accumulator columns [0, BN/2) are
 // the gate and [BN/2, BN) the up projection of the same BN/2 features.
 #pragma once

@@ -1,5 +1,6 @@
 // Persistent whole-stack kernel for small cached steps (T <= 64 tokens, the batch-1 "cache step" of P:347 that the
-// headline workload spends 31 of every 32 steps in): ALL layers of the step in ONE launch, one CTA per SM.
+// headline workload spends 31 of every 32 steps in): ALL layers of the step in ONE launch, one CTA per SM.  An experiment that
+// is kept because it is correct and instructive, not because it is faster (see Status below).
 //
 // Why.  With 32 tokens a layer is pure weight streaming (436 MB per layer at the LLaDA shape = 66.7 us at the measured
 // HBM rate) and the in-kernel timeline of the multi-kernel path (DLM_OPT_TRACE) shows its GEMMs already AT that rate --
@@ -25,15 +26,21 @@
 // consumer phase sums the slices of a tile in slice order, so results are deterministic (no atomics).
 //
 // Phases per layer (each ends with one arrival per CTA on a global counter; waiting = polling that counter):
-//   0 fold + norm   x += sum of the down-projection slices of the previous layer; u = bf16(RMSNorm(x))
-//   1 QKV GEMM      u -> partial slices
-//   2 attention     per (request, KV head): sum the Q/K/V slices, RoPE, write K/V to the pages, softmax(QK^T)V over all S
+//   0 fold + norm   x += sum of the down-projection slices of the previous layer; u = bf16(RMSNorm(x))   (one row per CTA)
+//   1 QKV GEMM      u -> partial slices; the CTA that completes a 128-column tile (= one head) finishes it: slice sum, RoPE,
+//                   Q row / K,V page rows (qkv_finish.cuh)
+//   2 attention     per (request, KV head, K/V range): mma.sync flash loop over the pages; the last range of a head to arrive
+//                   merges the ranges
 //   3 O GEMM        attn -> slices
-//   4 fold + norm
-//   5 gate/up GEMM  u -> slices (64 gate + 64 up rows per tile)
-//   6 SwiGLU        act = bf16(silu(sum gate) * sum up)
-//   7 down GEMM     act -> slices
-// and a final fold after the last layer.  Rounding points are those of the multi-kernel path.
+//   4 fold + norm   -> u2
+//   5 gate/up GEMM  u2 -> slices (64 gate + 64 up rows per tile); the completing CTA applies SwiGLU -> act
+//   6 down GEMM     act -> slices
+// and a final fold after the last layer.  Rounding points are those of the per-stage path.
+//
+// Status: correct (tests/test_gpu_engine.py::test_layer_kernel_option_*), but 3.95 ms per C2 cached step against 3.2 ms for the
+// per-stage kernels: a grid-wide phase boundary is a chain of dependent L2 round trips (slice stores, fence, atomic, poll, TMA
+// of X, first MMA) that costs what a kernel boundary costs under programmatic dependent launch, and the ring here is smaller.
+// Off by default (DLM_OPT_LAYER_KERNEL); DESIGN.md section 8 has the phase timings.
 #pragma once
 #include <math_constants.h>
 
