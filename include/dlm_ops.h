@@ -66,6 +66,39 @@ DLM_API int dlm_op_lmhead_unmask_bf16(const void* hidden, const void* W_lm, int3
                               int32_t* n_committed, int32_t* pos, int32_t* tok, float* conf, void* scratch,
                               void* stream);
 
+/* dlm_op_lmhead_bf16 for callers that must not allocate device memory and have none to spare for scratch.
+ *
+ * Who this is for: code that runs where cudaMalloc is off the table -- a serving loop whose whole HBM budget was handed
+ * to a pool at start-up (K/V pages, weights) and must not grow, a latency-critical section that cannot afford the
+ * device-wide synchronisation cudaMalloc / cudaFree imply, a plug-in that is only ever given input and output buffers by
+ * its host program.  dlm_op_lmhead_bf16 asks such a caller for a scratch buffer (the split-vocabulary partials: one
+ * (max, sum, argmax) record per row and 128-column vocabulary tile); this entry point keeps that scratch inside the
+ * library instead, in one file-scope device array of DLM_LMHEAD_STATIC_SCRATCH_BYTES bytes that every GPU which loads
+ * libdlm.so holds from module load until the process exits.  The caller passes inputs and outputs only.
+ *
+ * Same operation, same kernels, same results as dlm_op_lmhead_bf16 (tok = argmax_v z, lowest id on ties;
+ * conf = softmax(z)[tok]; lse = log sum exp z; z = scale * hidden . W_lm^T, z[mask_id] = -inf).
+ * hidden bf16 [R, K], W_lm bf16 [V, K], tok int32 [R], conf / lse fp32 [R]: device pointers, caller-owned.
+ *
+ * Limits: 1 <= R <= DLM_LMHEAD_STATIC_MAX_ROWS and dlm_op_lmhead_static_bytes(R, V) <= DLM_LMHEAD_STATIC_SCRATCH_BYTES
+ * (128 rows x 152 064 columns needs 2.4 MB); anything larger returns DLM_E_CAPACITY with the numbers in
+ * dlm_last_error(NULL) and launches nothing.  K % 8 == 0 as for the other GEMMs.
+ *
+ * The call performs no cudaMalloc / cudaFree / cudaMallocAsync and calls no library routine that does; it only
+ * enqueues kernels on `stream` and returns without synchronising.  The first call on each device looks up the array's
+ * device address (cudaGetSymbolAddress, with that device current) and sets the GEMM kernel's shared-memory attribute;
+ * make that first call during start-up, outside any stream capture.  Later calls on that device reuse the address.
+ *
+ * All calls on a device share the one array and it keeps whatever the previous call left: each call rewrites every word
+ * it later reads (partials, row metadata, the zeroed token / threshold rows), so calls that follow one another on one
+ * stream are independent, but two calls whose kernels may overlap on the GPU (different streams, no event between them)
+ * race on it and give garbage.  Serialise them, or use dlm_op_lmhead_bf16 with a scratch buffer per stream. */
+#define DLM_LMHEAD_STATIC_MAX_ROWS      128
+#define DLM_LMHEAD_STATIC_SCRATCH_BYTES (4 << 20)
+DLM_API int64_t dlm_op_lmhead_static_bytes(int32_t R, int32_t V);   /* bytes of the array a call with these sizes uses */
+DLM_API int dlm_op_lmhead_static_bf16(const void* hidden, const void* W_lm, int32_t R, int32_t V, int32_t K, float scale,
+                              int32_t mask_id, int32_t* tok, float* conf, float* lse, void* stream);
+
 /* Non-causal block attention over a contiguous (unpaged) K/V, bf16 (a5): q [Tq, H, d_h], k/v [S, H_kv, d_h]
  * -> out [Tq, H, d_h]; softmax_j(q.k_j/sqrt(d_h)) v_j over all j.  flash = 0: plain kernel; 1: mma.sync
  * online-softmax kernel; 2: tcgen05/TMEM kernel with the K/V split the engine would pick (the transposed-score variant when Tq * H / H_kv <= 64); 2 + s: the same

@@ -140,6 +140,9 @@ def lib() -> C.CDLL:
         L.dlm_op_lmhead_scratch_bytes.restype = i64
         L.dlm_op_lmhead_bf16.argtypes = [vp, vp, i32, i32, i32, f32, i32, vp, vp, vp, vp, vp]
         L.dlm_op_lmhead_unmask_bf16.argtypes = [vp, vp, i32, i32, i32, i32, f32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.dlm_op_lmhead_static_bytes.argtypes = [i32, i32]
+        L.dlm_op_lmhead_static_bytes.restype = i64
+        L.dlm_op_lmhead_static_bf16.argtypes = [vp, vp, i32, i32, i32, f32, i32, vp, vp, vp, vp]
         L.dlm_op_attention_bf16.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
         _lib = L
     return _lib
@@ -479,6 +482,28 @@ def op_lmhead_bf16(hidden, W_lm, scale: float, mask_id: int):
     scratch = torch.empty(lib().dlm_op_lmhead_scratch_bytes(R, V), device=hidden.device, dtype=torch.uint8)
     _op_check(lib().dlm_op_lmhead_bf16(hidden.data_ptr(), W_lm.data_ptr(), R, V, K, scale, mask_id, tok.data_ptr(),
                                        conf.data_ptr(), lse.data_ptr(), scratch.data_ptr(), _stream_ptr()))
+    return tok, conf, lse
+
+
+LMHEAD_STATIC_MAX_ROWS, LMHEAD_STATIC_SCRATCH_BYTES = 128, 4 << 20
+
+
+def op_lmhead_static_bf16(hidden, W_lm, scale: float, mask_id: int, outs=None):
+    """dlm_op_lmhead_static_bf16: the fused LM head for callers that cannot allocate device memory (a serving loop
+    whose HBM was all handed to a pool at start-up, a section that cannot take cudaMalloc's device-wide
+    synchronisation, a plug-in that is only given input and output buffers).  The scratch is an array inside libdlm.so,
+    LMHEAD_STATIC_SCRATCH_BYTES per GPU, shared by every call: at most LMHEAD_STATIC_MAX_ROWS rows, and calls whose
+    kernels could overlap on the GPU must be serialised by the caller.  Pass `outs` = (tok int32 [R], conf fp32 [R],
+    lse fp32 [R]) to make this wrapper allocation-free as well; without it the three outputs come from torch."""
+    import torch
+    R, K = hidden.shape
+    V = W_lm.shape[0]
+    if outs is None:
+        outs = (torch.empty(R, device=hidden.device, dtype=torch.int32), torch.empty(R, device=hidden.device, dtype=torch.float32),
+                torch.empty(R, device=hidden.device, dtype=torch.float32))
+    tok, conf, lse = outs
+    _op_check(lib().dlm_op_lmhead_static_bf16(hidden.data_ptr(), W_lm.data_ptr(), R, V, K, scale, mask_id, tok.data_ptr(),
+                                              conf.data_ptr(), lse.data_ptr(), _stream_ptr()))
     return tok, conf, lse
 
 

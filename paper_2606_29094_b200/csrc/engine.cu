@@ -2187,3 +2187,113 @@ extern "C" int dlm_op_attention_bf16(const void* q, const void* k, const void* v
   if (rc) return rc;
   return attn_op_contiguous(q, k, v, out, Tq, S, H, Hkv, dh, flash, (cudaStream_t)stream, &g_init_error);
 }
+
+// ------------------------------------------------------------------------------------------------
+// dlm_op_lmhead_static_bf16 (dlm_ops.h): the fused LM head for callers that cannot allocate device memory.
+// Its scratch is the file-scope array below, part of the module image: every GPU that loads libdlm.so holds
+// DLM_LMHEAD_STATIC_SCRATCH_BYTES for it until the process exits, and all calls on a device share it.
+// In host code the name `g_lmhead_static` is only the host-side handle of that array, not a device address: the
+// address comes from cudaGetSymbolAddress, looked up once per device with that device current.  Device code in this
+// file may name the array directly (lmhead_static_meta_kernel does).
+// Layout of one call's use (every region a multiple of 256 bytes):
+//   RowPartial part[R][n_tiles] | int slot[R] blk_lo[R] blk_len[R] row_off[R] | int n_committed[R] pos[R] tok[R]
+//   float conf[R] | int tokens[R] | float tau[R]
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_lmhead_static[DLM_LMHEAD_STATIC_SCRATCH_BYTES];
+
+static inline size_t static_align256(size_t b) { return (b + 255) & ~(size_t)255; }
+constexpr int kStaticHeadIntRows = 10;    // the ten R-long rows that follow the partials
+
+extern "C" int64_t dlm_op_lmhead_static_bytes(int32_t R, int32_t V) {
+  if (R <= 0 || V <= 0) return 0;
+  return (int64_t)(static_align256((size_t)R * ((V + 127) / 128) * sizeof(RowPartial)) + kStaticHeadIntRows * static_align256((size_t)R * 4));
+}
+
+// Row metadata of "R requests of one block row each" and the rows that have to start at zero (token ids: nothing is
+// masked, nothing committed from an earlier call; thresholds), rewritten by every call because the array keeps the
+// previous call's contents.  Names the array directly: in device code the symbol IS the device array.
+__global__ void lmhead_static_meta_kernel(long long meta_off, int R, int stride) {
+  int* meta = reinterpret_cast<int*>(g_lmhead_static + meta_off);
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= R) return;
+  meta[i] = i;                    // slot
+  meta[stride + i] = 0;           // blk_lo
+  meta[2 * stride + i] = 1;       // blk_len
+  meta[3 * stride + i] = i;       // row_off
+  meta[8 * stride + i] = 0;       // tokens
+  meta[9 * stride + i] = 0;       // tau = 0.0f
+}
+
+// Device address of g_lmhead_static on the current device; looked up on the first call per device.
+static int lmhead_static_base(unsigned char** base) {
+  static unsigned char* ptrs[kMaxDevices] = {};
+  const int d = g_dev;            // set by op_check_device() from cudaGetDevice()
+  if (!ptrs[d]) {
+    void* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_lmhead_static);
+    if (e != cudaSuccess || !p) {
+      cudaGetLastError();
+      set_err(&g_init_error, "dlm_op_lmhead_static_bf16: cudaGetSymbolAddress on device %d failed: %s", d, cudaGetErrorString(e));
+      return DLM_E_CUDA;
+    }
+    ptrs[d] = (unsigned char*)p;
+  }
+  *base = ptrs[d];
+  return DLM_OK;
+}
+
+extern "C" int dlm_op_lmhead_static_bf16(const void* hidden, const void* Wlm, int32_t R, int32_t V, int32_t K, float scale,
+                                          int32_t mask_id, int32_t* tok, float* conf, float* lse, void* stream) {
+  int rc = op_check_device();
+  if (rc) return rc;
+  if (!hidden || !Wlm || !tok || !conf || !lse || R <= 0 || V <= 0 || K <= 0 || K % 8) {
+    set_err(&g_init_error, "dlm_op_lmhead_static_bf16: bad arguments"); return DLM_E_ARG;
+  }
+  const long long need = dlm_op_lmhead_static_bytes(R, V);
+  if (R > DLM_LMHEAD_STATIC_MAX_ROWS || need > (long long)DLM_LMHEAD_STATIC_SCRATCH_BYTES) {
+    set_err(&g_init_error, "dlm_op_lmhead_static_bf16: R = %d rows x V = %d columns needs %lld bytes of scratch; the built-in array "
+            "holds %d bytes and at most %d rows (use dlm_op_lmhead_bf16 with a caller-owned scratch buffer)",
+            R, V, need, (int)DLM_LMHEAD_STATIC_SCRATCH_BYTES, (int)DLM_LMHEAD_STATIC_MAX_ROWS);
+    return DLM_E_CAPACITY;
+  }
+  unsigned char* base = nullptr;
+  if ((rc = lmhead_static_base(&base)) != DLM_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n_tiles = (V + 127) / 128;
+  const size_t meta_off = static_align256((size_t)R * n_tiles * sizeof(RowPartial));
+  const int stride = (int)(static_align256((size_t)R * 4) / 4);
+  RowPartial* part = (RowPartial*)base;
+  int* meta = (int*)(base + meta_off);
+
+  lmhead_static_meta_kernel<<<(R + 127) / 128, 128, 0, st>>>((long long)meta_off, R, stride);
+  DLM_LAUNCH_CHECK();
+
+  // the single-CTA-per-tile tcgen05 GEMM with the split-vocab epilogue, as op_head / gemm_tc set it up for R <= 128;
+  // tensor maps live on this stack frame (kernel parameters are copied at launch)
+  GemmTcParams p = {};
+  p.M = R; p.N = V; p.K = K; p.bn = 128;
+  p.a_box_rows = R <= 32 ? 32 : (R <= 64 ? 64 : 128);
+  const int num_kb = (K + kBK - 1) / kBK;
+  p.stages = std::max(2, std::min(std::min(num_kb, 12), (200 * 1024) / gemm_tc_stage_bytes(128)));
+  p.w_policy = DLM_L2_EVICT_FIRST;
+  p.part = part; p.n_tiles = n_tiles; p.mask_id = mask_id; p.scale = scale;
+  CUtensorMap ma, mb;
+  if (!make_tmap_bf16(&ma, hidden, R, K, p.a_box_rows) || !make_tmap_bf16(&mb, Wlm, V, K, 128)) {
+    set_err(&g_init_error, "dlm_op_lmhead_static_bf16: cuTensorMapEncodeTiled failed"); return DLM_E_CUDA;
+  }
+  cudaError_t e = launch_gemm_tc_t<EPI_LMHEAD>(&ma, &mb, p, n_tiles, st, false);
+  if (e != cudaSuccess) { set_err(&g_init_error, "dlm_op_lmhead_static_bf16: launch failed: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+
+  // every row is its own request of one block row; the commit lists go to the array and are dropped (dry run)
+  StepOut so;
+  so.n_committed = meta + 4 * stride; so.pos = meta + 5 * stride; so.tok = meta + 6 * stride; so.conf = (float*)(meta + 7 * stride);
+  so.row_lse = lse; so.row_conf = conf; so.row_tok = tok;
+  BatchDesc bd = {};
+  bd.n = R; bd.R = R; bd.slot = meta; bd.blk_lo = meta + stride; bd.blk_len = meta + 2 * stride; bd.row_off = meta + 3 * stride;
+  bd.tau = (const float*)(meta + 9 * stride);
+  combine_unmask_kernel<<<R, 1024, 0, st>>>(so, part, n_tiles, meta + 8 * stride, 1, 1, mask_id, bd, 1);
+  DLM_LAUNCH_CHECK();
+  e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err(&g_init_error, "dlm_op_lmhead_static_bf16: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
+  return DLM_OK;
+}
