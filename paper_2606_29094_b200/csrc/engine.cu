@@ -44,6 +44,31 @@ static void set_err(std::string* dst, const char* fmt, ...) {
 
 // One launch path for every kernel of a step: a plain launch, or a programmatic dependent launch (PDL) whose
 // prologue (and, for the GEMMs, weight prefetch) overlaps the tail of the previous kernel in the stream.
+// launch_k_attr: the same with an optional cooperative launch (all CTAs co-resident, or the launch fails instead of hanging).
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k_attr(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, bool coop, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  int na = 0;
+  if (pdl) {
+    at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
+  if (coop) {
+    at[na].id = cudaLaunchAttributeCooperative;
+    at[na].val.cooperative = 1;
+    ++na;
+  }
+  if (na) { cfg.attrs = at; cfg.numAttrs = na; }
+  g_launches++;
+  if constexpr (sizeof...(Args) + 1 == sizeof...(KArgs))       // caller left out the trailing TraceSlot: tracing off for this launch
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)..., TraceSlot{nullptr});
+  else
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+
 template <typename... KArgs, typename... Args>
 static cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, Args&&... args) {
   cudaLaunchConfig_t cfg = {};
@@ -769,19 +794,21 @@ struct KScope {
 
 // Every entry point that takes a ctx binds the calling thread to the context's device for the duration of the call (a
 // request may be imported into a context on another GPU of the same process) and credits its launches to the context.
+static thread_local int g_guard_depth = 0;   // entry points nest (dlm_profile_step_costs_ex -> dlm_refresh_step -> run_step)
 struct DevGuard {
   dlm_ctx* c;
   int prev = -1;
   long long l0;
   explicit DevGuard(dlm_ctx* c_) : c(c_), l0(g_launches) {
     if (!c) return;
+    ++g_guard_depth;
     cudaGetDevice(&prev);
     if (prev != c->device) cudaSetDevice(c->device);
     g_dev = c->device; g_num_sms = c->num_sms;
   }
   ~DevGuard() {
     if (!c) return;
-    c->launches += g_launches - l0;
+    if (--g_guard_depth == 0) c->launches += g_launches - l0;      // only the outermost guard credits the launches (once)
     if (prev >= 0 && prev != c->device) cudaSetDevice(prev);
   }
 };
@@ -1054,7 +1081,7 @@ extern "C" int dlm_step_trace(dlm_ctx* c, dlm_trace_row* rows, int32_t cap, int3
 }
 
 extern "C" int dlm_layer_kernel_phases(dlm_ctx* c, float* usec, int32_t cap) {
-  if (!c || !usec || !c->mega_ts) return DLM_E_ARG;
+  if (!c || !usec || cap <= 0 || !c->mega_ts) return DLM_E_ARG;
   DevGuard dev_guard(c);
   const int n = std::min<int>(cap, kMgPhasesPerLayer * c->a.n_layers + 1);
   std::vector<unsigned long long> h(n);
@@ -1079,7 +1106,19 @@ extern "C" int dlm_set_option(dlm_ctx* c, int32_t key, int32_t value) {
     case DLM_OPT_TRACE: c->opt_trace = value != 0; return DLM_OK;
     case DLM_OPT_LAYER_KERNEL: c->opt_mega = value != 0; return DLM_OK;
     case DLM_OPT_LAYER_KERNEL_PHASE_TS: c->opt_mega_ts = value != 0; return DLM_OK;
-    case DLM_OPT_TCT_MIN_ITEMS: c->opt_tct_min_items = std::max(1, value); return DLM_OK;
+    case DLM_OPT_TCT_MIN_ITEMS: {
+      // selects the attention kernel a step enqueues but is not part of the graph key: a captured graph of the old selection
+      // must not be replayed (an A/B timing on one context would measure the same kernel twice)
+      const int v = std::max(1, value);
+      if (v != c->opt_tct_min_items) {
+        DevGuard dev_guard(c);
+        if (c->st) cudaStreamSynchronize(c->st);
+        for (auto& g : c->graphs) if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
+        c->graphs.clear();
+      }
+      c->opt_tct_min_items = v;
+      return DLM_OK;
+    }
   }
   set_err(&c->err, "unknown option %d", key);
   return DLM_E_ARG;
@@ -1371,6 +1410,22 @@ static int gemm_big_resid(dlm_ctx* c, const void* A, const void* W, int M, int N
 }
 
 // Whole-stack persistent kernel (layer_mega.cuh): can this step take it?
+// The whole-stack kernel synchronises its CTAs through a grid-wide counter, so every CTA must be resident at once: it is launched
+// cooperatively (the driver refuses the launch instead of letting waiting CTAs spin when the grid does not fit beside other
+// work), and a device on which one CTA per SM does not fit never takes this path.
+static bool mega_configure(int tpad, int stages) {
+  static int state[kMaxDevices] = {};           // 0 unknown, 1 usable, -1 not
+  if (!state[g_dev]) {
+    int coop = 0, nb = 0;
+    bool ok = cudaFuncSetAttribute(layer_mega_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess &&
+              cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, g_dev) == cudaSuccess && coop &&
+              cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, layer_mega_kernel, kMgThreads, (size_t)mega_smem_bytes(tpad, stages)) == cudaSuccess && nb >= 1;
+    if (!ok) cudaGetLastError();
+    state[g_dev] = ok ? 1 : -1;
+  }
+  return state[g_dev] > 0;
+}
+
 static bool mega_ok(const dlm_ctx* c, const BatchDesc& bd) {
   const dlm_arch& a = c->a;
   if (!c->bf16_model || c->opt_simple || !c->opt_mega || !c->opt_skinny || !c->w_tiled || !c->mega_wmaps) return false;
@@ -1383,7 +1438,13 @@ static bool mega_ok(const dlm_ctx* c, const BatchDesc& bd) {
   const int G = g_num_sms, d = a.d_model, F = a.d_ffn, HQ = a.n_heads * a.head_dim;
   auto max_seg = [&](long long n_tiles, long long kbt) { const long long U = n_tiles * kbt; return (int)((kbt * G + U - 1) / U) + 1; };
   if (max_seg(NQKV / 128, d / 64) > kMgMaxSegQkv || max_seg(F / 64, d / 64) > kMgMaxSegGu || max_seg(d / 128, HQ / 64) > kMgMaxSeg || max_seg(d / 128, F / 64) > kMgMaxSeg) return false;
-  return true;
+  // what mega_launch would refuse: the shared-memory plan and the slice buffers -- such a step takes the per-stage kernels instead
+  const int tpad = (bd.T + 31) / 32 * 32, stages = mega_stages(tpad);
+  if (stages < 2 || stages * (tpad * 128) + kMgScratchOwn < kMgAttnBytes) return false;
+  const long long need_a = std::max<long long>((long long)max_seg(NQKV / 128, d / 64) * bd.T * NQKV, (long long)max_seg(F / 64, d / 64) * bd.T * 2 * F);
+  const long long need_x = (long long)std::max(max_seg(d / 128, HQ / 64), max_seg(d / 128, F / 64)) * bd.T * d;
+  if (need_a > c->qkv_rows * (long long)NQKV || need_x > c->part_rows * (long long)d) return false;
+  return mega_configure(tpad, stages);
 }
 
 static int mega_launch(dlm_ctx* c, const BatchDesc& bd, int layer0, int n_layers, bool dump, bool pdl) {
@@ -1425,14 +1486,9 @@ static int mega_launch(dlm_ctx* c, const BatchDesc& bd, int layer0, int n_layers
   const CUtensorMap* mat = c->tmaps.get(c->attn, c->Tmax, HQ, p.tpad);
   const CUtensorMap* mac = c->tmaps.get(c->act, c->Tmax, F, p.tpad);
   if (!mu || !mu2 || !mat || !mac) { set_err(&c->err, "cuTensorMapEncodeTiled failed (layer kernel activations)"); return DLM_E_CUDA; }
-  static bool configured[kMaxDevices] = {};
-  if (!configured[g_dev]) {
-    cudaError_t e = cudaFuncSetAttribute(layer_mega_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    if (e != cudaSuccess) { set_err(&c->err, "layer kernel: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
-    configured[g_dev] = true;
-  }
+  if (!mega_configure(p.tpad, p.stages)) { set_err(&c->err, "layer kernel: one CTA per SM does not fit on this device (or no cooperative launch)"); return DLM_E_CUDA; }
   CU_TRY(&c->err, cudaMemsetAsync(c->mega_bar, 0, 4096, c->st));
-  cudaError_t e = launch_k(layer_mega_kernel, dim3(G), dim3(kMgThreads), (size_t)mega_smem_bytes(p.tpad, p.stages), c->st, pdl, *mu, *mu2, *mat, *mac, p);
+  cudaError_t e = launch_k_attr(layer_mega_kernel, dim3(G), dim3(kMgThreads), (size_t)mega_smem_bytes(p.tpad, p.stages), c->st, pdl, /*coop=*/true, *mu, *mu2, *mat, *mac, p);
   if (e != cudaSuccess) { set_err(&c->err, "layer kernel launch: %s", cudaGetErrorString(e)); return DLM_E_CUDA; }
   c->paths |= DLM_PATH_LAYER_KERNEL;
   return DLM_OK;
@@ -1536,20 +1592,22 @@ static int forward(dlm_ctx* c, const BatchDesc& bd, bool dry_run) {
     bool flash_done = false;
     if (tc && c->opt_flash && c->opt_tcattn) {
       KScope ks(c, DLM_K_ATTENTION);
+      const size_t trace_mark = c->trace_cls.size();
       const TraceSlot tr3[3] = {c->tslot(), c->tslot(), c->tslot()};
       int rc = attn_tc_launch(c->tmaps, (bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, a.n_layers, c->page_table, bd, c->kg, l,
                               a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, st, pdl, err, &flash_done, 0, tr3, &c->paths, c->opt_tct_min_items);
       if (rc) return rc;
-      if (!flash_done && c->opt_trace) c->trace_cls.resize(c->trace_cls.size() - 3);      // nothing launched: give the records back
+      if (!flash_done) c->trace_cls.resize(trace_mark);      // nothing launched: give back the records taken (none once the table is full)
     }
     if (tc && c->opt_flash && !flash_done) {
       KScope ks(c, DLM_K_ATTENTION);
+      const size_t trace_mark = c->trace_cls.size();
       const TraceSlot t0 = c->tslot(), t1 = c->tslot();
       int rc = attn_flash_launch((bf16*)c->attn, (const bf16*)c->q, (const bf16*)c->kv_store, c->page_table, bd, c->kg, l,
                                  a.n_heads, scale, &c->attn_ws, &c->attn_ws_bytes, g_num_sms, st, pdl, err, &flash_done, t0, t1);
       if (rc) return rc;
       if (flash_done) c->paths |= DLM_PATH_ATTN_FLASH;
-      else if (c->opt_trace) c->trace_cls.resize(c->trace_cls.size() - 2);
+      else c->trace_cls.resize(trace_mark);
     }
     if (!flash_done) {
       KScope ks(c, DLM_K_ATTENTION);
