@@ -82,6 +82,16 @@ def roofline_ms(work, peaks, sustained=True):
     return 1e3 * max(t_f, t_b), ("tensor" if t_f > t_b else "hbm")
 
 
+def burst_applies(clocks):
+    """Which tensor peak a tensor-bound step is scored against: the BURST figure when the sampled SM clock stayed within 5 % of
+    its maximum and no power cap was seen during the timed region (a step that runs at full clock between HBM-bound steps),
+    else the SUSTAINED one (seconds of back-to-back GEMMs under sw_power_cap).  HBM-bound steps do not depend on it."""
+    mhz, mx = clocks.get("sm_mhz"), clocks.get("sm_max_mhz")
+    if not mhz or not mx:
+        return False
+    return mhz >= 0.95 * mx and "sw_power_cap" not in clocks.get("reasons", [])
+
+
 # ---------------------------------------------------------------------------------------------------------
 # clocks during the timed region
 # ---------------------------------------------------------------------------------------------------------
@@ -164,6 +174,10 @@ class Runner:
         self.ids = [None] * len(specs)
         self.h2d = 0
         self.d2h = 0
+        # host-side mirror of what the scheduler knows about each request (it decides the step kind from the tokens it was
+        # sent back): MASK positions left in total and in the current block, and whether the cache it built is still valid --
+        # no dlm_request_info round trip per request and step
+        self.left, self.blk_left, self.valid = [0] * len(specs), [0] * len(specs), [False] * len(specs)
         for i in range(len(specs)):
             self._add(i)
 
@@ -176,18 +190,24 @@ class Runner:
         if s.filled is not None and len(s.filled):
             self.eng.set_tokens(self.ids[i], initial_tokens(s, self.arch.mask_id))
             self.h2d += 4 * (len(s.prompt) + s.gen_len)
+        self._sync_state(i)
+
+    def _sync_state(self, i):
+        """Mirror of request i from the library (at submission, and if the mirror is ever contradicted)."""
+        s = self.specs[i]
+        st = self.eng.info(self.ids[i])
+        self.left[i], self.valid[i] = st["n_masked"], st["cache_valid"]
+        lo = len(s.prompt) + st["cur_block"] * s.block_len
+        self.blk_left[i] = int((self.eng.tokens(self.ids[i])[lo:lo + s.block_len] == self.arch.mask_id).sum()) if st["n_masked"] else 0
 
     def step(self):
         """One denoising step of the whole batch.  Returns (device_usec, commits, n_refresh_reqs, n_cached_reqs, work)."""
         eng = self.eng
         refresh, cached = [], []
-        for i, rid in enumerate(self.ids):
-            st = eng.info(rid)
-            if st["n_masked"] == 0:             # finished: the client submits it again (prompt upload inside the region)
+        for i in range(len(self.ids)):
+            if self.left[i] == 0:               # finished: the client submits it again (prompt upload inside the region)
                 self._add(i)
-                rid = self.ids[i]
-                st = eng.info(rid)
-            (cached if st["cache_valid"] else refresh).append(i)
+            (cached if self.valid[i] else refresh).append(i)
         usec, commits = 0.0, 0
         q_lens, kv_lens, rows = [], [], 0
         if refresh and cached and self.mixed_launch:
@@ -202,6 +222,12 @@ class Runner:
             g = eng.refresh_step(rids) if kind == "refresh" else (eng.cached_step(rids) if kind == "cached" else eng.mixed_step(rids))
             usec += g.usec
             commits += g.total
+            for j, i in enumerate(idx):         # the block completes when its last MASK goes: the next step of it is a recompute step
+                self.left[i] = int(g.n_masked_left[j])
+                self.blk_left[i] -= int(g.n_committed[j])
+                self.valid[i] = self.blk_left[i] > 0
+                if self.blk_left[i] <= 0:
+                    self.blk_left[i] = min(self.specs[i].block_len, self.left[i])
             self.h2d += 4 * (10 * len(rids) + sum((len(self.specs[i].prompt) + self.specs[i].gen_len) if (kind == "refresh" or (kind == "mixed" and i in is_ref))
                                                    else self.specs[i].block_len for i in idx))
             self.d2h += 4 * (len(self.specs) + 6 * len(self.specs) * self.max_block)
@@ -400,11 +426,49 @@ def job_value(world, steps, dev_us):
     return world * steps / (dev_us * 1e-6)
 
 
+def kind_roofline(rs, peaks, burst):
+    """Measured time of the steps `rs` (one step kind) against the sum of their rooflines.  `frac` uses the tensor peak that
+    applies to the run (burst_applies); frac_burst / frac_sustained give both, they differ only for tensor-bound steps."""
+    n = len(rs)
+    t_meas = sum(r["us"] for r in rs) * 1e-3
+    roofs = {sus: [roofline_ms(r["work"], peaks, sustained=sus) for r in rs] for sus in (True, False)}
+    t_sus, t_bur = sum(x[0] for x in roofs[True]), sum(x[0] for x in roofs[False])
+    used = roofs[not burst]
+    bounds = sorted({x[1] for x in used})
+    t_roof = t_bur if burst else t_sus
+    return {"n": n, "ms": t_meas / n, "ms_min": min(r["us"] for r in rs) * 1e-3, "roofline_ms": t_roof / n,
+            "bound": bounds[0] if len(bounds) == 1 else "mixed", "frac": t_roof / t_meas, "frac_burst": t_bur / t_meas, "frac_sustained": t_sus / t_meas,
+            "tensor_peak_used": "burst" if burst else "sustained",
+            "gflop": sum(r["work"]["flops"] for r in rs) / n * 1e-9, "gbytes": sum(r["work"]["bytes"] for r in rs) / n * 1e-9}
+
+
+def other_workload(pkg, name, steps, warm, peaks, clk_index):
+    """A short run of another BASELINE.json config inside the default line: `steps` timed steps after `warm`
+    untimed ones, per step kind the measured ms against the step's roofline, with the run's own clock record."""
+    arch, seed, specs, desc = get_workload(name)
+    run = Runner(pkg, arch, seed, specs)
+    try:
+        for _ in range(warm):
+            run.step()
+        recs, wall, clocks = timed_steps(run, steps, clk_index)
+    finally:
+        run.close()
+    burst = burst_applies(clocks)
+    us = sum(r["us"] for r in recs)
+    kinds = {}
+    for kind in ("refresh", "cached", "mixed"):
+        rs = [r for r in recs if r["kind"] == kind]
+        if rs:
+            kinds[kind] = kind_roofline(rs, peaks, burst)
+    return {"workload": desc, "steps": steps, "warmup": warm, "ms_per_step": us / steps * 1e-3, "steps_per_s": steps / (us * 1e-6),
+            "e2e_steps_per_s": steps / wall, "committed_tokens_per_s": sum(r["commits"] for r in recs) / (us * 1e-6),
+            "frac": sum(roofline_ms(r["work"], peaks, sustained=not burst)[0] for r in recs) / (us * 1e-3), "step_roofline": kinds, "clocks": clocks}
+
+
 # ---------------------------------------------------------------------------------------------------------
 def at_block_boundary(run):
     """True when the step that is due opens a block for the workload's first request (its K/V cache is not valid)."""
-    st = run.eng.info(run.ids[0])
-    return st["n_masked"] == 0 or not st["cache_valid"]
+    return run.left[0] == 0 or not run.valid[0]
 
 
 def timed_steps(run, K, clk_index):
@@ -432,6 +496,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-pass", action="store_true")
+    ap.add_argument("--no-other-workloads", action="store_true", help="C2 only: skip the short C4 / C3 / C5 runs the default line appends")
     ap.add_argument("--micro", default=None, choices=["lmhead"], help="isolated micro-benchmark instead of the step benchmark")
     ap.add_argument("--cost-table", action="store_true", help="print dlm_profile_step_costs for the workload's architecture")
     ap.add_argument("--two-call", action="store_true", help="mixed iterations as dlm_refresh_step + dlm_cached_step instead of one dlm_mixed_step")
@@ -505,28 +570,25 @@ def main():
            "gpu_launches": int(launches), "clocks": clocks}
     # ---- per step kind: measured vs the step's roofline (north_star: >= 60 %); work summed step by step ----
     steps_rf = {}
+    burst = burst_applies(clocks)
     for kind in ("refresh", "cached", "mixed"):
         rs = [r for r in recs if r["kind"] == kind]
         if not rs:
             continue
-        roofs = [roofline_ms(r["work"], peaks) for r in rs]
-        t_meas, t_roof = sum(r["us"] for r in rs) * 1e-3, sum(x[0] for x in roofs)
-        bounds = sorted({x[1] for x in roofs})
-        steps_rf[kind] = {"n": len(rs), "ms": t_meas / len(rs), "ms_min": min(r["us"] for r in rs) * 1e-3, "roofline_ms": t_roof / len(rs),
-                          "bound": bounds[0] if len(bounds) == 1 else "mixed", "frac": t_roof / t_meas,
-                          "gflop": sum(r["work"]["flops"] for r in rs) / len(rs) * 1e-9, "gbytes": sum(r["work"]["bytes"] for r in rs) / len(rs) * 1e-9}
+        steps_rf[kind] = kind_roofline(rs, peaks, burst)
     if "refresh" in steps_rf and "cached" in steps_rf and n_req == 1:
         Bk = specs[0].block_len                    # the block cycle of P:582: one recompute step + B - 1 cache steps
         t_cyc = steps_rf["refresh"]["ms"] + (Bk - 1) * steps_rf["cached"]["ms"]
         r_cyc = steps_rf["refresh"]["roofline_ms"] + (Bk - 1) * steps_rf["cached"]["roofline_ms"]
         steps_rf["block_cycle"] = {"steps": Bk, "ms": t_cyc / Bk, "steps_per_s": 1e3 * Bk / t_cyc, "roofline_ms": r_cyc / Bk, "frac": r_cyc / t_cyc}
     out["step_roofline"] = steps_rf
-    out["roofline_frac_all_steps"] = sum(roofline_ms(r["work"], peaks)[0] for r in recs) / (sum(r["us"] for r in recs) * 1e-3)
+    out["roofline_frac_all_steps"] = sum(roofline_ms(r["work"], peaks, sustained=not burst)[0] for r in recs) / (sum(r["us"] for r in recs) * 1e-3)
+    out["tensor_peak_used"] = "burst" if burst else "sustained"
     out["peaks"] = peaks
 
     # ---- dominant kernel class, timed inside the production launch by the in-kernel trace ----
     if rank == 0 and not args.no_kernel_pass:
-        out["roofline"], out["kernels"] = trace_pass(run, pkg, arch, peaks)
+        out["roofline"], out["kernels"] = trace_pass(run, pkg, arch, peaks, burst=burst)
     if rank == 0 and args.trace_rows > 0:
         out["trace_rows"] = trace_rows(run, pkg, args.trace_rows)
     if rank == 0 and args.layer_kernel:
@@ -534,6 +596,14 @@ def main():
         out["config"]["layer_kernel"] = True
     if rank == 0 and args.tau_sweep:
         out["tau_sweep"] = tau_sweep(pkg, arch, seed, specs, not args.two_call)
+    if rank == 0 and world == 1 and args.workload == "C2" and not args.no_other_workloads:
+        run.close()                                  # one model in HBM at a time
+        out["other_workloads"] = {}
+        for name, k in (("C4", 8), ("C3", 6), ("C5", 6)):
+            try:
+                out["other_workloads"][name] = other_workload(pkg, name, k, 3, peaks, local)
+            except Exception as e:                   # never take the headline down
+                out["other_workloads"][name] = {"failed": repr(e)}
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         try:
             out["cpu_baseline"] = cpu_baseline(arch, seed, specs, mix=(mix["refresh_request_steps"], mix["cached_request_steps"]))
@@ -602,7 +672,7 @@ def layer_kernel_phases(run, pkg, arch):
     return {n: round(float(d[:, j].mean()), 2) for j, n in enumerate(names)} | {"layer_total": round(float(d.sum(1).mean()), 2)}
 
 
-def trace_pass(run, pkg, arch, peaks, n_steps=12):
+def trace_pass(run, pkg, arch, peaks, n_steps=12, burst=False):
     """A few more steps of the same run with DLM_OPT_TRACE: every kernel stamps %globaltimer inside the production launch
     (CUDA graph + programmatic dependent launch; overhead < 1 %).  A launch holds the step's critical path from the moment
     its griddepcontrol.wait returns (the launch before it has completed) until the next launch's wait returns, so the
@@ -654,13 +724,23 @@ def trace_pass(run, pkg, arch, peaks, n_steps=12):
     t_b = w["weight_bytes"] / (peaks["hbm_gbs"] * 1e9)
     t_f = w["flops_linear"] / (peaks["bf16_tflops_sustained"] * 1e12)
     if t_b >= t_f:
-        ach = w["weight_bytes"] / (g_us * 1e-6) * 1e-9
+        # A weight-streaming launch fills its shared-memory rings BEFORE its griddepcontrol.wait returns (weights do not depend on
+        # the upstream kernel): gemm_skinny.cuh keeps 2 CTAs x 5 stages x 16 KB of W per SM, i.e. up to 2 x 148 x 80 KB = 23.7 MB per
+        # launch move while the previous kernel still holds the critical path.  `achieved` leaves those bytes out of the class's
+        # account (they were not moved in the time the class is charged); the figure with them in is an upper bound, kept as
+        # achieved_critical_path.  The whole-step number (step_roofline) needs no such correction.
+        prefill = min(w["weight_bytes"] / g_launch, 2 * 148 * 5 * 16384) if T <= 128 else 0.0
+        ach_cp = w["weight_bytes"] / (g_us * 1e-6) * 1e-9
+        ach = (w["weight_bytes"] - g_launch * prefill) / (g_us * 1e-6) * 1e-9
         rf = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+              "achieved_critical_path": ach_cp, "frac_critical_path": ach_cp / peaks["hbm_gbs"], "ring_prefill_bytes_per_launch": prefill,
               "algorithmic_bytes_per_launch": w["weight_bytes"] / g_launch}
     else:
         ach = w["flops_linear"] / (g_us * 1e-6) * 1e-12
-        rf = {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"],
-              "algorithmic_flops_per_launch": w["flops_linear"] / g_launch}
+        pk = peaks["bf16_tflops" if burst else "bf16_tflops_sustained"]
+        rf = {"bound": "tensor", "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
+              "frac_burst": ach / peaks["bf16_tflops"], "frac_sustained": ach / peaks["bf16_tflops_sustained"],
+              "tensor_peak_used": "burst" if burst else "sustained", "algorithmic_flops_per_launch": w["flops_linear"] / g_launch}
     rf.update({"traffic": None, "traffic_note": "dram bytes are not measured by this run; the ncu --set full capture of the same command is under profiles/",
                "kernel": ("gemm_pair_kernel (CTA-pair tcgen05 GEMM: QKV+RoPE, O, gate/up+SwiGLU, down, LM head)" if T > 128 else
                           "gemm_skinny_kernel (QKV, O, gate/up+SwiGLU, down) + gemm_tc_kernel<LM head>: the weight-streaming GEMMs") + f" inside {want} steps",
